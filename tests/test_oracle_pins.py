@@ -1,0 +1,349 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU needed).
+
+The paper prints no field values, so the oracle is pinned by:
+  P1  computer-algebra substitution of Psi = e^{im phi~} r^3 Phi into PAPER.md:68-76 (Eq. 1),
+      done here with sympy, plus the stored Table C values and the tortoise inversion;
+  P2  second-order self-convergence (PAPER.md:88 "second-order Lax-Wendroff", :102);
+  P3  Schwarzschild l = 2 quasinormal frequency 0.3737 - 0.0890i (BASELINE.json north_star),
+      for even and odd m (both pole-parity branches of PAPER.md:104);
+  P3b Kerr a = 0.9, l = m = 2: 0.6716 - 0.0649i (textbook, Berti et al. tables);
+  P4  (m, theta) -> (-m, pi - theta) reflection with complex conjugation;
+  P5  a = 0 keeps real data exactly real;
+  P6  linearity / exact power-of-two scaling / zero stays zero;
+  P7  unit norm, support and time-level placement of the Gaussian deposit.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from paper_1206_0270_b200 import workloads as wl
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+# ------------------------------------------------------------------------------------------ P1
+def _table_c():
+    rows = []
+    for line in open(os.path.join(GOLDEN, "table_c.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        left, right = line.split("|")
+        a, m, r, th = left.split()
+        v = [float(t) for t in right.split()]
+        rows.append((float(a), int(m), float(r), float(th), v))
+    return rows
+
+
+def test_p1_table_c(orc):
+    """Stored CAS values of Eq. (1)'s reduction (SURVEY.md 8(c) Table C)."""
+    for a, m, r, th, v in _table_c():
+        c = orc.coefficients(1.0, a, m, v[0], th)
+        got = [c["b"], c["bx"], c["kappa"].real, c["kappa"].imag, c["alpha"].real, c["alpha"].imag,
+               c["gamma"].real, c["gamma"].imag, c["cL"]]
+        assert abs(c["r"] - r) < 1e-12 * r
+        for g, e in zip(got, v[1:]):
+            assert abs(g - e) <= 5e-13 * max(1.0, abs(e)) and abs(g - e) <= 2e-11 * max(abs(e), 1e-3), (a, m, r, g, e)
+
+
+@pytest.mark.parametrize("a_num,a_den,m,r_val,th_val", [
+    (9, 10, 2, "3", "1.0471975511965976"),
+    (99, 100, 2, "3/2", "1/10"),
+    (7, 10, 4, "10", "3"),
+    (0, 1, 2, "3", "1.5707963267948966"),
+    (9, 10, -3, "2.2", "2.5"),
+    (99, 100, 1, "1.1510", "0.7"),   # close to the horizon r+ = 1.14107
+    (7, 10, 0, "40", "1.2"),
+])
+def test_p1_cas_substitution(orc, a_num, a_den, m, r_val, th_val):
+    """Brute force: apply the operator of PAPER.md:68-76 (Eq. 1) to
+    Psi = e^{i m phi~(r)} r^3 F(t, x(r), theta) for seven monomial F with sympy and read off every
+    coefficient of  F_tt = b^2 F_xx + beta F_x + alpha F_t + gamma F + cL (F_thth + cot F_th)."""
+    sp = pytest.importorskip("sympy")
+    t, r, th, ph, X = sp.symbols("t r theta phi X", real=True)
+    M = sp.Integer(1)
+    a = sp.Rational(a_num, a_den)
+    s = -2
+    rp = M + sp.sqrt(M * M - a * a)
+    rm = M - sp.sqrt(M * M - a * a)
+    Delta = r * r - 2 * M * r + a * a
+    R2 = r * r + a * a
+    Sig2 = R2 ** 2 - a * a * Delta * sp.sin(th) ** 2
+    xr = r + 2 * M * rp / (rp - rm) * sp.log((r - rp) / (2 * M))
+    pht = ph
+    if a != 0:
+        xr = xr - 2 * M * rm / (rp - rm) * sp.log((r - rm) / (2 * M))
+        pht = ph + a / (rp - rm) * sp.log((r - rp) / (r - rm))
+    point = {r: sp.Rational(r_val) if "/" in r_val else sp.Float(r_val, 40),
+             th: sp.Rational(th_val) if "/" in th_val else sp.Float(th_val, 40),
+             t: sp.Rational(7, 10), ph: sp.Rational(3, 10)}
+
+    def eq1_lhs(Psi):
+        sn, cs = sp.sin(th), sp.cos(th)
+        return (-(R2 ** 2 / Delta - a * a * sn ** 2) * sp.diff(Psi, t, 2)
+                - 4 * M * a * r / Delta * sp.diff(Psi, t, ph)
+                - 2 * s * (r - M * (r * r - a * a) / Delta + sp.I * a * cs) * sp.diff(Psi, t)
+                + Delta ** (-s) * sp.diff(Delta ** (s + 1) * sp.diff(Psi, r), r)
+                + sp.diff(sn * sp.diff(Psi, th), th) / sn
+                + (1 / sn ** 2 - a * a / Delta) * sp.diff(Psi, ph, 2)
+                + 2 * s * (a * (r - M) / Delta + sp.I * cs / sn ** 2) * sp.diff(Psi, ph)
+                - (s * s * cs ** 2 / sn ** 2 - s) * Psi)
+
+    def reduced(F):  # value of [F_tt - (b^2 F_xx + ...)] implied by Eq. (1)
+        Psi = sp.exp(sp.I * m * pht) * r ** 3 * F.subs(X, xr)
+        v = eq1_lhs(Psi) / (-(Sig2 / Delta) * r ** 3 * sp.exp(sp.I * m * pht))
+        return complex(sp.N(v.subs(point), 30))
+
+    tv = float(point[t])
+    thv = float(point[th])
+    xv = float(sp.N(xr.subs(point), 30))
+    v1 = reduced(sp.Integer(1) + 0 * X)
+    gamma = -v1
+    alpha = -reduced(t + 0 * X) - gamma * tv
+    norm = reduced(t * t / 2 + 0 * X) + alpha * tv + gamma * tv * tv / 2
+    beta = -reduced(X) - gamma * xv
+    b2 = -reduced(X * X / 2) - beta * xv - gamma * xv * xv / 2
+    cot_term = -reduced(th + 0 * X) - gamma * thv           # = cL cot(theta)
+    cL_a = (-reduced(th * th / 2 + 0 * X) - gamma * thv * thv / 2) / (1 + thv / math.tan(thv))
+    b_sym = R2 / sp.sqrt(Sig2)
+    bx = float(sp.N((Delta / R2 * sp.diff(b_sym, r)).subs(point), 30))
+    assert abs(norm - 1) < 1e-13            # the F_tt coefficient of Eq. (1) is -Sigma^2/Delta
+    assert abs(b2.imag) < 1e-13 and abs(cot_term - cL_a / math.tan(thv)) < 1e-12 * abs(cL_a) + 1e-15
+
+    c = orc.coefficients(1.0, float(a), m, xv, thv)
+
+    def close(got, exp, what):
+        tol = 2e-11 * max(abs(exp), 1e-3)
+        assert abs(got - exp) <= tol, (what, got, exp)
+
+    close(c["r"], float(point[r]), "r(x)")
+    close(c["b"] ** 2, b2.real, "b^2")
+    close(c["cL"], cL_a.real, "cL")
+    close(c["alpha"], alpha, "alpha")
+    close(c["beta"], beta, "beta")
+    close(c["gamma"], gamma, "gamma")
+    close(c["bx"], bx, "b_x")
+    b = math.sqrt(b2.real)
+    close(c["kappa"], beta - alpha * b - b * bx, "kappa = beta - alpha b - b b_x")
+
+
+@pytest.mark.parametrize("a", [0.0, 0.7, 0.9, 0.99])
+def test_p1_tortoise_inversion(orc, a):
+    """r(x) against a 40-digit root of the closed-form tortoise map; Delta from delta = r - r+
+    stays accurate where r - r+ is far below one ulp of r."""
+    mp = pytest.importorskip("mpmath")
+    mp.mp.dps = 60
+    M = mp.mpf(1)
+    am = mp.mpf(a)
+    rp = M + mp.sqrt(M * M - am * am)
+    rm = M - mp.sqrt(M * M - am * am)
+    cp = 2 * M * rp / (rp - rm)
+    cm = 2 * M * rm / (rp - rm)
+    for x in [-200.0, -100.0, -50.0, -20.0, -5.0, 0.0, 1.93503434588429, 7.5, 50.0, 400.0, 1800.0]:
+        # unknown y = ln(r - r+), exact in multiprecision
+        f = lambda y: rp + mp.e ** y + cp * (y - mp.log(2 * M)) - (cm * mp.log((mp.e ** y + rp - rm) / (2 * M)) if a else 0) - x
+        y0 = (mp.mpf(x) - rp) / cp + mp.log(2 * M) if x < 2 * float(rp) else mp.log(x)
+        y = mp.findroot(f, y0)
+        d = mp.e ** y
+        r_ref, D_ref = rp + d, d * (d + rp - rm)
+        r, delta, Delta = orc.r_of_rstar(1.0, a, x)
+        assert abs(r - float(r_ref)) <= 4e-15 * float(r_ref) + 1e-13 * (x > 100)
+        assert abs(delta - float(d)) <= 1e-12 * float(d)
+        assert abs(Delta - float(D_ref)) <= 1e-12 * float(D_ref)
+    if a == 0.0:  # textbook Schwarzschild closed form x = r + 2M ln(r/2M - 1)
+        for rr in [2.0001, 2.5, 3.0, 10.0, 100.0]:
+            x = rr + 2.0 * math.log(rr / 2.0 - 1.0)
+            assert abs(orc.r_of_rstar(1.0, 0.0, x)[0] - rr) < 1e-13 * rr
+
+
+def test_p1_workload_tortoise_roundtrip(orc):
+    """The trajectory generator's forward map and the oracle's inversion are written separately."""
+    for a in [0.0, 0.7, 0.99]:
+        for rr in [1.5 + 0.7 * (a < 0.9) + 0.6 * (a == 0.0), 6.0, 10.0, 12.0]:
+            x = float(wl.tortoise_forward(rr, 1.0, a))
+            assert abs(orc.r_of_rstar(1.0, a, x)[0] - rr) < 1e-13 * rr
+
+
+# ------------------------------------------------------------------------------------ helpers
+def _pulse_run(orc, n_r, n_theta, a, m, cfl, T, shape, x_obs=50.0, rs=(-50.0, 150.0)):
+    dx = (rs[1] - rs[0]) / (n_r - 1)
+    dt = cfl * dx
+    o = orc.OracleSolver(a, 1.0, [m], rs[0], rs[1], n_r, n_theta, dt)
+    x = rs[0] + dx * np.arange(n_r)
+    th = (np.arange(n_theta) + 0.5) * math.pi / n_theta
+    ang = {"sin2": np.sin(th) ** 2, "y22": (1 + np.cos(th)) ** 2, "y21": np.sin(th) * (1 + np.cos(th))}[shape]
+    o.set_initial(np.ascontiguousarray((np.exp(-(x - 20.0) ** 2 / 4.0)[:, None] * ang[None, :])[None]))
+    harm = (1 + np.cos(th)) ** 2 if m % 2 == 0 else np.sin(th) * (1 + np.cos(th))
+    o.add_observer(x_obs, harm * np.sin(th) * math.pi / n_theta)
+    o.step(int(round(T / dt)))
+    t, w = o.waveform()
+    o.close()
+    return t, w[:, 0]
+
+
+def _prony(t, w, t0, t1, n_poles):
+    """Linear-prediction fit  w(t) = sum_k c_k exp(-i omega_k t)  on [t0, t1]; returns omega_k."""
+    sel = (t >= t0) & (t <= t1)
+    tt, ww = t[sel], w[sel]
+    stride = max(1, int(round(1.0 / (tt[1] - tt[0]))))
+    ww = ww[::stride]
+    h = (tt[1] - tt[0]) * stride
+    N, p = len(ww), n_poles
+    A = np.stack([ww[k:N - p + k] for k in range(p)], axis=1)
+    c = np.linalg.lstsq(A, ww[p:], rcond=None)[0]
+    z = np.roots(np.concatenate([[1.0], -c[::-1]]))
+    return 1j * np.log(z) / h
+
+
+# ------------------------------------------------------------------------------------------ P2
+def test_p2_second_order_convergence(orc):
+    """Halving (dx, dtheta, dt) twice divides the waveform error by 4."""
+    runs = []
+    for k in (1, 2, 4):
+        t, w = _pulse_run(orc, 384 * k + 1, 12 * k, 0.0, 2, 0.08, 120.0, "sin2")
+        runs.append((t[k - 1::k], w[k - 1::k]))
+    n = min(len(r[0]) for r in runs)
+    tc = runs[0][0][:n]
+    assert np.allclose(tc, runs[1][0][:n]) and np.allclose(tc, runs[2][0][:n])
+    wc, wm, wf = [r[1][:n] for r in runs]
+    sel = (tc >= 40.0) & (tc <= 120.0)
+    ratio = np.linalg.norm(wc[sel] - wm[sel]) / np.linalg.norm(wm[sel] - wf[sel])
+    assert np.linalg.norm(wf[sel]) > 10.0
+    assert 3.5 < ratio < 5.0, ratio
+
+
+# ------------------------------------------------------------------------------------------ P3
+@pytest.mark.parametrize("m,shape", [(2, "y22"), (1, "y21"), (2, "sin2")])
+def test_p3_schwarzschild_qnm(orc, m, shape):
+    """Ringdown frequency M omega = 0.3737 - 0.0890i, independent of m for a = 0."""
+    t, w = _pulse_run(orc, 1025, 32, 0.0, m, 0.08, 170.0, shape)
+    assert np.all(w.imag == 0.0)
+    om = _prony(t, w.real, 110.0, 170.0, 2)
+    om = om[np.argmax(om.real)]
+    assert abs(om - (0.3737 - 0.0890j)) < 1.5e-3, om
+
+
+def test_p3b_kerr_qnm(orc):
+    """Kerr a = 0.9, l = m = 2 fundamental mode M omega = 0.6716 - 0.0649i: pins every a != 0 term."""
+    t, w = _pulse_run(orc, 1537, 24, 0.9, 2, 0.16, 200.0, "y22")
+    for (t0, t1) in [(110.0, 190.0), (100.0, 160.0)]:
+        om = _prony(t, w, t0, t1, 6)
+        om = om[np.argmin(abs(om - (0.6716 - 0.0649j)))]
+        assert abs(om - (0.6716 - 0.0649j)) < 4e-3, om
+
+
+# ------------------------------------------------------------------------------------------ P4
+@pytest.mark.parametrize("m", [2, 1])
+def test_p4_reflection_invariant(orc, m):
+    """Phi_{-m}(x, pi - theta) = conj Phi_{+m}(x, theta) for data related the same way."""
+    n_r, n_th, a = 257, 16, 0.9
+    rs = (-30.0, 70.0)
+    dx = (rs[1] - rs[0]) / (n_r - 1)
+    x = rs[0] + dx * np.arange(n_r)
+    th = (np.arange(n_th) + 0.5) * math.pi / n_th
+    f = (np.exp(-(x - 15.0) ** 2 / 9.0) * np.exp(0.7j * x))[:, None] * (np.sin(th) ** 2 * (1.3 + np.cos(th)) * np.exp(0.4j * th))[None, :]
+    g = 0.3 * (np.exp(-(x - 5.0) ** 2 / 4.0))[:, None] * (np.sin(th) ** 2 * np.exp(-0.2j * th))[None, :]
+    outs = []
+    for sign in (+1, -1):
+        o = orc.OracleSolver(a, 1.0, [sign * m], rs[0], rs[1], n_r, n_th, 0.1 * dx)
+        ff, gg = (f, g) if sign > 0 else (np.conj(f[:, ::-1]), np.conj(g[:, ::-1]))
+        o.set_initial(*[np.ascontiguousarray(q[None]) for q in (ff.real, ff.imag, gg.real, gg.imag)])
+        o.step(600)
+        s = o.get_state()
+        outs.append((s[0][0] + 1j * s[1][0], s[2][0] + 1j * s[3][0]))
+        o.close()
+    for q in (0, 1):
+        ref = outs[0][q]
+        err = np.linalg.norm(outs[1][q][:, ::-1] - np.conj(ref)) / np.linalg.norm(ref)
+        assert err < 1e-12, err
+    # and the symmetry is not vacuous: +m and -m differ without the reflection
+    assert np.linalg.norm(outs[1][0] - outs[0][0]) > 1e-3 * np.linalg.norm(outs[0][0])
+
+
+# ------------------------------------------------------------------------------------------ P5
+def test_p5_schwarzschild_stays_real(orc):
+    cfg = wl.CONFIGS[1]
+    o = orc.OracleSolver.from_config(cfg)
+    o.set_initial(*wl.initial_data(cfg))
+    o.step(300)
+    s = o.get_state()
+    assert np.all(s[1] == 0.0) and np.all(s[3] == 0.0)
+    assert np.abs(s[0]).max() > 0.1 and np.abs(s[2]).max() > 0.01
+
+
+# ------------------------------------------------------------------------------------------ P6
+def _small_sourced(orc, scale=1.0, initial=None, source=True):
+    cfg = wl.small_test_configs()[3].scaled(n_r=301, steps=60)
+    o = orc.OracleSolver.from_config(cfg)
+    if initial is not None:
+        o.set_initial(*initial)
+    if source:
+        orb = wl.orbit_table(cfg)
+        orb["amp_re"] = orb["amp_re"] * scale
+        orb["amp_im"] = orb["amp_im"] * scale
+        o.set_source(orb)
+    o.add_observer(30.0, wl.observer_weights(cfg))
+    o.step(60)
+    return cfg, o.get_state(), o.waveform()[1]
+
+
+def test_p6_linearity(orc):
+    cfg, s1, w1 = _small_sourced(orc, 1.0)
+    _, s2, w2 = _small_sourced(orc, 2.0)
+    assert max(np.abs(q).max() for q in s1) > 0.0
+    for q1, q2 in zip(s1, s2):
+        assert np.array_equal(2.0 * q1, q2)          # scaling by 2 is exact in binary FP
+    assert np.array_equal(2.0 * w1, w2)
+    _, s0, _ = _small_sourced(orc, source=False)
+    assert all(np.all(q == 0.0) for q in s0)         # zero data, no source: stays zero
+    ini = wl.random_state(cfg, 7)
+    _, sa, _ = _small_sourced(orc, initial=ini, source=False)
+    _, sb, _ = _small_sourced(orc, initial=ini, source=True)
+    for qa, qb, q1 in zip(sa, sb, s1):               # superposition of data and source responses
+        assert np.linalg.norm(qb - qa - q1) <= 1e-12 * np.linalg.norm(qb)
+
+
+# ------------------------------------------------------------------------------------------ P7
+def test_p7_source_norm_support_and_time_levels(orc):
+    cfg = wl.small_test_configs()[3].scaled(n_r=401)
+    orb = wl.orbit_table(cfg, n_steps=4)
+    orb["amp_re"] = np.ones_like(orb["amp_re"])
+    orb["amp_im"] = np.zeros_like(orb["amp_im"])
+    o = orc.OracleSolver.from_config(cfg)
+    o.set_source(orb)
+    x, th = wl.grid_axes(cfg)
+    for half in (False, True):
+        T = o.source_field(0, 0, half)
+        assert abs(T.real.sum() * cfg.dx * cfg.dtheta - 1.0) < 1e-8       # unit mass
+        assert np.all(T.imag == 0.0)
+        nz = np.argwhere(T.real != 0.0)
+        assert nz[:, 0].max() - nz[:, 0].min() == 48 and nz[:, 1].max() - nz[:, 1].min() == 48
+        xs = (x[:-1] + 0.5 * cfg.dx) if half else x
+        i_pk, j_pk = np.unravel_index(np.argmax(T.real), T.shape)
+        assert abs(xs[i_pk] - orb["rs_p"][0]) <= 0.5 * cfg.dx + 1e-12
+        assert abs(th[j_pk] - orb["theta_p"][0]) <= 0.5 * cfg.dtheta + 1e-12
+        # first moment = particle position (Gaussian centred on the particle, not on a cell)
+        assert abs((T.real * xs[:, None]).sum() * cfg.dx * cfg.dtheta - orb["rs_p"][0]) < 1e-6
+    # closed form of the first iteration from zero data: the half step sees sample 0 at the
+    # half points, the full step sees sample 1 at the nodes (C.5, C.6).
+    for k_on in (0, 1):
+        o2 = orc.OracleSolver.from_config(cfg)
+        ob = dict(orb)
+        ob["amp_re"] = np.zeros_like(orb["amp_re"])
+        ob["amp_re"][:, k_on] = 1.0
+        o2.set_source(ob)
+        o2.step(1)
+        phi_re, phi_im, pi_re, pi_im = o2.get_state()
+        hs = o2.get_half()
+        if k_on == 0:
+            Th = o.source_field(0, 0, True)
+            assert np.allclose(hs[2][0], 0.5 * cfg.dt * Th.real, rtol=1e-14, atol=0)
+            assert np.all(hs[0] == 0.0)
+            exp_phi = cfg.dt * 0.5 * (hs[2][0][1:] + hs[2][0][:-1])          # Phi^1 = dt * Pi~
+            assert np.allclose(phi_re[0][1:-1], exp_phi, rtol=1e-13, atol=1e-300)
+        else:
+            Tn = o.source_field(0, 1, False)
+            assert np.all(hs[2] == 0.0) and np.all(phi_re == 0.0)
+            assert np.allclose(pi_re[0][1:-1], cfg.dt * Tn.real[1:-1], rtol=1e-14, atol=0)
+        o2.close()
