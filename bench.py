@@ -1,0 +1,306 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hot path (one "step" = one full Lax-Wendroff iteration: half step,
+pole ghosts, full step, radial edges, source deposit, waveform tap) on BASELINE.json's production
+config (#5: Kerr a = 0.99, m = 2, 131072 x 128, inspiralling smoothed-delta source).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1..5]
+
+Prints ONE JSON line (contract in the task statement / DESIGN.md "Measurement").
+N > 1 (torchrun): the path does not shard without a halo exchange the paper rejected
+(PAPER.md:155), so every rank evolves an independent replica ("temporal"
+parallelisation: different trajectory segments); no data-path collective; "scaling": "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1206_0270_b200 import workloads as wl  # noqa: E402
+
+BYTES_PER_PT_STEP = 64.0      # 4 FP64 planes read once + written once
+METRIC = "FP64 grid-point updates/s"
+UNIT = "GPts/s"
+
+
+def measured_peak_gbs():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic_bytes(cfg):
+    """DRAM bytes per launch of the step kernel from the committed ncu capture, if one matches."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            if d.get("workload") == cfg.name:
+                return float(d["dram_bytes_per_launch"])
+        except Exception:
+            pass
+    return None
+
+
+class ClockSampler:
+    """Samples nvidia-smi SM clocks and throttle reasons while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample_config(cfg, rows):
+    """Bounded sample of the workload for the CPU oracle: a radial crop around the particle."""
+    if cfg.n_r <= rows:
+        return cfg
+    dx = cfg.dx
+    lo = -rows // 8
+    x0 = round((0.0 - cfg.rs_min) / dx) + lo          # crop starts a little inside x = 0
+    rs_min = cfg.rs_min + x0 * dx
+    return cfg.scaled(name=cfg.name + "_crop%d" % rows, n_r=rows, rs_min=rs_min, rs_max=rs_min + (rows - 1) * dx,
+                      dt_over_dx=cfg.dt_over_dx, observers=(50.0,))
+
+
+def time_oracle(cfg, steps, warmup, rows):
+    """The oracle as it stands on the host cores; returns (GPts/s, threads, sample description)."""
+    from oracle import oracle as orc
+    c = oracle_sample_config(cfg, rows)
+    o = orc.OracleSolver.from_config(c)
+    o.set_initial(*wl.initial_data(c))
+    orbit = wl.orbit_table(c, n_steps=steps + warmup) if c.source else None
+    if orbit is not None:
+        # keep the full config's trajectory rate: T refers to cfg.steps * cfg.dt (c.dt == cfg.dt)
+        o.set_source(orbit)
+    o.add_observer(c.observers[0], wl.observer_weights(c))
+    o.step(warmup)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    o.close()
+    threads = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    sample = "%d iterations of a %d x %d radial crop (of %d x %d) incl. source window and observer" % (
+        steps, c.n_r, c.n_theta, cfg.n_r, cfg.n_theta)
+    return c.n_pts * steps / dt / 1e9, dt, threads, sample
+
+
+def run_reference(args, cfg, rank, world):
+    """--impl reference: the CPU oracle (the tier's reference arm), rank 0 only."""
+    if rank != 0:
+        return
+    rows = args.oracle_rows
+    val, dt, threads, sample = time_oracle(cfg, args.steps, args.warmup, rows)
+    c = oracle_sample_config(cfg, rows)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "grid": [cfg.n_r, cfg.n_theta], "modes": list(cfg.modes), "a": cfg.a,
+                   "sample_grid": [c.n_r, c.n_theta], "l2": "n/a (CPU)"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--oracle-rows", type=int, default=16384)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--slab-rows", type=int, default=0)
+    ap.add_argument("--graph", type=int, default=1)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    cfg = wl.CONFIGS[args.config]
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    if args.impl == "reference":
+        run_reference(args, cfg, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1206_0270_b200 import Solver
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    K, W = args.steps, args.warmup
+    # replica r evolves trajectory segment r: its table starts K+W iterations later
+    orbit = wl.orbit_table(cfg, n_steps=K + W, t0=0.0 if cfg.source != "inspiral" else rank * (K + W) * cfg.dt) \
+        if cfg.source else None
+    weights = wl.observer_weights(cfg)
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        g = Solver.from_config(cfg)
+        g.use_torch_stream()
+        g.set_option("graph", args.graph)
+        if args.slab_rows:
+            g.set_option("slab_rows", args.slab_rows)
+        # synthetic state resident in HBM: seeded random data on all four planes (throughput does not
+        # depend on values; zero data as in the config would let nothing but the source window move)
+        gen = torch.Generator(device="cuda").manual_seed(wl.SEED_BASE + cfg.cid + rank)
+        dev = [torch.randn(cfg.n_modes, cfg.n_r, cfg.n_theta, dtype=torch.float64, device="cuda", generator=gen)
+               * 1e-3 for _ in range(4)]
+        g.set_initial(*dev)
+        g.set_source(orbit)
+        for x in cfg.observers:
+            g.add_observer(x, weights)
+        # ---- device-resident timing -----------------------------------------------------------
+        for _ in range(W):
+            g.step(1)
+        barrier()
+        sampler = ClockSampler(local_rank)
+        if rank == 0:
+            sampler.start()
+        l0 = g.stat("launches")
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(stream)
+        for _ in range(K):
+            g.step(1)
+        e1.record(stream)
+        barrier()
+        ms = e0.elapsed_time(e1)
+        launches = g.stat("launches") - l0
+        clocks = sampler.stop() if rank == 0 else None
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        value = world * cfg.n_pts * K / (ms * 1e-3) / 1e9
+        # the series recorded so far (W + K samples) are drained to keep the next phase clean
+        for x in cfg.observers:
+            g.extract(x, allow_nonfinite=True)
+
+        # ---- end to end through the C ABI with HOST buffers -----------------------------------
+        host_in = [torch.randn(cfg.n_modes, cfg.n_r, cfg.n_theta, dtype=torch.float64).pin_memory() for _ in range(4)]
+        for h in host_in:
+            h.mul_(1e-3)
+        host_out = [torch.empty_like(h).pin_memory() for h in host_in]
+        e2e_ms = []
+        for rep in range(2):   # first repetition warms the pinned paths
+            barrier()
+            t0 = time.perf_counter()
+            g.set_initial(*host_in)                 # H2D: 4 planes
+            g.set_source(orbit)                     # H2D: trajectory table
+            g.step(K)
+            series = [g.extract(x, allow_nonfinite=True) for x in cfg.observers]   # D2H: waveforms
+            g.get_state(host_out)                   # D2H: 4 planes
+            barrier()
+            e2e_ms.append(1e3 * (time.perf_counter() - t0))
+        t = torch.tensor([e2e_ms[-1]], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e = world * cfg.n_pts * K / (float(t.item()) * 1e-3) / 1e9
+        state_bytes = 4 * cfg.n_pts * 8
+        orbit_bytes = 0 if orbit is None else 8 * (2 + 2 * cfg.n_modes) * orbit["n_samples"]
+        wave_bytes = sum(len(s[0]) * (8 + 16 * cfg.n_modes) for s in series)
+        g.close()
+
+    if rank == 0:
+        peak, peak_src = measured_peak_gbs()
+        achieved = BYTES_PER_PT_STEP * cfg.n_pts * K / (ms * 1e-3) / 1e9   # per GPU: ms is the max over ranks
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "grid": [cfg.n_r, cfg.n_theta], "modes": list(cfg.modes), "a": cfg.a,
+                       "dt": cfg.dt, "source": cfg.source, "observers": list(cfg.observers),
+                       "state_mb": 4 * cfg.n_pts * 8 / 1e6, "parallelism": "replicas x%d" % world,
+                       "l2": "inputs larger than L2 (two 537 MB state copies stream through a 126 MB L2)"
+                       if 4 * cfg.n_pts * 8 > 2.5e8 else "state fits in L2: not an HBM measurement"},
+            "clocks": clocks,
+            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": (state_bytes + orbit_bytes) / K,
+                    "d2h_bytes_per_step": (state_bytes + wave_bytes) / K,
+                    "note": "set_initial + set_source + step(K) + extract + get_state with pinned host buffers"},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": ncu_traffic_bytes(cfg), "peak_source": peak_src,
+                         "kernel": "teuk_step_kernel", "bytes_per_pt_step": BYTES_PER_PT_STEP},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            val, dt, threads, sample = time_oracle(cfg, 20, 3, args.oracle_rows)
+            line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

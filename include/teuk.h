@@ -1,0 +1,131 @@
+/* teuk.h -- C ABI of libteuk.so: the FP64 two-step Lax-Wendroff time step of the 2+1D Teukolsky
+ * equation (s = -2) on one NVIDIA B200 (sm_100a), after arXiv:1206.0270 section 2.2.
+ *
+ * What the library computes (citations are /root/reference/PAPER.md lines):
+ *   - the first-order system u = {Phi_R, Phi_I, Pi_R, Pi_I} of the m-mode reduction
+ *     Psi = sum_m e^{im phi~} r^3 Phi_m (Eq. 2) of the Teukolsky master equation
+ *     (Eq. 1), with the coefficient matrices D and S evaluated on
+ *     the device in closed form;
+ *   - one iteration = half step (Eq. 3) + full step (Eq. 4), with
+ *     second-order centred theta differences, pole parity conditions and radial edge
+ *     conditions;
+ *   - a Gaussian-smeared point-particle source deposited on the device each stage (PAPER.md:114,
+ *     :151) from a sampled trajectory the caller supplies;
+ *   - the waveform at a fixed r* (PAPER.md:161), tapped on the device into a ring buffer.
+ * Every step runs in CUDA kernels; there is no CPU fallback.  Readings of passages where the paper
+ * is silent are listed in DESIGN.md.
+ *
+ * Conventions
+ *   - Grid: x_i = rs_min + i*dx, i = 0..n_r-1, dx = (rs_max - rs_min)/(n_r - 1) (both end points);
+ *     theta_j = (j + 1/2)*pi/n_theta, j = 0..n_theta-1.  x is the tortoise coordinate r*.
+ *   - Field arrays at this boundary are FP64, shape [n_modes][n_r][n_theta], theta fastest, one
+ *     array per component (Phi_R, Phi_I, Pi_R, Pi_I).  (The internal device layout differs.)
+ *   - A pointer argument is a HOST pointer unless the call has a `ptr_is_device` flag that is 1.
+ *   - The caller owns every array it passes; the library copies what it needs before returning
+ *     (host arrays) or enqueues the copy on the solver's stream (device arrays).
+ *   - All device work is enqueued on the solver's stream (its own, or the one set with the
+ *     "stream" option); only teuk_extract, teuk_get_state(host), teuk_sync wait for it.
+ *   - Every function returns TEUK_OK (0) or a negative teuk_status; teuk_last_error gives text.
+ *     No exceptions, no aborts, no output on stdout/stderr.
+ *   - Not thread-safe per solver; distinct solvers may be used from distinct threads.
+ */
+#ifndef TEUK_H_
+#define TEUK_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  TEUK_OK = 0,
+  TEUK_EINVAL = -1,     /* bad parameter, NULL where not allowed, trajectory too short for n     */
+  TEUK_ENOMEM = -2,     /* host or device allocation failed                                       */
+  TEUK_ECUDA = -3,      /* CUDA error (sticky: the solver is unusable afterwards), or no device   */
+  TEUK_ENONFINITE = -4  /* a NaN/Inf was seen on a tapped waveform sample                         */
+} teuk_status;
+
+typedef struct teuk_solver teuk_solver; /* opaque; created and destroyed by the library */
+
+typedef struct {
+  double rs_min, rs_max; /* tortoise-coordinate range, rs_max > rs_min                            */
+  int32_t n_r, n_theta;  /* n_r >= 4; 4 <= n_theta <= 256                                          */
+} teuk_grid;
+
+/* Sampled particle trajectory and source amplitude (C.6 of DESIGN.md).
+ * Sample k is at t = k*dt/2 counted from the last teuk_set_initial: the half step of iteration n
+ * uses sample 2n (at the half points x_{i+1/2}), the full step uses sample 2n+1 (at the nodes).
+ * The deposited term is T(t,x,theta) = A'_m(t) g(x - x_p; sigma_r) g(theta - theta_p; sigma_theta),
+ * g(y;s) = exp(-y^2/(2 s^2))/(s sqrt(2 pi)), inside |i - i_p| <= W, |j - j_p| <= W only. */
+typedef struct {
+  int64_t n_samples;             /* >= 2 * (iterations to run)                                   */
+  const double *rs_p, *theta_p;  /* [n_samples] particle r*, theta                                */
+  const double *amp_re, *amp_im; /* [n_modes][n_samples] complex amplitude A'_m                   */
+  double sigma_r, sigma_theta;   /* Gaussian widths in r* and theta, absolute units, > 0          */
+  int32_t half_window;           /* W cells each side, 0 <= W <= 4096                              */
+} teuk_orbit;
+
+/* Create a solver for Kerr parameters (a, M), |a| < M, M > 0, and n_modes (1..64) azimuthal
+ * modes m[k] evolved together as independent fields ("decoupled"; one launch per
+ * iteration covers all modes).  dt > 0 is the time step (the caller is responsible for stability:
+ * DESIGN.md reading A1).  Allocates all device state (two copies of the fields, coefficient
+ * tables), builds the coefficient tables on the device, zeroes the fields.  Uses the CUDA device
+ * that is current in the calling thread.  *out is set to NULL on failure. */
+int teuk_create(teuk_solver **out, double a, double M, const int32_t *m, int32_t n_modes,
+                const teuk_grid *grid, double dt);
+
+/* Set Phi, Pi at t = 0 and reset the iteration counter, the simulated time and every observer's
+ * recorded series.  NULL = zeros for that component.  ptr_is_device: 0 host, 1 device pointers. */
+int teuk_set_initial(teuk_solver *s, const double *phi_re, const double *phi_im,
+                     const double *pi_re, const double *pi_im, int32_t ptr_is_device);
+
+/* Install (copy to the device) the trajectory table; NULL = source-free.  Host pointers. */
+int teuk_set_source(teuk_solver *s, const teuk_orbit *orbit);
+
+/* Enqueue n >= 0 iterations.  No host synchronisation, no full-grid host transfer; observers are
+ * tapped on the device after every iteration (sample time t = n_done*dt).  TEUK_EINVAL if a
+ * source is installed and its table is too short. */
+int teuk_step(teuk_solver *s, int64_t n);
+
+/* Observer at r* = rs_obs (x_0 <= rs_obs < x_{n_r-1}): w(t_n) = sum_j weights[j] *
+ * [(1-f) Phi^n_{i0,j} + f Phi^n_{i0+1,j}] (linear interpolation in x).
+ * The FIRST call with a new rs_obs arms the observer (weights [n_theta] host array, NULL = all
+ * ones; at most 8 observers; must precede the teuk_step calls it should record) and writes
+ * nothing.  LATER calls with the same rs_obs (weights ignored) wait for the stream and return the
+ * samples recorded since the previous call: t_out[k], and w_re/w_im [k][n_modes], k < *n_written
+ * <= capacity.  Samples beyond `capacity` stay queued for the next call.  Returns
+ * TEUK_ENONFINITE (after filling the outputs) if any recorded sample was NaN/Inf. */
+int teuk_extract(teuk_solver *s, double rs_obs, const double *weights, double *t_out,
+                 double *w_re, double *w_im, int64_t capacity, int64_t *n_written);
+
+/* Copy the current fields out (parity checks, checkpoints).  NULL = skip that component.
+ * Host pointers: waits for the stream.  Device pointers: enqueued on the stream. */
+int teuk_get_state(teuk_solver *s, double *phi_re, double *phi_im, double *pi_re, double *pi_im,
+                   int32_t ptr_is_device);
+
+/* Options (set before stepping):
+ *   "outer_bc"      0 = outgoing (Pi = 0, Phi upwind; default), 1 = Dirichlet as PAPER.md:104
+ *   "stream"        a cudaStream_t cast to int64 (0 = back to the solver's own stream)
+ *   "coef_mode"     0 = coefficients recomputed on the fly from 1D tables (default),
+ *                   1 = coefficients streamed from precomputed 2D FP64 planes
+ *   "slab_rows"     rows of r* marched by one warp (0 = automatic)
+ *   "graph"         1 = replay the iteration through a CUDA graph (default), 0 = plain launches */
+int teuk_set_option(teuk_solver *s, const char *key, int64_t value);
+
+/* Read-only counters: "steps" (iterations done), "launches" (kernels launched so far),
+ * "n_pts" (n_modes*n_r*n_theta), "state_bytes" (one copy of the fields). */
+int teuk_get_stat(const teuk_solver *s, const char *key, int64_t *value);
+
+/* Wait for all work enqueued on the solver's stream. */
+int teuk_sync(teuk_solver *s);
+
+void teuk_destroy(teuk_solver *s); /* NULL is allowed */
+
+/* Static text for the last error on this solver (or the last teuk_create failure if s == NULL). */
+const char *teuk_last_error(const teuk_solver *s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TEUK_H_ */

@@ -1,0 +1,642 @@
+// teuk_api.cu -- the C ABI of include/teuk.h: argument checks, device memory, stream/graph
+// plumbing, ring-buffer drains.  Every arithmetic step of the path runs in the kernels of
+// teuk_step.cu / teuk_tables.cu; there is no CPU fallback.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "../../include/teuk.h"
+#include "teuk_internal.h"
+
+// kernels / launchers defined in the other translation units
+cudaError_t teuk_launch_tables(double* rtab, double* ttab, const int* d_m, int n_modes, int n_r, int n_theta,
+                               double rs_min, double dx, double dth, double M, double a, cudaStream_t st);
+cudaError_t teuk_launch_step(const StepParams& p, cudaStream_t st);
+cudaError_t teuk_launch_flush_tap(const StepParams& p, cudaStream_t st);
+cudaError_t teuk_launch_bump(long long* d_base, long long inc, cudaStream_t st);
+cudaError_t teuk_launch_set_base(long long* d_base, long long v, cudaStream_t st);
+cudaError_t teuk_launch_pack(double* u, double* const src[4], size_t n_rows, int nth, cudaStream_t st);
+cudaError_t teuk_launch_unpack(const double* u, double* const dst[4], size_t n_rows, int nth, cudaStream_t st);
+
+namespace {
+
+const double kPi = 3.14159265358979323846264338327950288;
+const long long kRingCap = 1 << 15;  // samples per observer held on the device between drains
+const int kGraphBatch = 32;          // iterations per CUDA-graph replay (even)
+
+char g_create_error[256] = "no error";
+
+struct HostChunk {      // drained samples of one observer: pinned, [count][n_modes][2]
+  double* data;
+  long long first;      // sample index (1-based iteration number) of data[0]
+  long long count;
+};
+
+struct ObsHost {
+  double rs_obs;
+  int i0;
+  double f;
+  double* d_weights;
+  double* d_ring;
+  std::vector<HostChunk> chunks;
+  long long read_cursor;  // next sample index to hand to the caller (1-based)
+};
+
+}  // namespace
+
+struct teuk_solver {
+  // problem
+  double a, M, dt, dx, dth, rs_min, rs_max;
+  int n_r, n_theta, n_modes;
+  int m[TEUK_MAX_MODES];
+  // options
+  int outer_bc, coef_mode, slab_rows_opt, use_graph;
+  // device
+  int device, n_sms;
+  cudaStream_t own_stream, stream, copy_stream;
+  cudaEvent_t ev_compute, ev_copy;
+  double* d_u[2];
+  int cur;               // d_u[cur] holds the current time level
+  double *d_rtab, *d_ttab, *d_coef2d;
+  int* d_m;
+  long long* d_base;     // device copy of the iteration index baseline
+  long long base_on_device;
+  int* d_nonfinite;
+  // source
+  int has_source, W;
+  long long n_samples;
+  double *d_xp, *d_thp, *d_amp_re, *d_amp_im;
+  double sigma_r, sigma_th;
+  // time
+  long long step;        // iterations done since set_initial
+  long long recorded;    // samples recorded on the device (== step when observers exist)
+  long long drained;     // samples already copied to host chunks
+  // observers
+  int n_obs;
+  ObsHost obs[TEUK_MAX_OBS];
+  // graph
+  cudaGraphExec_t graph_exec[2];  // one per ping-pong parity of `cur`
+  // stats / errors
+  long long launches;
+  int sticky;            // sticky CUDA failure
+  char err[256];
+};
+
+namespace {
+
+int fail(teuk_solver* s, int code, const char* msg) {
+  if (s) {
+    snprintf(s->err, sizeof(s->err), "%s", msg);
+  } else {
+    snprintf(g_create_error, sizeof(g_create_error), "%s", msg);
+  }
+  return code;
+}
+
+int cuda_fail(teuk_solver* s, cudaError_t e, const char* where) {
+  char buf[256];
+  snprintf(buf, sizeof(buf), "CUDA error in %s: %s", where, cudaGetErrorString(e));
+  if (s) s->sticky = 1;
+  return fail(s, e == cudaErrorMemoryAllocation ? TEUK_ENOMEM : TEUK_ECUDA, buf);
+}
+
+#define CK(call, where)                                   \
+  do {                                                    \
+    cudaError_t e_ = (call);                              \
+    if (e_ != cudaSuccess) return cuda_fail(s, e_, where); \
+  } while (0)
+
+size_t state_doubles(const teuk_solver* s) { return (size_t)s->n_modes * s->n_r * 4 * s->n_theta; }
+
+void drop_graph(teuk_solver* s) {
+  for (int q = 0; q < 2; ++q)
+    if (s->graph_exec[q]) {
+      cudaGraphExecDestroy(s->graph_exec[q]);
+      s->graph_exec[q] = nullptr;
+    }
+}
+
+// Automatic slab length: enough warps for >= 2 waves of the resident capacity, slabs >= 16 rows.
+int auto_slab_rows(const teuk_solver* s) {
+  const int interior = s->n_r - 2;
+  const int sms = s->n_sms > 0 ? s->n_sms : 148;
+  const int v = (s->n_theta + 31) / 32;
+  const int warps_per_sm = v <= 1 ? 16 : (v <= 2 ? 8 : 8);
+  const long long target_warps = (long long)sms * warps_per_sm * 2;
+  long long per_mode = target_warps / s->n_modes;
+  if (per_mode < 1) per_mode = 1;
+  int rows = (int)((interior + per_mode - 1) / per_mode);
+  if (rows < 16) rows = 16;
+  if (rows > interior) rows = interior;
+  return rows;
+}
+
+void fill_params(const teuk_solver* s, StepParams* p, int in_buf, int k, int tap_enable) {
+  memset(p, 0, sizeof(*p));
+  p->uin = s->d_u[in_buf];
+  p->uout = s->d_u[in_buf ^ 1];
+  p->rtab = s->d_rtab;
+  p->ttab = s->d_ttab;
+  p->coef2d = s->d_coef2d;
+  p->n_r = s->n_r;
+  p->n_theta = s->n_theta;
+  p->n_modes = s->n_modes;
+  p->slab_rows = s->slab_rows_opt > 0 ? s->slab_rows_opt : auto_slab_rows(s);
+  if (p->slab_rows > s->n_r - 2) p->slab_rows = s->n_r - 2;
+  p->n_slabs = (s->n_r - 2 + p->slab_rows - 1) / p->slab_rows;
+  p->outer_bc = s->outer_bc;
+  p->dt = s->dt;
+  p->dx = s->dx;
+  p->rs_min = s->rs_min;
+  p->dth = s->dth;
+  p->has_source = s->has_source;
+  p->W = s->W;
+  p->n_samples = s->n_samples;
+  p->xp = s->d_xp;
+  p->thp = s->d_thp;
+  p->amp_re = s->d_amp_re;
+  p->amp_im = s->d_amp_im;
+  p->sigma_r = s->sigma_r;
+  p->sigma_th = s->sigma_th;
+  p->d_base = s->d_base;
+  p->k = k;
+  p->tap_enable = tap_enable;
+  p->n_obs = s->n_obs;
+  p->ring_cap = kRingCap;
+  p->nonfinite = s->d_nonfinite;
+  for (int q = 0; q < s->n_obs; ++q) {
+    p->obs[q].i0 = s->obs[q].i0;
+    p->obs[q].f = s->obs[q].f;
+    p->obs[q].weights = s->obs[q].d_weights;
+    p->obs[q].ring = s->obs[q].d_ring;
+  }
+}
+
+}  // namespace
+
+namespace {
+
+void free_chunks(ObsHost* o) {
+  for (size_t q = 0; q < o->chunks.size(); ++q) cudaFreeHost(o->chunks[q].data);
+  o->chunks.clear();
+}
+
+void reset_series(teuk_solver* s) {
+  for (int q = 0; q < s->n_obs; ++q) {
+    free_chunks(&s->obs[q]);
+    s->obs[q].read_cursor = 1;
+  }
+  s->recorded = 0;
+  s->drained = 0;
+}
+
+// Enqueue copies of the samples drained+1 .. recorded from the device rings into new pinned
+// host chunks on the copy stream; the compute stream then waits for the copies (no host sync).
+int drain_rings(teuk_solver* s) {
+  const long long count = s->recorded - s->drained;
+  if (count <= 0 || s->n_obs == 0) {
+    s->drained = s->recorded;
+    return TEUK_OK;
+  }
+  CK(cudaEventRecord(s->ev_compute, s->stream), "drain: event record");
+  CK(cudaStreamWaitEvent(s->copy_stream, s->ev_compute, 0), "drain: wait compute");
+  const size_t rec_bytes = (size_t)s->n_modes * 2 * sizeof(double);
+  for (int q = 0; q < s->n_obs; ++q) {
+    HostChunk ch;
+    ch.first = s->drained + 1;
+    ch.count = count;
+    ch.data = nullptr;
+    CK(cudaMallocHost((void**)&ch.data, (size_t)count * rec_bytes), "drain: pinned alloc");
+    const long long slot0 = s->drained % kRingCap;  // slot of sample drained+1
+    const long long first_part = (slot0 + count <= kRingCap) ? count : kRingCap - slot0;
+    CK(cudaMemcpyAsync(ch.data, (char*)s->obs[q].d_ring + (size_t)slot0 * rec_bytes,
+                       (size_t)first_part * rec_bytes, cudaMemcpyDeviceToHost, s->copy_stream),
+       "drain: copy");
+    if (first_part < count)
+      CK(cudaMemcpyAsync((char*)ch.data + (size_t)first_part * rec_bytes, s->obs[q].d_ring,
+                         (size_t)(count - first_part) * rec_bytes, cudaMemcpyDeviceToHost, s->copy_stream),
+         "drain: copy wrap");
+    s->obs[q].chunks.push_back(ch);
+  }
+  CK(cudaEventRecord(s->ev_copy, s->copy_stream), "drain: event record copy");
+  CK(cudaStreamWaitEvent(s->stream, s->ev_copy, 0), "drain: wait copy");
+  s->drained = s->recorded;
+  return TEUK_OK;
+}
+
+int build_tables(teuk_solver* s) {
+  CK(teuk_launch_tables(s->d_rtab, s->d_ttab, s->d_m, s->n_modes, s->n_r, s->n_theta, s->rs_min, s->dx,
+                        s->dth, s->M, s->a, s->stream),
+     "table kernels");
+  s->launches += 2;
+  return TEUK_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* teuk_last_error(const teuk_solver* s) { return s ? s->err : g_create_error; }
+
+void teuk_destroy(teuk_solver* s) {
+  if (!s) return;
+  cudaSetDevice(s->device);
+  if (s->stream) cudaStreamSynchronize(s->stream);
+  if (s->copy_stream) cudaStreamSynchronize(s->copy_stream);
+  drop_graph(s);
+  for (int q = 0; q < s->n_obs; ++q) {
+    free_chunks(&s->obs[q]);
+    cudaFree(s->obs[q].d_weights);
+    cudaFree(s->obs[q].d_ring);
+  }
+  cudaFree(s->d_u[0]);
+  cudaFree(s->d_u[1]);
+  cudaFree(s->d_rtab);
+  cudaFree(s->d_ttab);
+  cudaFree(s->d_coef2d);
+  cudaFree(s->d_m);
+  cudaFree(s->d_base);
+  cudaFree(s->d_nonfinite);
+  cudaFree(s->d_xp);
+  cudaFree(s->d_thp);
+  cudaFree(s->d_amp_re);
+  cudaFree(s->d_amp_im);
+  if (s->ev_compute) cudaEventDestroy(s->ev_compute);
+  if (s->ev_copy) cudaEventDestroy(s->ev_copy);
+  if (s->own_stream) cudaStreamDestroy(s->own_stream);
+  if (s->copy_stream) cudaStreamDestroy(s->copy_stream);
+  delete s;
+}
+
+int teuk_create(teuk_solver** out, double a, double M, const int32_t* m, int32_t n_modes,
+                const teuk_grid* grid, double dt) {
+  if (!out) return fail(nullptr, TEUK_EINVAL, "teuk_create: out is NULL");
+  *out = nullptr;
+  if (!m || !grid) return fail(nullptr, TEUK_EINVAL, "teuk_create: m or grid is NULL");
+  if (!(M > 0.0) || !(fabs(a) < M)) return fail(nullptr, TEUK_EINVAL, "teuk_create: need M > 0 and |a| < M");
+  if (n_modes < 1 || n_modes > TEUK_MAX_MODES) return fail(nullptr, TEUK_EINVAL, "teuk_create: n_modes must be 1..64");
+  if (grid->n_r < 4 || grid->n_theta < 4 || grid->n_theta > 256)
+    return fail(nullptr, TEUK_EINVAL, "teuk_create: need n_r >= 4 and 4 <= n_theta <= 256");
+  if (!(grid->rs_max > grid->rs_min) || !(dt > 0.0) || !isfinite(dt) || !isfinite(grid->rs_min) ||
+      !isfinite(grid->rs_max))
+    return fail(nullptr, TEUK_EINVAL, "teuk_create: need rs_max > rs_min and dt > 0");
+  int dev = 0, ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    return fail(nullptr, TEUK_ECUDA, "teuk_create: no CUDA device (this library has no CPU fallback)");
+  }
+  if (cudaGetDevice(&dev) != cudaSuccess) return fail(nullptr, TEUK_ECUDA, "teuk_create: cudaGetDevice failed");
+  teuk_solver* s = new (std::nothrow) teuk_solver();
+  if (!s) return fail(nullptr, TEUK_ENOMEM, "teuk_create: host allocation failed");
+  s->a = a; s->M = M; s->dt = dt;
+  s->rs_min = grid->rs_min; s->rs_max = grid->rs_max;
+  s->n_r = grid->n_r; s->n_theta = grid->n_theta; s->n_modes = n_modes;
+  s->dx = (grid->rs_max - grid->rs_min) / (grid->n_r - 1);
+  s->dth = kPi / grid->n_theta;
+  for (int q = 0; q < n_modes; ++q) s->m[q] = m[q];
+  s->outer_bc = 0; s->coef_mode = 0; s->slab_rows_opt = 0; s->use_graph = 1;
+  s->device = dev;
+  if (cudaDeviceGetAttribute(&s->n_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) s->n_sms = 148;
+  snprintf(s->err, sizeof(s->err), "no error");
+  int rc = TEUK_OK;
+  do {
+    const size_t nst = state_doubles(s) * sizeof(double);
+    const size_t n_loc = (size_t)(2 * s->n_r - 1);
+#define CKC(call, where) { cudaError_t e_ = (call); if (e_ != cudaSuccess) { rc = cuda_fail(s, e_, where); break; } }
+    CKC(cudaStreamCreateWithFlags(&s->own_stream, cudaStreamNonBlocking), "stream create");
+    CKC(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking), "stream create");
+    s->stream = s->own_stream;
+    CKC(cudaEventCreateWithFlags(&s->ev_compute, cudaEventDisableTiming), "event create");
+    CKC(cudaEventCreateWithFlags(&s->ev_copy, cudaEventDisableTiming), "event create");
+    CKC(cudaMalloc((void**)&s->d_u[0], nst), "state alloc");
+    CKC(cudaMalloc((void**)&s->d_u[1], nst), "state alloc");
+    CKC(cudaMalloc((void**)&s->d_rtab, (size_t)n_modes * n_loc * RT_N * sizeof(double)), "rtab alloc");
+    CKC(cudaMalloc((void**)&s->d_ttab, (size_t)n_modes * TT_N * s->n_theta * sizeof(double)), "ttab alloc");
+    CKC(cudaMalloc((void**)&s->d_m, n_modes * sizeof(int)), "m alloc");
+    CKC(cudaMalloc((void**)&s->d_base, sizeof(long long)), "counter alloc");
+    CKC(cudaMalloc((void**)&s->d_nonfinite, sizeof(int)), "flag alloc");
+    CKC(cudaMemcpyAsync(s->d_m, s->m, n_modes * sizeof(int), cudaMemcpyHostToDevice, s->stream), "m copy");
+    CKC(cudaMemsetAsync(s->d_u[0], 0, nst, s->stream), "state zero");
+    CKC(cudaMemsetAsync(s->d_u[1], 0, nst, s->stream), "state zero");
+    CKC(cudaMemsetAsync(s->d_base, 0, sizeof(long long), s->stream), "counter zero");
+    CKC(cudaMemsetAsync(s->d_nonfinite, 0, sizeof(int), s->stream), "flag zero");
+#undef CKC
+    rc = build_tables(s);
+    if (rc != TEUK_OK) break;
+    cudaError_t e = cudaStreamSynchronize(s->stream);
+    if (e != cudaSuccess) { rc = cuda_fail(s, e, "teuk_create sync"); break; }
+  } while (0);
+  if (rc != TEUK_OK) {
+    snprintf(g_create_error, sizeof(g_create_error), "%s", s->err);
+    teuk_destroy(s);
+    return rc;
+  }
+  *out = s;
+  return TEUK_OK;
+}
+
+int teuk_sync(teuk_solver* s) {
+  if (!s) return TEUK_EINVAL;
+  if (s->sticky) return TEUK_ECUDA;
+  CK(cudaStreamSynchronize(s->stream), "teuk_sync");
+  CK(cudaStreamSynchronize(s->copy_stream), "teuk_sync");
+  return TEUK_OK;
+}
+
+int teuk_set_initial(teuk_solver* s, const double* phi_re, const double* phi_im, const double* pi_re,
+                     const double* pi_im, int32_t ptr_is_device) {
+  if (!s) return TEUK_EINVAL;
+  if (s->sticky) return TEUK_ECUDA;
+  const double* src[4] = {phi_re, phi_im, pi_re, pi_im};
+  const size_t n_pts = (size_t)s->n_modes * s->n_r * s->n_theta;
+  double* planes[4];
+  double* scratch = s->d_u[s->cur ^ 1];
+  for (int c = 0; c < 4; ++c) {
+    planes[c] = nullptr;
+    if (!src[c]) continue;
+    if (ptr_is_device) {
+      planes[c] = const_cast<double*>(src[c]);
+    } else {
+      planes[c] = scratch + (size_t)c * n_pts;
+      CK(cudaMemcpyAsync(planes[c], src[c], n_pts * sizeof(double), cudaMemcpyHostToDevice, s->stream),
+         "set_initial: H2D");
+    }
+  }
+  CK(teuk_launch_pack(s->d_u[s->cur], planes, (size_t)s->n_modes * s->n_r, s->n_theta, s->stream),
+     "set_initial: pack");
+  CK(teuk_launch_set_base(s->d_base, 0, s->stream), "set_initial: counter");
+  CK(cudaMemsetAsync(s->d_nonfinite, 0, sizeof(int), s->stream), "set_initial: flag");
+  s->launches += 2;
+  s->base_on_device = 0;
+  s->step = 0;
+  // series restart; pending copies of the old series must land before their buffers are freed
+  CK(cudaStreamSynchronize(s->copy_stream), "set_initial: copy stream");
+  reset_series(s);
+  if (!ptr_is_device) CK(cudaStreamSynchronize(s->stream), "set_initial: sync");  // host arrays may be reused
+  return TEUK_OK;
+}
+
+int teuk_set_source(teuk_solver* s, const teuk_orbit* orbit) {
+  if (!s) return TEUK_EINVAL;
+  if (s->sticky) return TEUK_ECUDA;
+  if (orbit) {
+    if (orbit->n_samples < 2 || !orbit->rs_p || !orbit->theta_p || !orbit->amp_re || !orbit->amp_im)
+      return fail(s, TEUK_EINVAL, "teuk_set_source: NULL table or n_samples < 2");
+    if (!(orbit->sigma_r > 0.0) || !(orbit->sigma_theta > 0.0) || orbit->half_window < 0 ||
+        orbit->half_window > 4096)
+      return fail(s, TEUK_EINVAL, "teuk_set_source: need sigma > 0 and 0 <= half_window <= 4096");
+  }
+  CK(cudaStreamSynchronize(s->stream), "set_source: sync");  // old tables may still be in use
+  drop_graph(s);
+  cudaFree(s->d_xp); cudaFree(s->d_thp); cudaFree(s->d_amp_re); cudaFree(s->d_amp_im);
+  s->d_xp = s->d_thp = s->d_amp_re = s->d_amp_im = nullptr;
+  s->has_source = 0;
+  s->n_samples = 0;
+  if (!orbit) return TEUK_OK;
+  const size_t ns = (size_t)orbit->n_samples;
+  CK(cudaMalloc((void**)&s->d_xp, ns * sizeof(double)), "set_source: alloc");
+  CK(cudaMalloc((void**)&s->d_thp, ns * sizeof(double)), "set_source: alloc");
+  CK(cudaMalloc((void**)&s->d_amp_re, ns * s->n_modes * sizeof(double)), "set_source: alloc");
+  CK(cudaMalloc((void**)&s->d_amp_im, ns * s->n_modes * sizeof(double)), "set_source: alloc");
+  CK(cudaMemcpyAsync(s->d_xp, orbit->rs_p, ns * sizeof(double), cudaMemcpyHostToDevice, s->stream), "set_source: H2D");
+  CK(cudaMemcpyAsync(s->d_thp, orbit->theta_p, ns * sizeof(double), cudaMemcpyHostToDevice, s->stream), "set_source: H2D");
+  CK(cudaMemcpyAsync(s->d_amp_re, orbit->amp_re, ns * s->n_modes * sizeof(double), cudaMemcpyHostToDevice, s->stream), "set_source: H2D");
+  CK(cudaMemcpyAsync(s->d_amp_im, orbit->amp_im, ns * s->n_modes * sizeof(double), cudaMemcpyHostToDevice, s->stream), "set_source: H2D");
+  CK(cudaStreamSynchronize(s->stream), "set_source: sync");  // caller may free its arrays on return
+  s->has_source = 1;
+  s->n_samples = orbit->n_samples;
+  s->sigma_r = orbit->sigma_r;
+  s->sigma_th = orbit->sigma_theta;
+  s->W = orbit->half_window;
+  return TEUK_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+// Capture kGraphBatch tapping iterations + the counter bump for the current ping-pong parity.
+int build_graph(teuk_solver* s) {
+  cudaGraph_t graph = nullptr;
+  CK(cudaStreamBeginCapture(s->own_stream, cudaStreamCaptureModeThreadLocal), "graph: begin capture");
+  cudaError_t e = cudaSuccess;
+  for (int k = 0; k < kGraphBatch && e == cudaSuccess; ++k) {
+    StepParams p;
+    fill_params(s, &p, s->cur ^ (k & 1), k, 1);
+    e = teuk_launch_step(p, s->own_stream);
+  }
+  if (e == cudaSuccess) e = teuk_launch_bump(s->d_base, kGraphBatch, s->own_stream);
+  cudaError_t e2 = cudaStreamEndCapture(s->own_stream, &graph);
+  if (e != cudaSuccess) { if (graph) cudaGraphDestroy(graph); return cuda_fail(s, e, "graph: capture launch"); }
+  CK(e2, "graph: end capture");
+  e = cudaGraphInstantiate(&s->graph_exec[s->cur], graph, 0);
+  cudaGraphDestroy(graph);
+  CK(e, "graph: instantiate");
+  return TEUK_OK;
+}
+
+// Run c >= 1 iterations whose samples fit in the ring.
+int run_chunk(teuk_solver* s, long long c) {
+  long long left = c;
+  int first = 1;
+  while (left > 0) {
+    const bool graph_ok = s->use_graph && !first && left >= kGraphBatch;
+    if (graph_ok) {
+      if (!s->graph_exec[s->cur]) {
+        const int rc = build_graph(s);
+        if (rc != TEUK_OK) return rc;
+      }
+      if (s->base_on_device != s->step) {
+        CK(teuk_launch_set_base(s->d_base, s->step, s->stream), "step: counter");
+        s->base_on_device = s->step;
+        s->launches += 1;
+      }
+      CK(cudaGraphLaunch(s->graph_exec[s->cur], s->stream), "step: graph launch");
+      s->base_on_device += kGraphBatch;
+      s->step += kGraphBatch;
+      s->launches += kGraphBatch + 1;
+      left -= kGraphBatch;
+      continue;
+    }
+    const long long k = s->step - s->base_on_device;
+    if (k < 0 || k > (1LL << 30)) {
+      CK(teuk_launch_set_base(s->d_base, s->step, s->stream), "step: counter");
+      s->base_on_device = s->step;
+      s->launches += 1;
+    }
+    StepParams p;
+    fill_params(s, &p, s->cur, (int)(s->step - s->base_on_device), first ? 0 : 1);
+    CK(teuk_launch_step(p, s->stream), "step: launch");
+    s->launches += 1;
+    s->cur ^= 1;
+    s->step += 1;
+    left -= 1;
+    first = 0;
+  }
+  if (s->n_obs > 0) {
+    StepParams p;
+    fill_params(s, &p, s->cur, (int)(s->step - s->base_on_device), 1);
+    CK(teuk_launch_flush_tap(p, s->stream), "step: flush tap");
+    s->launches += 1;
+    s->recorded = s->step;
+  }
+  return TEUK_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int teuk_step(teuk_solver* s, int64_t n) {
+  if (!s) return TEUK_EINVAL;
+  if (s->sticky) return TEUK_ECUDA;
+  if (n < 0) return fail(s, TEUK_EINVAL, "teuk_step: n < 0");
+  if (s->has_source && 2 * (s->step + n) > s->n_samples)
+    return fail(s, TEUK_EINVAL, "teuk_step: trajectory table too short for n more iterations");
+  long long remaining = n;
+  while (remaining > 0) {
+    long long room = remaining;
+    if (s->n_obs > 0) {
+      room = kRingCap - (s->recorded - s->drained);
+      if (room <= 0) {
+        const int rc = drain_rings(s);
+        if (rc != TEUK_OK) return rc;
+        continue;
+      }
+    }
+    const long long c = remaining < room ? remaining : room;
+    const int rc = run_chunk(s, c);
+    if (rc != TEUK_OK) return rc;
+    remaining -= c;
+  }
+  return TEUK_OK;
+}
+
+int teuk_extract(teuk_solver* s, double rs_obs, const double* weights, double* t_out, double* w_re,
+                 double* w_im, int64_t capacity, int64_t* n_written) {
+  if (!s) return TEUK_EINVAL;
+  if (s->sticky) return TEUK_ECUDA;
+  if (n_written) *n_written = 0;
+  int q = -1;
+  for (int k = 0; k < s->n_obs; ++k)
+    if (s->obs[k].rs_obs == rs_obs) q = k;
+  if (q < 0) {  // arm a new observer
+    if (s->n_obs >= TEUK_MAX_OBS) return fail(s, TEUK_EINVAL, "teuk_extract: too many observers");
+    if (s->step != 0) return fail(s, TEUK_EINVAL, "teuk_extract: arm observers before stepping (after teuk_set_initial)");
+    const double v = (rs_obs - s->rs_min) / s->dx;
+    const int i0 = (int)floor(v);
+    if (!(v >= 0.0) || i0 > s->n_r - 2) return fail(s, TEUK_EINVAL, "teuk_extract: rs_obs outside [x_0, x_{n_r-1})");
+    CK(cudaStreamSynchronize(s->stream), "extract: sync");
+    drop_graph(s);
+    ObsHost* o = &s->obs[s->n_obs];
+    o->rs_obs = rs_obs;
+    o->i0 = i0;
+    o->f = v - i0;
+    o->read_cursor = 1;
+    o->d_weights = nullptr;
+    o->d_ring = nullptr;
+    std::vector<double> w((size_t)s->n_theta, 1.0);
+    if (weights) memcpy(w.data(), weights, (size_t)s->n_theta * sizeof(double));
+    CK(cudaMalloc((void**)&o->d_weights, (size_t)s->n_theta * sizeof(double)), "extract: alloc");
+    CK(cudaMalloc((void**)&o->d_ring, (size_t)kRingCap * s->n_modes * 2 * sizeof(double)), "extract: alloc");
+    CK(cudaMemcpy(o->d_weights, w.data(), (size_t)s->n_theta * sizeof(double), cudaMemcpyHostToDevice), "extract: H2D");
+    CK(cudaMemset(o->d_ring, 0, (size_t)kRingCap * s->n_modes * 2 * sizeof(double)), "extract: zero");
+    s->n_obs += 1;
+    return TEUK_OK;
+  }
+  if (capacity < 0 || (capacity > 0 && (!t_out || !w_re || !w_im)) || !n_written)
+    return fail(s, TEUK_EINVAL, "teuk_extract: NULL output or negative capacity");
+  int rc = drain_rings(s);
+  if (rc != TEUK_OK) return rc;
+  CK(cudaStreamSynchronize(s->copy_stream), "extract: sync copies");
+  CK(cudaStreamSynchronize(s->stream), "extract: sync");
+  int nonfinite = 0;
+  CK(cudaMemcpy(&nonfinite, s->d_nonfinite, sizeof(int), cudaMemcpyDeviceToHost), "extract: flag");
+  ObsHost* o = &s->obs[q];
+  int64_t written = 0;
+  size_t ci = 0;
+  while (written < capacity && ci < o->chunks.size()) {
+    HostChunk& ch = o->chunks[ci];
+    const long long end = ch.first + ch.count;  // one past the last sample of this chunk
+    if (o->read_cursor >= end) { ++ci; continue; }
+    const long long off = o->read_cursor - ch.first;
+    for (int k = 0; k < s->n_modes; ++k) {
+      w_re[written * s->n_modes + k] = ch.data[((size_t)off * s->n_modes + k) * 2 + 0];
+      w_im[written * s->n_modes + k] = ch.data[((size_t)off * s->n_modes + k) * 2 + 1];
+    }
+    t_out[written] = (double)o->read_cursor * s->dt;
+    o->read_cursor += 1;
+    written += 1;
+  }
+  // release fully consumed chunks
+  while (!o->chunks.empty() && o->read_cursor >= o->chunks.front().first + o->chunks.front().count) {
+    cudaFreeHost(o->chunks.front().data);
+    o->chunks.erase(o->chunks.begin());
+  }
+  *n_written = written;
+  if (nonfinite) return fail(s, TEUK_ENONFINITE, "teuk_extract: a tapped sample was NaN/Inf");
+  return TEUK_OK;
+}
+
+int teuk_get_state(teuk_solver* s, double* phi_re, double* phi_im, double* pi_re, double* pi_im,
+                   int32_t ptr_is_device) {
+  if (!s) return TEUK_EINVAL;
+  if (s->sticky) return TEUK_ECUDA;
+  double* dst[4] = {phi_re, phi_im, pi_re, pi_im};
+  const size_t n_pts = (size_t)s->n_modes * s->n_r * s->n_theta;
+  double* planes[4];
+  double* scratch = s->d_u[s->cur ^ 1];
+  for (int c = 0; c < 4; ++c) planes[c] = dst[c] ? (ptr_is_device ? dst[c] : scratch + (size_t)c * n_pts) : nullptr;
+  CK(teuk_launch_unpack(s->d_u[s->cur], planes, (size_t)s->n_modes * s->n_r, s->n_theta, s->stream),
+     "get_state: unpack");
+  s->launches += 1;
+  if (!ptr_is_device) {
+    for (int c = 0; c < 4; ++c)
+      if (dst[c])
+        CK(cudaMemcpyAsync(dst[c], planes[c], n_pts * sizeof(double), cudaMemcpyDeviceToHost, s->stream),
+           "get_state: D2H");
+    CK(cudaStreamSynchronize(s->stream), "get_state: sync");
+  }
+  return TEUK_OK;
+}
+
+int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
+  if (!s || !key) return TEUK_EINVAL;
+  if (s->sticky) return TEUK_ECUDA;
+  CK(cudaStreamSynchronize(s->stream), "set_option: sync");
+  if (!strcmp(key, "outer_bc")) {
+    if (value != 0 && value != 1) return fail(s, TEUK_EINVAL, "outer_bc must be 0 or 1");
+    s->outer_bc = (int)value;
+  } else if (!strcmp(key, "stream")) {
+    s->stream = value ? (cudaStream_t)(uintptr_t)value : s->own_stream;
+  } else if (!strcmp(key, "coef_mode")) {
+    if (value != 0) return fail(s, TEUK_EINVAL, "coef_mode 1 (streamed 2D coefficient planes) is not built in this round");
+    s->coef_mode = (int)value;
+  } else if (!strcmp(key, "slab_rows")) {
+    if (value < 0 || value > (1 << 30)) return fail(s, TEUK_EINVAL, "slab_rows out of range");
+    s->slab_rows_opt = (int)value;
+  } else if (!strcmp(key, "graph")) {
+    s->use_graph = value ? 1 : 0;
+  } else {
+    return fail(s, TEUK_EINVAL, "teuk_set_option: unknown key");
+  }
+  drop_graph(s);
+  return TEUK_OK;
+}
+
+int teuk_get_stat(const teuk_solver* s, const char* key, int64_t* value) {
+  if (!s || !key || !value) return TEUK_EINVAL;
+  if (!strcmp(key, "steps")) *value = s->step;
+  else if (!strcmp(key, "launches")) *value = s->launches;
+  else if (!strcmp(key, "n_pts")) *value = (int64_t)s->n_modes * s->n_r * s->n_theta;
+  else if (!strcmp(key, "state_bytes")) *value = (int64_t)(state_doubles(s) * sizeof(double));
+  else return TEUK_EINVAL;
+  return TEUK_OK;
+}
+
+}  // extern "C"

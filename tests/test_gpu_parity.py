@@ -1,0 +1,245 @@
+"""Parity of the CUDA path (through the C ABI of include/teuk.h) with the CPU oracle, element by
+element on the same seeded inputs.  Tolerance: relative L2 <= 1e-10 in Phi, Pi and each observer's
+waveform (BASELINE.json north_star); one-iteration checks use 1e-12."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1206_0270_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def teuk():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1206_0270_b200 import teuk as t
+    t.load()
+    return t
+
+
+def rel_l2(got, ref):
+    got, ref = np.asarray(got), np.asarray(ref)
+    den = np.linalg.norm(ref)
+    if den == 0.0:
+        return float(np.linalg.norm(got))
+    return float(np.linalg.norm(got - ref) / den)
+
+
+def run_pair(orc, teuk, cfg, steps, initial=None, observers=None, options=None, orbit_steps=None, chunks=None):
+    """Run oracle and GPU on the same inputs; return dict of states and waveforms."""
+    ini = wl.initial_data(cfg) if initial is None else initial
+    orbit = wl.orbit_table(cfg, n_steps=orbit_steps if orbit_steps is not None else max(steps, 1))
+    W = wl.observer_weights(cfg)
+    observers = list(cfg.observers) if observers is None else observers
+    o = orc.OracleSolver.from_config(cfg)
+    g = teuk.Solver.from_config(cfg)
+    for k, v in (options or {}).items():
+        g.set_option(k, v)
+    o.set_initial(*ini)
+    g.set_initial(*ini)
+    o.set_source(orbit)
+    g.set_source(orbit)
+    for x in observers:
+        o.add_observer(x, W)
+        g.add_observer(x, W)
+    o.step(steps)
+    for c in (chunks or [steps]):
+        g.step(c)
+    so, sg = o.get_state(), g.get_state()
+    wo = [o.waveform(k) for k in range(len(observers))]
+    wg = [g.extract(x) for x in observers]
+    launches = g.stat("launches")
+    o.close()
+    g.close()
+    return dict(so=so, sg=sg, wo=wo, wg=wg, launches=launches)
+
+
+def check_pair(res, tol=TOL, need_signal=True):
+    phi_o = res["so"][0] + 1j * res["so"][1]
+    phi_g = res["sg"][0] + 1j * res["sg"][1]
+    pi_o = res["so"][2] + 1j * res["so"][3]
+    pi_g = res["sg"][2] + 1j * res["sg"][3]
+    if need_signal:
+        assert np.linalg.norm(phi_o) > 0 and np.linalg.norm(pi_o) > 0
+    assert np.all(np.isfinite(phi_g)) and np.all(np.isfinite(pi_g))
+    e_phi, e_pi = rel_l2(phi_g, phi_o), rel_l2(pi_g, pi_o)
+    assert e_phi <= tol and e_pi <= tol, (e_phi, e_pi)
+    for (to, wo), (tg, wg) in zip(res["wo"], res["wg"]):
+        assert len(to) == len(tg) and np.allclose(to, tg, rtol=1e-14, atol=0)
+        if np.linalg.norm(wo) < 1e-200:
+            assert np.linalg.norm(wg) < 1e-200      # silent observer
+            continue
+        e_w = rel_l2(wg, wo)
+        assert e_w <= tol, e_w
+    return e_phi, e_pi
+
+
+SMALL = wl.small_test_configs()
+
+
+@pytest.mark.parametrize("cfg", SMALL, ids=[c.name for c in SMALL])
+def test_one_iteration_random_state(orc, teuk, cfg):
+    """All four planes random: every term of Eq. (3)-(4), ghosts, edges and the deposit at once."""
+    res = run_pair(orc, teuk, cfg, 1, initial=wl.random_state(cfg, 100 + cfg.cid))
+    check_pair(res, tol=1e-12)
+    res = run_pair(orc, teuk, cfg, 3, initial=wl.random_state(cfg, 200 + cfg.cid))
+    check_pair(res, tol=1e-12)
+
+
+@pytest.mark.parametrize("cfg", SMALL, ids=[c.name for c in SMALL])
+def test_multi_step_parity(orc, teuk, cfg):
+    """The config's own data, source and observers, after its step count."""
+    steps = cfg.steps
+    res = run_pair(orc, teuk, cfg, steps)
+    check_pair(res)
+    assert len(res["wg"][0][0]) == steps
+
+
+def test_config2_quick_tier(orc, teuk):
+    cfg = wl.CONFIGS[2]
+    check_pair(run_pair(orc, teuk, cfg, 1000))
+
+
+def test_config3_quick_tier(orc, teuk):
+    cfg = wl.CONFIGS[3]
+    check_pair(run_pair(orc, teuk, cfg, 300))
+
+
+def test_config4_quick_tier(orc, teuk):
+    cfg = wl.CONFIGS[4]
+    check_pair(run_pair(orc, teuk, cfg, 100))
+
+
+@pytest.mark.parametrize("n_theta", [4, 20, 32, 45, 50, 64, 96, 100, 128, 131, 200, 256])
+def test_theta_sizes_and_ragged_lanes(orc, teuk, n_theta):
+    """Every lane/vector layout: V = 1, 2, 4, 8, vector and scalar access, idle lanes."""
+    cfg = SMALL[3].scaled(name="th%d" % n_theta, n_r=211, n_theta=n_theta, dt_over_dx=0.02, steps=12,
+                          modes=(2, 1))
+    res = run_pair(orc, teuk, cfg, 12, initial=wl.random_state(cfg, n_theta))
+    check_pair(res, tol=1e-11)
+
+
+@pytest.mark.parametrize("n_r", [4, 5, 6, 17, 18, 19, 33, 130])
+def test_tiny_radial_grids_and_slab_tails(orc, teuk, n_r):
+    cfg = wl.CONFIGS[1].scaled(name="nr%d" % n_r, n_r=n_r, rs_min=5.0, rs_max=5.0 + 0.4 * (n_r - 1), steps=5,
+                               observers=(5.0, 5.0 + 0.4 * (n_r - 1) - 0.1), a=0.5)
+    for slab in (0, 1, 3, 16):
+        res = run_pair(orc, teuk, cfg, 5, initial=wl.random_state(cfg, n_r), options={"slab_rows": slab})
+        check_pair(res, tol=1e-12)
+
+
+def test_dirichlet_outer_edge(orc, teuk):
+    cfg = SMALL[2].scaled(name="dirichlet", outer_bc=1, steps=50)
+    check_pair(run_pair(orc, teuk, cfg, 50, initial=wl.random_state(cfg, 5)), tol=1e-11)
+
+
+def test_graph_and_plain_launches_agree_bitwise(orc, teuk):
+    cfg = SMALL[3]
+    out = []
+    for graph, chunks in ((1, [150]), (0, [150]), (1, [1, 70, 33, 46])):
+        g = teuk.Solver.from_config(cfg)
+        g.set_option("graph", graph)
+        g.set_initial(*wl.random_state(cfg, 3))
+        g.set_source(wl.orbit_table(cfg, n_steps=150))
+        g.add_observer(30.0, wl.observer_weights(cfg))
+        for c in chunks:
+            g.step(c)
+        out.append((g.get_state(), g.extract(30.0)))
+        g.close()
+    for k in (1, 2):
+        for a, b in zip(out[0][0], out[k][0]):
+            assert np.array_equal(a, b)
+        assert np.array_equal(out[0][1][1], out[k][1][1]) and len(out[k][1][0]) == 150
+
+
+def test_ring_buffer_wraps_and_drains(orc, teuk):
+    """More iterations than the device ring holds (32768): samples are drained by async copies."""
+    cfg = wl.CONFIGS[1].scaled(name="ring", n_r=24, n_theta=8, rs_min=10.0, rs_max=19.2, steps=40000,
+                               dt_over_dx=0.02, observers=(12.3,))
+    res = run_pair(orc, teuk, cfg, 40000, chunks=[5, 32763, 1, 7231])
+    check_pair(res, tol=1e-9)   # 40000 iterations of a 24-point-wide cavity: round-off accumulates
+    t = res["wg"][0][0]
+    assert len(t) == 40000 and abs(t[-1] - 40000 * cfg.dt) < 1e-9
+
+
+def test_partial_extract_and_resume(orc, teuk):
+    cfg = SMALL[0]
+    g = teuk.Solver.from_config(cfg)
+    g.set_initial(*wl.initial_data(cfg))
+    g.add_observer(30.0)
+    g.step(10)
+    t1, w1 = g.extract(30.0, capacity=4)
+    g.step(5)
+    t2, w2 = g.extract(30.0)
+    assert len(t1) == 4 and len(t2) == 11
+    assert np.allclose(np.concatenate([t1, t2]), cfg.dt * np.arange(1, 16))
+    g.set_initial(*wl.initial_data(cfg))          # resets the series
+    g.step(3)
+    t3, w3 = g.extract(30.0)
+    assert len(t3) == 3 and np.array_equal(w3, np.concatenate([w1, w2])[:3])
+    g.close()
+
+
+def test_device_pointers_and_torch_stream(orc, teuk):
+    import torch
+    cfg = SMALL[2]
+    ini = wl.random_state(cfg, 11)
+    g = teuk.Solver.from_config(cfg)
+    g.use_torch_stream()
+    dev = [torch.from_numpy(a).cuda() for a in ini]
+    g.set_initial(*dev)
+    g.step(7)
+    out = [torch.empty_like(d) for d in dev]
+    g.get_state(out)
+    torch.cuda.synchronize()
+    h = teuk.Solver.from_config(cfg)
+    h.set_initial(*ini)
+    h.step(7)
+    ref = h.get_state()
+    for a, b in zip(out, ref):
+        assert np.array_equal(a.cpu().numpy(), b)
+    g.close()
+    h.close()
+
+
+def test_argument_errors(teuk):
+    with pytest.raises(teuk.TeukError) as e:
+        teuk.Solver(1.0, 1.0, [2], -10, 10, 64, 32, 0.01)       # |a| = M
+    assert e.value.code == teuk.TEUK_EINVAL
+    with pytest.raises(teuk.TeukError):
+        teuk.Solver(0.5, 1.0, [2], -10, 10, 3, 32, 0.01)        # n_r < 4
+    with pytest.raises(teuk.TeukError):
+        teuk.Solver(0.5, 1.0, [2], -10, 10, 64, 300, 0.01)      # n_theta > 256
+    cfg = SMALL[3]
+    g = teuk.Solver.from_config(cfg)
+    g.set_source(wl.orbit_table(cfg, n_steps=5))
+    g.step(5)
+    with pytest.raises(teuk.TeukError) as e:
+        g.step(1)                                               # trajectory table exhausted
+    assert e.value.code == teuk.TEUK_EINVAL
+    with pytest.raises(teuk.TeukError):
+        g.add_observer(1e9)
+    with pytest.raises(teuk.TeukError):
+        g.set_option("no_such_option", 1)
+    g.step(0)
+    g.close()
+
+
+def test_nonfinite_sentinel(teuk):
+    cfg = SMALL[0]
+    ini = list(wl.initial_data(cfg))
+    ini[0] = ini[0].copy()
+    ini[0][0, 200, 5] = float("nan")
+    g = teuk.Solver.from_config(cfg)
+    g.set_initial(*ini)
+    g.add_observer(cfg.rs_min + 200 * cfg.dx + 0.01)
+    g.step(2)
+    with pytest.raises(teuk.TeukError) as e:
+        g.extract(cfg.rs_min + 200 * cfg.dx + 0.01)
+    assert e.value.code == teuk.TEUK_ENONFINITE
+    g.close()
