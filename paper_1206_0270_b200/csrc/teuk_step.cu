@@ -113,11 +113,11 @@ template <int V, bool HALF>
 __device__ __forceinline__ void lw_stage(const Row<V>& A, const Row<V>& B, const Row<V>& base,
                                          const double* __restrict__ rec, const ThetaTab<V>& th,
                                          double tau, double two_over_dx, Row<V>& out) {
-  const double2 r01 = __ldg(reinterpret_cast<const double2*>(rec + 0));
-  const double2 r23 = __ldg(reinterpret_cast<const double2*>(rec + 2));
-  const double2 r45 = __ldg(reinterpret_cast<const double2*>(rec + 4));
-  const double2 r67 = __ldg(reinterpret_cast<const double2*>(rec + 6));
-  const double2 r89 = __ldg(reinterpret_cast<const double2*>(rec + 8));
+  const double2 r01 = *reinterpret_cast<const double2*>(rec + 0);
+  const double2 r23 = *reinterpret_cast<const double2*>(rec + 2);
+  const double2 r45 = *reinterpret_cast<const double2*>(rec + 4);
+  const double2 r67 = *reinterpret_cast<const double2*>(rec + 6);
+  const double2 r89 = *reinterpret_cast<const double2*>(rec + 8);
   const double eps = r01.x, x32 = r01.y, bre2 = r23.x, bim2 = r23.y;
   const double a0 = r45.x, a1 = r45.y, a2 = r67.x, g1 = r67.y, gr = r89.x, cl = r89.y;
 
@@ -261,6 +261,25 @@ __device__ __forceinline__ void tap(const Row<V>& lo, const Row<V>& hi, const St
 
 }  // namespace
 
+// r-table staging: the 2*RT_CH records (node + half point) of the next RT_CH marching iterations
+// are copied global -> shared with cp.async while the current chunk is being consumed, so the
+// warp-uniform coefficient loads are short LDS broadcasts instead of exposed L2 round trips.
+constexpr int RT_CH = 16;
+constexpr int RT_CHUNK_DOUBLES = RT_CH * 2 * RT_N;
+
+__device__ __forceinline__ void stage_rtab_chunk(double* sbuf, const double* __restrict__ rtab, int p_begin,
+                                                 int n_loc, int lane) {
+  const size_t g0 = (size_t)p_begin * RT_N, gend = (size_t)n_loc * RT_N;
+#pragma unroll
+  for (int q = lane; q < RT_CHUNK_DOUBLES / 2; q += 32) {
+    if (g0 + 2 * q < gend) {
+      const unsigned saddr = (unsigned)__cvta_generic_to_shared(sbuf + 2 * q);
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(saddr), "l"(rtab + g0 + 2 * q) : "memory");
+    }
+  }
+  asm volatile("cp.async.commit_group;" ::: "memory");
+}
+
 template <int V, bool VEC>
 __global__ void __launch_bounds__(128) teuk_step_kernel(const __grid_constant__ StepParams p) {
   const int lane = threadIdx.x & 31;
@@ -276,6 +295,9 @@ __global__ void __launch_bounds__(128) teuk_step_kernel(const __grid_constant__ 
   double* __restrict__ uout = p.uout + (size_t)mode * nr * row_stride;
   const double* __restrict__ rtab = p.rtab + (size_t)mode * (2 * nr - 1) * RT_N;
   const long long n = *p.d_base + p.k;               // index of the input time level
+  __shared__ __align__(16) double s_rt[4][2][RT_CHUNK_DOUBLES];
+  double* const rt_buf = &s_rt[threadIdx.x >> 5][0][0];
+  stage_rtab_chunk(rt_buf, rtab, 2 * r0, 2 * nr - 1, lane);
 
   ThetaTab<V> th;
   {
@@ -304,13 +326,23 @@ __global__ void __launch_bounds__(128) teuk_step_kernel(const __grid_constant__ 
   lw_stage<V, true>(ua, ub, ua, rtab + (size_t)(2 * (r0 - 1) + 1) * RT_N, th, tau_h, tdx, hp);
   add_source<V>(hp, src_h, p, r0 - 1, true);
 
+  const double* rt_cur = rt_buf;
   for (int i = r0; i < r1; ++i) {
     // ub = u^n_i, uc = u^n_{i+1}, hp = 2 u^{n+1/2}_{i-1/2}; prefetch row i+2 into ua (dead)
     if (i + 2 <= r1) load_row<V, VEC>(ua, uin + (size_t)(i + 2) * row_stride, nth, j0);
+    const int o = (i - r0) & (RT_CH - 1);
+    if (o == 0) {  // chunk boundary (warp-uniform): current chunk has landed, start the next one
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+      __syncwarp();
+      const int c = (i - r0) / RT_CH;
+      rt_cur = rt_buf + (c & 1) * RT_CHUNK_DOUBLES;
+      if (i + RT_CH < r1)
+        stage_rtab_chunk(rt_buf + ((c + 1) & 1) * RT_CHUNK_DOUBLES, rtab, 2 * (i + RT_CH), 2 * nr - 1, lane);
+    }
     if (do_tap) tap<V>(ub, uc, p, i, mode, n, j0, lane);
-    lw_stage<V, true>(ub, uc, ub, rtab + (size_t)(2 * i + 1) * RT_N, th, tau_h, tdx, hn);
+    lw_stage<V, true>(ub, uc, ub, rt_cur + (2 * o + 1) * RT_N, th, tau_h, tdx, hn);
     add_source<V>(hn, src_h, p, i, true);
-    lw_stage<V, false>(hp, hn, ub, rtab + (size_t)(2 * i) * RT_N, th, tau_f, tdx, out);
+    lw_stage<V, false>(hp, hn, ub, rt_cur + (2 * o) * RT_N, th, tau_f, tdx, out);
     add_source<V>(out, src_f, p, i, false);
     store_row<V, VEC>(out, uout + (size_t)i * row_stride, nth, j0);
     hp = hn;
