@@ -261,6 +261,53 @@ __device__ __forceinline__ void tap(const Row<V>& lo, const Row<V>& hi, const St
 
 }  // namespace
 
+// ---- TMA bulk-copy row prefetch (cp.async.bulk + mbarrier; SASS: UBLKCP) ------------------------
+// One lane of each warp asks the TMA engine for the whole next r* row (4 components x n_theta
+// doubles, contiguous in HBM) into the warp's shared-memory landing slot; the warp keeps computing
+// and picks the row up from shared memory 1.5 marching iterations later.  No registers are tied
+// up by loads in flight.
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void tma_load_row(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  unsigned ok;
+  do {
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  } while (!ok);
+}
+
+// shared-memory row (same [comp][n_theta] layout as HBM) -> registers
+template <int V>
+__device__ __forceinline__ void lds_row(Row<V>& u, const double* srow, int nth, int j0) {
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    if (j0 < nth) {
+      const double* q = srow + c * nth + j0;
+      if (V == 1) {
+        u.c[c][0] = q[0];
+      } else {
+#pragma unroll
+        for (int v = 0; v < V; v += 2) {
+          const double2 t = *reinterpret_cast<const double2*>(q + v);
+          u.c[c][v] = t.x;
+          u.c[c][v + 1] = t.y;
+        }
+      }
+    } else {
+#pragma unroll
+      for (int v = 0; v < V; ++v) u.c[c][v] = 0.0;
+    }
+  }
+}
+
 // r-table staging: the 2*RT_CH records (node + half point) of the next RT_CH marching iterations
 // are copied global -> shared with cp.async while the current chunk is being consumed, so the
 // warp-uniform coefficient loads are short LDS broadcasts instead of exposed L2 round trips.
@@ -296,8 +343,27 @@ __global__ void __launch_bounds__(128) teuk_step_kernel(const __grid_constant__ 
   const double* __restrict__ rtab = p.rtab + (size_t)mode * (2 * nr - 1) * RT_N;
   const long long n = *p.d_base + p.k;               // index of the input time level
   __shared__ __align__(16) double s_rt[4][2][RT_CHUNK_DOUBLES];
-  double* const rt_buf = &s_rt[threadIdx.x >> 5][0][0];
+  __shared__ __align__(8) unsigned long long s_bar[4][2];
+  extern __shared__ __align__(128) unsigned char s_dyn[];   // VEC: [warp][2 slots][4 n_theta] doubles
+  const int wib = threadIdx.x >> 5;
+  double* const rt_buf = &s_rt[wib][0][0];
   stage_rtab_chunk(rt_buf, rtab, 2 * r0, 2 * nr - 1, lane);
+  const unsigned row_bytes = (unsigned)(row_stride * sizeof(double));
+  double* const slot0 = reinterpret_cast<double*>(s_dyn) + (size_t)wib * 2 * row_stride;
+  unsigned long long* const bars = &s_bar[wib][0];
+  if (VEC) {
+    if (lane == 0) {
+      mbar_init(&bars[0], 1);
+      mbar_init(&bars[1], 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      // row q lands in slot q & 1; rows r0+2 and (mid-iteration r0) r0+3 are the first uses
+      if (r0 + 2 <= r1)
+        tma_load_row(slot0 + (size_t)((r0 + 2) & 1) * row_stride, uin + (size_t)(r0 + 2) * row_stride, row_bytes,
+                     &bars[(r0 + 2) & 1]);
+    }
+    __syncwarp();
+  }
 
   ThetaTab<V> th;
   {
@@ -328,8 +394,10 @@ __global__ void __launch_bounds__(128) teuk_step_kernel(const __grid_constant__ 
 
   const double* rt_cur = rt_buf;
   for (int i = r0; i < r1; ++i) {
-    // ub = u^n_i, uc = u^n_{i+1}, hp = 2 u^{n+1/2}_{i-1/2}; prefetch row i+2 into ua (dead)
-    if (i + 2 <= r1) load_row<V, VEC>(ua, uin + (size_t)(i + 2) * row_stride, nth, j0);
+    // ub = u^n_i, uc = u^n_{i+1}, hp = 2 u^{n+1/2}_{i-1/2}
+    if (!VEC) {  // scalar fallback: prefetch row i+2 into ua (dead) with plain loads
+      if (i + 2 <= r1) load_row<V, VEC>(ua, uin + (size_t)(i + 2) * row_stride, nth, j0);
+    }
     const int o = (i - r0) & (RT_CH - 1);
     if (o == 0) {  // chunk boundary (warp-uniform): current chunk has landed, start the next one
       asm volatile("cp.async.wait_group 0;" ::: "memory");
@@ -342,12 +410,27 @@ __global__ void __launch_bounds__(128) teuk_step_kernel(const __grid_constant__ 
     if (do_tap) tap<V>(ub, uc, p, i, mode, n, j0, lane);
     lw_stage<V, true>(ub, uc, ub, rt_cur + (2 * o + 1) * RT_N, th, tau_h, tdx, hn);
     add_source<V>(hn, src_h, p, i, true);
+    if (VEC) {
+      // uc (row i+1, read from slot (i+1)&1 at the end of the last iteration) has been consumed by
+      // every lane: its slot may now receive row i+3.
+      __syncwarp();
+      if (lane == 0 && i + 3 <= r1)
+        tma_load_row(slot0 + (size_t)((i + 3) & 1) * row_stride, uin + (size_t)(i + 3) * row_stride, row_bytes,
+                     &bars[(i + 3) & 1]);
+    }
     lw_stage<V, false>(hp, hn, ub, rt_cur + (2 * o) * RT_N, th, tau_f, tdx, out);
     add_source<V>(out, src_f, p, i, false);
     store_row<V, VEC>(out, uout + (size_t)i * row_stride, nth, j0);
     hp = hn;
     ub = uc;
-    uc = ua;
+    if (VEC) {
+      if (i + 2 <= r1) {
+        mbar_wait(&bars[(i + 2) & 1], (unsigned)(((i + 2) - (r0 + 2)) >> 1) & 1u);
+        lds_row<V>(uc, slot0 + (size_t)((i + 2) & 1) * row_stride, nth, j0);
+      }
+    } else {
+      uc = ua;
+    }
   }
 
   // radial edges (outer edge: DESIGN.md reading A6)
@@ -447,10 +530,19 @@ template <int V>
 static cudaError_t launch_v(const StepParams& p, cudaStream_t st) {
   const int warps_per_block = 4;
   dim3 grid((p.n_slabs + warps_per_block - 1) / warps_per_block, p.n_modes), block(32 * warps_per_block);
-  if (p.n_theta % V == 0)
-    teuk_step_kernel<V, true><<<grid, block, 0, st>>>(p);
-  else
+  if (p.n_theta % V == 0) {
+    const size_t dyn = (size_t)warps_per_block * 2 * 4 * p.n_theta * sizeof(double);
+    static bool attr_set = false;   // per instantiation
+    if (!attr_set) {
+      cudaError_t e = cudaFuncSetAttribute(teuk_step_kernel<V, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           (int)((size_t)warps_per_block * 2 * 4 * 32 * V * sizeof(double)));
+      if (e != cudaSuccess) return e;
+      attr_set = true;
+    }
+    teuk_step_kernel<V, true><<<grid, block, dyn, st>>>(p);
+  } else {
     teuk_step_kernel<V, false><<<grid, block, 0, st>>>(p);
+  }
   return cudaGetLastError();
 }
 

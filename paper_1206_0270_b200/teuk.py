@@ -13,7 +13,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libteuk.so")
+LIB_PATH = os.environ.get("TEUK_LIB") or os.path.join(_HERE, "libteuk.so")  # TEUK_LIB: development override
 
 TEUK_OK, TEUK_EINVAL, TEUK_ENOMEM, TEUK_ECUDA, TEUK_ENONFINITE = 0, -1, -2, -3, -4
 SYMBOLS = ["teuk_create", "teuk_set_initial", "teuk_set_source", "teuk_step", "teuk_extract",
