@@ -35,10 +35,73 @@ struct Row {
   double c[4][V];  // Phi_R, Phi_I, Pi_R, Pi_I for this lane's V columns
 };
 
+#ifndef TEUK_TT_SMEM
+#define TEUK_TT_SMEM 0   // theta tables: 0 = registers (measured faster), 1 = shared memory (16-byte pieces)
+#endif
+#ifndef TEUK_MIN_BLOCKS
+#define TEUK_MIN_BLOCKS 2
+#endif
+#ifndef TEUK_FAST_RSQRT
+#define TEUK_FAST_RSQRT 1
+#endif
+#ifndef TEUK_UNROLL2
+#define TEUK_UNROLL2 1
+#endif
+#ifndef TEUK_PHASED
+#define TEUK_PHASED 1   // compute the V reciprocal square roots of a stage up front (independent chains)
+#endif
+
+// theta-dependent factors of this lane's V columns (rows of teuk_internal.h TT_*)
 template <int V>
-struct ThetaTab {
+struct ThetaVals {
   double s2[V], cs[V], ap[V], am[V], d0[V];
 };
+
+#if TEUK_TT_SMEM
+// Block-shared copy, laid out so that a warp-wide 16-byte load touches 512 contiguous bytes:
+// double index ((tbl * NP + piece) * 32 + lane) * PW + (v % PW), PW = min(V,2), NP = V / PW.
+template <int V>
+struct ThetaTab {
+  const double* base;   // shared memory
+  int lane;
+  __device__ __forceinline__ void get(ThetaVals<V>& t) const {
+    constexpr int PW = V >= 2 ? 2 : 1, NP = V / PW;
+    double* dst[TT_N] = {t.s2, t.cs, t.ap, t.am, t.d0};
+#pragma unroll
+    for (int k = 0; k < TT_N; ++k)
+#pragma unroll
+      for (int q = 0; q < NP; ++q) {
+        const double* src = base + ((k * NP + q) * 32 + lane) * PW;
+        if (PW == 2) {
+          const double2 w = *reinterpret_cast<const double2*>(src);
+          dst[k][2 * q] = w.x;
+          dst[k][2 * q + 1] = w.y;
+        } else {
+          dst[k][q] = src[0];
+        }
+      }
+  }
+};
+#else
+template <int V>
+struct ThetaTab {
+  ThetaVals<V> vals;
+  __device__ __forceinline__ void get(ThetaVals<V>& t) const { t = vals; }
+};
+#endif
+
+// 1/sqrt(x) for x in (0.9, 1]: MUFU.RSQ64H seed (rel. error < 2^-20) + one third-order step
+// y <- y + y e (1/2 + 3/8 e), e = 1 - x y^2  (error ~ e^3): no range checks, no branch.
+__device__ __forceinline__ double rsqrt_near_one(double x) {
+#if TEUK_FAST_RSQRT
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double e = fma(-x * y, y, 1.0);
+  return fma(y * e, fma(0.375, e, 0.5), y);
+#else
+  return rsqrt(x);
+#endif
+}
 
 // ---- global <-> register rows ---------------------------------------------------------------
 __device__ __forceinline__ void ld256(const double* p, double& a, double& b, double& c, double& d) {
@@ -111,8 +174,10 @@ __device__ __forceinline__ void store_row(const Row<V>& u, double* __restrict__ 
 // else: A = H_{i-1/2}, B = H_{i+1/2} (doubled), out = u^{n+1}_i, base = u^n_i   (Eq. 4, tau = dt/4)
 template <int V, bool HALF>
 __device__ __forceinline__ void lw_stage(const Row<V>& A, const Row<V>& B, const Row<V>& base,
-                                         const double* __restrict__ rec, const ThetaTab<V>& th,
+                                         const double* __restrict__ rec, const ThetaTab<V>& tht,
                                          double tau, double two_over_dx, Row<V>& out) {
+  ThetaVals<V> th;
+  tht.get(th);
   const double2 r01 = *reinterpret_cast<const double2*>(rec + 0);
   const double2 r23 = *reinterpret_cast<const double2*>(rec + 2);
   const double2 r45 = *reinterpret_cast<const double2*>(rec + 4);
@@ -130,6 +195,11 @@ __device__ __forceinline__ void lw_stage(const Row<V>& A, const Row<V>& B, const
   // theta-neighbours across lanes (pole ghosts are folded into ap/am/d0; see teuk_ttab_kernel)
   const double left_r = __shfl_up_sync(FULL, sfr[V - 1], 1), left_i = __shfl_up_sync(FULL, sfi[V - 1], 1);
   const double right_r = __shfl_down_sync(FULL, sfr[0], 1), right_i = __shfl_down_sync(FULL, sfi[0], 1);
+#if TEUK_PHASED
+  double bv[V];
+#pragma unroll
+  for (int v = 0; v < V; ++v) bv[v] = rsqrt_near_one(fma(-eps, th.s2[v], 1.0));
+#endif
 #pragma unroll
   for (int v = 0; v < V; ++v) {
     const double dfr = B.c[0][v] - A.c[0][v], dfi = B.c[1][v] - A.c[1][v];
@@ -139,7 +209,11 @@ __device__ __forceinline__ void lw_stage(const Row<V>& A, const Row<V>& B, const
     const double fpr = (v < V - 1) ? sfr[v < V - 1 ? v + 1 : 0] : right_r;
     const double fpi = (v < V - 1) ? sfi[v < V - 1 ? v + 1 : 0] : right_i;
     // coefficients at (r, theta_j)
-    const double b = rsqrt(fma(-eps, th.s2[v], 1.0));
+#if TEUK_PHASED
+    const double b = bv[v];
+#else
+    const double b = rsqrt_near_one(fma(-eps, th.s2[v], 1.0));
+#endif
     const double Q = b * b;
     const double b2d = b * two_over_dx;
     const double aim = fma(a2, th.cs[v], a1);
@@ -328,12 +402,27 @@ __device__ __forceinline__ void stage_rtab_chunk(double* sbuf, const double* __r
 }
 
 template <int V, bool VEC>
-__global__ void __launch_bounds__(128) teuk_step_kernel(const __grid_constant__ StepParams p) {
+__global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const __grid_constant__ StepParams p) {
   const int lane = threadIdx.x & 31;
   const int slab = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   const int mode = blockIdx.y;
-  if (slab >= p.n_slabs) return;
   const int nth = p.n_theta, nr = p.n_r;
+#if TEUK_TT_SMEM
+  __shared__ __align__(16) double s_tt[TT_N * 32 * V];
+  {
+    constexpr int PW = V >= 2 ? 2 : 1, NP = V / PW;
+    const double* tb = p.ttab + (size_t)mode * TT_N * nth;
+    for (int t = threadIdx.x; t < TT_N * 32 * V; t += blockDim.x) {
+      const int k = t / (32 * V), r = t - k * 32 * V;      // table, position inside the table
+      const int q = r / (32 * PW), l = (r / PW) % 32, w = r % PW;
+      const int j = l * V + q * PW + w;                    // column owned by lane l
+      s_tt[t] = (j < nth) ? tb[k * nth + j] : 0.0;
+      (void)NP;
+    }
+    __syncthreads();
+  }
+#endif
+  if (slab >= p.n_slabs) return;
   const int r0 = 1 + slab * p.slab_rows;             // first interior node of this slab
   const int r1 = min(r0 + p.slab_rows, nr - 1);      // one past the last
   const int j0 = lane * V;
@@ -366,18 +455,23 @@ __global__ void __launch_bounds__(128) teuk_step_kernel(const __grid_constant__ 
   }
 
   ThetaTab<V> th;
+#if TEUK_TT_SMEM
+  th.base = s_tt;
+  th.lane = lane;
+#else
   {
     const double* tb = p.ttab + (size_t)mode * TT_N * nth;
 #pragma unroll
     for (int v = 0; v < V; ++v) {
       const bool ok = j0 + v < nth;
-      th.s2[v] = ok ? tb[TT_S2 * nth + j0 + v] : 0.0;
-      th.cs[v] = ok ? tb[TT_COS * nth + j0 + v] : 0.0;
-      th.ap[v] = ok ? tb[TT_AP * nth + j0 + v] : 0.0;
-      th.am[v] = ok ? tb[TT_AM * nth + j0 + v] : 0.0;
-      th.d0[v] = ok ? tb[TT_D0 * nth + j0 + v] : 0.0;
+      th.vals.s2[v] = ok ? tb[TT_S2 * nth + j0 + v] : 0.0;
+      th.vals.cs[v] = ok ? tb[TT_COS * nth + j0 + v] : 0.0;
+      th.vals.ap[v] = ok ? tb[TT_AP * nth + j0 + v] : 0.0;
+      th.vals.am[v] = ok ? tb[TT_AM * nth + j0 + v] : 0.0;
+      th.vals.d0[v] = ok ? tb[TT_D0 * nth + j0 + v] : 0.0;
     }
   }
+#endif
   StageSource<V> src_h, src_f;   // half stage: sample 2n at half points; full stage: 2n+1 at nodes
   setup_source<V>(src_h, p, mode, 2 * n, true, r0 - 1, r1 - 1, j0);
   setup_source<V>(src_f, p, mode, 2 * n + 1, false, r0, r1 - 1, j0);
@@ -393,9 +487,11 @@ __global__ void __launch_bounds__(128) teuk_step_kernel(const __grid_constant__ 
   add_source<V>(hp, src_h, p, r0 - 1, true);
 
   const double* rt_cur = rt_buf;
-  for (int i = r0; i < r1; ++i) {
-    // ub = u^n_i, uc = u^n_{i+1}, hp = 2 u^{n+1/2}_{i-1/2}
-    if (!VEC) {  // scalar fallback: prefetch row i+2 into ua (dead) with plain loads
+  // One marching iteration at node i.  On entry A = u^n_i, B = u^n_{i+1}, Hp = 2 u^{n+1/2}_{i-1/2};
+  // on exit Hn = 2 u^{n+1/2}_{i+1/2} and A = u^n_{i+2}.  The caller alternates the roles of
+  // (A, B) and (Hp, Hn), so no register rotation is needed.
+  auto march = [&](const int i, Row<V>& A, Row<V>& B, Row<V>& Hp, Row<V>& Hn) {
+    if (!VEC) {  // scalar fallback: prefetch row i+2 with plain loads
       if (i + 2 <= r1) load_row<V, VEC>(ua, uin + (size_t)(i + 2) * row_stride, nth, j0);
     }
     const int o = (i - r0) & (RT_CH - 1);
@@ -407,30 +503,44 @@ __global__ void __launch_bounds__(128) teuk_step_kernel(const __grid_constant__ 
       if (i + RT_CH < r1)
         stage_rtab_chunk(rt_buf + ((c + 1) & 1) * RT_CHUNK_DOUBLES, rtab, 2 * (i + RT_CH), 2 * nr - 1, lane);
     }
-    if (do_tap) tap<V>(ub, uc, p, i, mode, n, j0, lane);
-    lw_stage<V, true>(ub, uc, ub, rt_cur + (2 * o + 1) * RT_N, th, tau_h, tdx, hn);
-    add_source<V>(hn, src_h, p, i, true);
+    if (do_tap) tap<V>(A, B, p, i, mode, n, j0, lane);
+    lw_stage<V, true>(A, B, A, rt_cur + (2 * o + 1) * RT_N, th, tau_h, tdx, Hn);
+    add_source<V>(Hn, src_h, p, i, true);
     if (VEC) {
-      // uc (row i+1, read from slot (i+1)&1 at the end of the last iteration) has been consumed by
+      // B (row i+1, read from slot (i+1)&1 at the end of the last iteration) has been consumed by
       // every lane: its slot may now receive row i+3.
       __syncwarp();
       if (lane == 0 && i + 3 <= r1)
         tma_load_row(slot0 + (size_t)((i + 3) & 1) * row_stride, uin + (size_t)(i + 3) * row_stride, row_bytes,
                      &bars[(i + 3) & 1]);
     }
-    lw_stage<V, false>(hp, hn, ub, rt_cur + (2 * o) * RT_N, th, tau_f, tdx, out);
+    lw_stage<V, false>(Hp, Hn, A, rt_cur + (2 * o) * RT_N, th, tau_f, tdx, out);
     add_source<V>(out, src_f, p, i, false);
     store_row<V, VEC>(out, uout + (size_t)i * row_stride, nth, j0);
-    hp = hn;
-    ub = uc;
     if (VEC) {
       if (i + 2 <= r1) {
         mbar_wait(&bars[(i + 2) & 1], (unsigned)(((i + 2) - (r0 + 2)) >> 1) & 1u);
-        lds_row<V>(uc, slot0 + (size_t)((i + 2) & 1) * row_stride, nth, j0);
+        lds_row<V>(A, slot0 + (size_t)((i + 2) & 1) * row_stride, nth, j0);
       }
     } else {
-      uc = ua;
+      A = ua;
     }
+  };
+  {
+    int i = r0;
+#if TEUK_UNROLL2
+    for (; i + 1 < r1; i += 2) {
+      march(i, ub, uc, hp, hn);
+      march(i + 1, uc, ub, hn, hp);
+    }
+    if (i < r1) march(i, ub, uc, hp, hn);
+#else
+    for (; i < r1; ++i) {
+      march(i, ub, uc, hp, hn);
+      hp = hn;
+      Row<V> t = ub; ub = uc; uc = t;
+    }
+#endif
   }
 
   // radial edges (outer edge: DESIGN.md reading A6)
@@ -442,13 +552,15 @@ __global__ void __launch_bounds__(128) teuk_step_kernel(const __grid_constant__ 
     store_row<V, VEC>(out, uout, nth, j0);
   }
   if (r1 == nr - 1) {
-    // ub = u^n_{nr-1} after the rotation
+    load_row<V, VEC>(ub, uin + (size_t)(nr - 1) * row_stride, nth, j0);
     load_row<V, VEC>(ua, uin + (size_t)(nr - 2) * row_stride, nth, j0);
     const double eps = __ldg(rtab + (size_t)(2 * (nr - 1)) * RT_N + RT_EPS);
+    ThetaVals<V> tv;
+    th.get(tv);
 #pragma unroll
     for (int v = 0; v < V; ++v) {
       if (p.outer_bc == 0) {
-        const double b = rsqrt(fma(-eps, th.s2[v], 1.0));
+        const double b = rsqrt_near_one(fma(-eps, tv.s2[v], 1.0));
         out.c[0][v] = ub.c[0][v] - p.dt * b * (ub.c[0][v] - ua.c[0][v]) / p.dx;
         out.c[1][v] = ub.c[1][v] - p.dt * b * (ub.c[1][v] - ua.c[1][v]) / p.dx;
       } else {
