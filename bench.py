@@ -117,8 +117,10 @@ def oracle_sample_config(cfg, rows):
     lo = -rows // 8
     x0 = round((0.0 - cfg.rs_min) / dx) + lo          # crop starts a little inside x = 0
     rs_min = cfg.rs_min + x0 * dx
-    return cfg.scaled(name=cfg.name + "_crop%d" % rows, n_r=rows, rs_min=rs_min, rs_max=rs_min + (rows - 1) * dx,
-                      dt_over_dx=cfg.dt_over_dx, observers=(50.0,))
+    rs_max = rs_min + (rows - 1) * dx
+    obs = 50.0 if rs_min < 50.0 < rs_max - 2 * dx else rs_min + 0.75 * (rs_max - rs_min)
+    return cfg.scaled(name=cfg.name + "_crop%d" % rows, n_r=rows, rs_min=rs_min, rs_max=rs_max,
+                      dt_over_dx=cfg.dt_over_dx, observers=(obs,))
 
 
 def time_oracle(cfg, steps, warmup, rows):
@@ -141,6 +143,25 @@ def time_oracle(cfg, steps, warmup, rows):
     sample = "%d iterations of a %d x %d radial crop (of %d x %d) incl. source window and observer" % (
         steps, c.n_r, c.n_theta, cfg.n_r, cfg.n_theta)
     return c.n_pts * steps / dt / 1e9, dt, threads, sample
+
+
+def replica_orbit(cfg, rank, n_steps):
+    """Trajectory table of replica `rank`: segment `rank` of the run (PAPER.md:167 temporal
+    parallelisation), i.e. the samples a single long table would hold from iteration rank*n_steps on."""
+    if not cfg.source:
+        return None
+    t0 = rank * n_steps * cfg.dt if cfg.source in ("inspiral", "circular") else 0.0
+    return wl.orbit_table(cfg, n_steps=n_steps, t0=t0)
+
+
+def max_over_ranks(value, device, world):
+    """Device-time reduction of the contract: the slowest rank defines the step time."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
 
 
 def run_reference(args, cfg, rank, world):
@@ -166,7 +187,7 @@ def run_reference(args, cfg, rank, world):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=1000)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=5)
@@ -203,8 +224,7 @@ def main():
 
     K, W = args.steps, args.warmup
     # replica r evolves trajectory segment r: its table starts K+W iterations later
-    orbit = wl.orbit_table(cfg, n_steps=K + W, t0=0.0 if cfg.source != "inspiral" else rank * (K + W) * cfg.dt) \
-        if cfg.source else None
+    orbit = replica_orbit(cfg, rank, K + W)
     weights = wl.observer_weights(cfg)
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
@@ -240,10 +260,7 @@ def main():
         ms = e0.elapsed_time(e1)
         launches = g.stat("launches") - l0
         clocks = sampler.stop() if rank == 0 else None
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+        ms = max_over_ranks(ms, "cuda", world)
         value = world * cfg.n_pts * K / (ms * 1e-3) / 1e9
         # the series recorded so far (W + K samples) are drained to keep the next phase clean
         for x in cfg.observers:
@@ -268,10 +285,8 @@ def main():
             g.get_state(host_out)                   # D2H: 4 planes
             barrier()
             e2e_ms.append(1e3 * (time.perf_counter() - t0))
-        t = torch.tensor([e2e_ms[-1] if e2e_ms else float("inf")], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e = world * cfg.n_pts * K / (float(t.item()) * 1e-3) / 1e9
+        e2e_t = max_over_ranks(e2e_ms[-1] if e2e_ms else float("inf"), "cuda", world)
+        e2e = world * cfg.n_pts * K / (e2e_t * 1e-3) / 1e9
         state_bytes = 4 * cfg.n_pts * 8
         orbit_bytes = 0 if orbit is None else 8 * (2 + 2 * cfg.n_modes) * orbit["n_samples"]
         wave_bytes = sum(len(s[0]) * (8 + 16 * cfg.n_modes) for s in series)
