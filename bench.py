@@ -196,6 +196,7 @@ def main():
     ap.add_argument("--quick", action="store_true", help="development: device-resident timing only")
     ap.add_argument("--slab-rows", type=int, default=0)
     ap.add_argument("--graph", type=int, default=1)
+    ap.add_argument("--kernel", type=int, default=-1, help="-1 library default, 0 register-resident, 1 smem-resident")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     cfg = wl.CONFIGS[args.config]
@@ -233,6 +234,8 @@ def main():
         g.set_option("graph", args.graph)
         if args.slab_rows:
             g.set_option("slab_rows", args.slab_rows)
+        if args.kernel >= 0:
+            g.set_option("kernel", args.kernel)
         # synthetic state resident in HBM: seeded random data on all four planes (throughput does not
         # depend on values; zero data as in the config would let nothing but the source window move)
         gen = torch.Generator(device="cuda").manual_seed(wl.SEED_BASE + cfg.cid + rank)
@@ -243,8 +246,7 @@ def main():
         for x in cfg.observers:
             g.add_observer(x, weights)
         # ---- device-resident timing -----------------------------------------------------------
-        for _ in range(W):
-            g.step(1)
+        g.step(W)
         barrier()
         sampler = ClockSampler(local_rank)
         if rank == 0:
@@ -253,8 +255,7 @@ def main():
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         e0.record(stream)
-        for _ in range(K):
-            g.step(1)
+        g.step(K)            # K iterations: one plain launch, CUDA-graph replays of 32, remainder, flush tap
         e1.record(stream)
         barrier()
         ms = e0.elapsed_time(e1)

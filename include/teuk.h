@@ -110,7 +110,9 @@ int teuk_get_state(teuk_solver *s, double *phi_re, double *phi_im, double *pi_re
  *   "coef_mode"     0 = coefficients recomputed on the fly from 1D tables (default),
  *                   1 = coefficients streamed from precomputed 2D FP64 planes
  *   "slab_rows"     rows of r* marched by one warp (0 = automatic)
- *   "graph"         1 = replay the iteration through a CUDA graph (default), 0 = plain launches */
+ *   "graph"         1 = replay the iteration through a CUDA graph (default), 0 = plain launches
+ *   "kernel"        0 = register-resident marching kernel, 1 = shared-memory-resident marching kernel
+ *                   (same arithmetic, bitwise identical fields; they differ in on-chip residency) */
 int teuk_set_option(teuk_solver *s, const char *key, int64_t value);
 
 /* Read-only counters: "steps" (iterations done), "launches" (kernels launched so far),

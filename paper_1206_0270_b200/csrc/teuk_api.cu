@@ -55,7 +55,7 @@ struct teuk_solver {
   int n_r, n_theta, n_modes;
   int m[TEUK_MAX_MODES];
   // options
-  int outer_bc, coef_mode, slab_rows_opt, use_graph;
+  int outer_bc, coef_mode, slab_rows_opt, use_graph, variant;
   // device
   int device, n_sms;
   cudaStream_t own_stream, stream, copy_stream;
@@ -126,7 +126,7 @@ int auto_slab_rows(const teuk_solver* s) {
   const int interior = s->n_r - 2;
   const int sms = s->n_sms > 0 ? s->n_sms : 148;
   const int v = (s->n_theta + 31) / 32;
-  const int warps_per_sm = v <= 1 ? 16 : (v <= 2 ? 8 : 8);
+  const int warps_per_sm = s->variant == 1 ? 12 : (v <= 1 ? 16 : 8);
   const long long target_warps = (long long)sms * warps_per_sm * 2;
   long long per_mode = target_warps / s->n_modes;
   if (per_mode < 1) per_mode = 1;
@@ -150,6 +150,7 @@ void fill_params(const teuk_solver* s, StepParams* p, int in_buf, int k, int tap
   if (p->slab_rows > s->n_r - 2) p->slab_rows = s->n_r - 2;
   p->n_slabs = (s->n_r - 2 + p->slab_rows - 1) / p->slab_rows;
   p->outer_bc = s->outer_bc;
+  p->variant = s->variant;
   p->dt = s->dt;
   p->dx = s->dx;
   p->rs_min = s->rs_min;
@@ -622,6 +623,9 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
     s->slab_rows_opt = (int)value;
   } else if (!strcmp(key, "graph")) {
     s->use_graph = value ? 1 : 0;
+  } else if (!strcmp(key, "kernel")) {
+    if (value != 0 && value != 1) return fail(s, TEUK_EINVAL, "kernel must be 0 (register-resident) or 1 (shared-memory-resident)");
+    s->variant = (int)value;
   } else {
     return fail(s, TEUK_EINVAL, "teuk_set_option: unknown key");
   }

@@ -58,6 +58,7 @@ struct StepParams {
   const double* coef2d;   // coef_mode 1: [n_modes][2 n_r - 1][8][n_theta] (b,kre,kim,are,aim,gre,gim,cL)
   int n_r, n_theta, n_modes;
   int slab_rows, n_slabs;
+  int variant;            // 0 = register-resident kernel, 1 = shared-memory-resident kernel
   int outer_bc;
   double dt, dx, rs_min, dth;
   // source

@@ -35,9 +35,6 @@ struct Row {
   double c[4][V];  // Phi_R, Phi_I, Pi_R, Pi_I for this lane's V columns
 };
 
-#ifndef TEUK_TT_SMEM
-#define TEUK_TT_SMEM 0   // theta tables: 0 = registers (measured faster), 1 = shared memory (16-byte pieces)
-#endif
 #ifndef TEUK_MIN_BLOCKS
 #define TEUK_MIN_BLOCKS 2
 #endif
@@ -47,8 +44,8 @@ struct Row {
 #ifndef TEUK_UNROLL2
 #define TEUK_UNROLL2 1
 #endif
-#ifndef TEUK_PHASED
-#define TEUK_PHASED 1   // compute the V reciprocal square roots of a stage up front (independent chains)
+#ifndef TEUK_GROUP
+#define TEUK_GROUP 2    // columns processed "vertically" together inside a stage (ILP)
 #endif
 
 // theta-dependent factors of this lane's V columns (rows of teuk_internal.h TT_*)
@@ -57,41 +54,16 @@ struct ThetaVals {
   double s2[V], cs[V], ap[V], am[V], d0[V];
 };
 
-#if TEUK_TT_SMEM
-// Block-shared copy, laid out so that a warp-wide 16-byte load touches 512 contiguous bytes:
-// double index ((tbl * NP + piece) * 32 + lane) * PW + (v % PW), PW = min(V,2), NP = V / PW.
-template <int V>
-struct ThetaTab {
-  const double* base;   // shared memory
-  int lane;
-  __device__ __forceinline__ void get(ThetaVals<V>& t) const {
-    constexpr int PW = V >= 2 ? 2 : 1, NP = V / PW;
-    double* dst[TT_N] = {t.s2, t.cs, t.ap, t.am, t.d0};
-#pragma unroll
-    for (int k = 0; k < TT_N; ++k)
-#pragma unroll
-      for (int q = 0; q < NP; ++q) {
-        const double* src = base + ((k * NP + q) * 32 + lane) * PW;
-        if (PW == 2) {
-          const double2 w = *reinterpret_cast<const double2*>(src);
-          dst[k][2 * q] = w.x;
-          dst[k][2 * q + 1] = w.y;
-        } else {
-          dst[k][q] = src[0];
-        }
-      }
-  }
-};
-#else
 template <int V>
 struct ThetaTab {
   ThetaVals<V> vals;
   __device__ __forceinline__ void get(ThetaVals<V>& t) const { t = vals; }
 };
-#endif
 
 // 1/sqrt(x) for x in (0.9, 1]: MUFU.RSQ64H seed (rel. error < 2^-20) + one third-order step
 // y <- y + y e (1/2 + 3/8 e), e = 1 - x y^2  (error ~ e^3): no range checks, no branch.
+__device__ __forceinline__ double rsqrt_near_one(double x);
+__device__ __forceinline__ double rsqrt_near_one_arg(double x) { return rsqrt_near_one(x); }
 __device__ __forceinline__ double rsqrt_near_one(double x) {
 #if TEUK_FAST_RSQRT
   double y;
@@ -169,13 +141,53 @@ __device__ __forceinline__ void store_row(const Row<V>& u, double* __restrict__ 
   }
 }
 
+// ---- lane <-> column mappings ------------------------------------------------------------------
+// MAP 0 (register-resident kernel): lane owns V contiguous columns j = lane*V + v.
+// MAP 1 (shared-memory-resident kernel): lane owns V/2 two-column pieces, j = (v/2)*64 + 2*lane + (v&1)
+//        (V = 1: j = lane), so a warp-wide 16-byte access touches 512 contiguous bytes: shared-memory
+//        reads are bank-conflict free and global stores are fully coalesced.
+template <int V, int MAP>
+__device__ __forceinline__ int col_of(int lane, int v) {
+  if (MAP == 0 || V == 1) return lane * V + v;
+  return (v >> 1) * 64 + 2 * lane + (v & 1);
+}
+
+// theta-neighbours of f[v] across lanes: lf[v] = f at column-1, rt[v] = f at column+1 (values beyond
+// the poles are garbage-but-finite: their coefficients are zero, see teuk_ttab_kernel).
+template <int V, int MAP>
+__device__ __forceinline__ void theta_neighbours(const double (&f)[V], double (&lf)[V], double (&rt)[V], int lane) {
+  if (MAP == 0 || V == 1) {
+    const double l = __shfl_up_sync(FULL, f[V - 1], 1), r = __shfl_down_sync(FULL, f[0], 1);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      lf[v] = (v > 0) ? f[v > 0 ? v - 1 : 0] : l;
+      rt[v] = (v < V - 1) ? f[v < V - 1 ? v + 1 : 0] : r;
+    }
+  } else {
+    constexpr int NP = V / 2;
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+      // right neighbour of (q, lane, 1): (q, lane+1, 0), or (q+1, 0, 0) for lane 31
+      const double send_r = (lane == 0 && q + 1 < NP) ? f[2 * (q + 1 < NP ? q + 1 : q)] : f[2 * q];
+      // left neighbour of (q, lane, 0): (q, lane-1, 1), or (q-1, 31, 1) for lane 0
+      const double send_l = (lane == 31 && q > 0) ? f[2 * (q > 0 ? q - 1 : 0) + 1] : f[2 * q + 1];
+      const double r = __shfl_sync(FULL, send_r, (lane + 1) & 31);
+      const double l = __shfl_sync(FULL, send_l, (lane + 31) & 31);
+      lf[2 * q] = l;
+      lf[2 * q + 1] = f[2 * q];
+      rt[2 * q] = f[2 * q + 1];
+      rt[2 * q + 1] = r;
+    }
+  }
+}
+
 // ---- one Lax-Wendroff stage at one radial location ------------------------------------------
 // HALF: A = u^n_i, B = u^n_{i+1}, out = 2 u^{n+1/2}_{i+1/2}             (Eq. 3, tau = dt/2)
 // else: A = H_{i-1/2}, B = H_{i+1/2} (doubled), out = u^{n+1}_i, base = u^n_i   (Eq. 4, tau = dt/4)
-template <int V, bool HALF>
+template <int V, bool HALF, int MAP = 0>
 __device__ __forceinline__ void lw_stage(const Row<V>& A, const Row<V>& B, const Row<V>& base,
                                          const double* __restrict__ rec, const ThetaTab<V>& tht,
-                                         double tau, double two_over_dx, Row<V>& out) {
+                                         double tau, double two_over_dx, Row<V>& out, int lane = 0) {
   ThetaVals<V> th;
   tht.get(th);
   const double2 r01 = *reinterpret_cast<const double2*>(rec + 0);
@@ -193,55 +205,49 @@ __device__ __forceinline__ void lw_stage(const Row<V>& A, const Row<V>& B, const
     sfi[v] = A.c[1][v] + B.c[1][v];
   }
   // theta-neighbours across lanes (pole ghosts are folded into ap/am/d0; see teuk_ttab_kernel)
-  const double left_r = __shfl_up_sync(FULL, sfr[V - 1], 1), left_i = __shfl_up_sync(FULL, sfi[V - 1], 1);
-  const double right_r = __shfl_down_sync(FULL, sfr[0], 1), right_i = __shfl_down_sync(FULL, sfi[0], 1);
-#if TEUK_PHASED
-  double bv[V];
+  double nlr[V], nrr[V], nli[V], nri[V];
+  theta_neighbours<V, MAP>(sfr, nlr, nrr, lane);
+  theta_neighbours<V, MAP>(sfi, nli, nri, lane);
+  // The V columns are processed in groups of G: inside a group every operation is written for all
+  // G columns back to back, so consecutive FP64 instructions are independent (DFMA latency is 8
+  // cycles at one issue per 2 cycles: a lone dependent chain leaves the pipe 3/4 idle).
+  constexpr int G = (TEUK_GROUP < V) ? TEUK_GROUP : V;
 #pragma unroll
-  for (int v = 0; v < V; ++v) bv[v] = rsqrt_near_one(fma(-eps, th.s2[v], 1.0));
-#endif
-#pragma unroll
-  for (int v = 0; v < V; ++v) {
-    const double dfr = B.c[0][v] - A.c[0][v], dfi = B.c[1][v] - A.c[1][v];
-    const double spr = A.c[2][v] + B.c[2][v], spi = A.c[3][v] + B.c[3][v];
-    const double dpr = B.c[2][v] - A.c[2][v], dpi = B.c[3][v] - A.c[3][v];
-    const double fmr = (v > 0) ? sfr[v > 0 ? v - 1 : 0] : left_r, fmi = (v > 0) ? sfi[v > 0 ? v - 1 : 0] : left_i;
-    const double fpr = (v < V - 1) ? sfr[v < V - 1 ? v + 1 : 0] : right_r;
-    const double fpi = (v < V - 1) ? sfi[v < V - 1 ? v + 1 : 0] : right_i;
-    // coefficients at (r, theta_j)
-#if TEUK_PHASED
-    const double b = bv[v];
-#else
-    const double b = rsqrt_near_one(fma(-eps, th.s2[v], 1.0));
-#endif
-    const double Q = b * b;
-    const double b2d = b * two_over_dx;
-    const double aim = fma(a2, th.cs[v], a1);
-    const double diag = th.d0[v] - gr;
-    const double bre = fma(-Q, th.s2[v] * x32, bre2);
+  for (int v0 = 0; v0 < V; v0 += G) {
+    double dfr[G], dfi[G], spr[G], spi[G], dpr[G], dpi[G], b[G], Q[G], b2d[G], aim[G], diag[G], bre[G];
+    double e2r[G], e2i[G], ltr[G], lti[G], br[G], bi[G];
+#define FORG _Pragma("unroll") for (int g = 0; g < G; ++g)
+    FORG b[g] = fma(-eps, th.s2[v0 + g], 1.0);
+    FORG b[g] = rsqrt_near_one_arg(b[g]);
+    FORG { dfr[g] = B.c[0][v0 + g] - A.c[0][v0 + g]; dfi[g] = B.c[1][v0 + g] - A.c[1][v0 + g]; }
+    FORG { spr[g] = A.c[2][v0 + g] + B.c[2][v0 + g]; spi[g] = A.c[3][v0 + g] + B.c[3][v0 + g]; }
+    FORG { dpr[g] = B.c[2][v0 + g] - A.c[2][v0 + g]; dpi[g] = B.c[3][v0 + g] - A.c[3][v0 + g]; }
+    FORG { aim[g] = fma(a2, th.cs[v0 + g], a1); diag[g] = th.d0[v0 + g] - gr; }
+    FORG { Q[g] = b[g] * b[g]; b2d[g] = b[g] * two_over_dx; }
+    FORG bre[g] = fma(-Q[g], th.s2[v0 + g] * x32, bre2);
     // E2 = 2 (Pi - b dPhi/dx)
-    const double e2r = fma(-b2d, dfr, spr), e2i = fma(-b2d, dfi, spi);
-    out.c[0][v] = fma(tau, e2r, HALF ? sfr[v] : base.c[0][v]);
-    out.c[1][v] = fma(tau, e2i, HALF ? sfi[v] : base.c[1][v]);
+    FORG { e2r[g] = fma(-b2d[g], dfr[g], spr[g]); e2i[g] = fma(-b2d[g], dfi[g], spi[g]); }
+    FORG {
+      out.c[0][v0 + g] = fma(tau, e2r[g], HALF ? sfr[v0 + g] : base.c[0][v0 + g]);
+      out.c[1][v0 + g] = fma(tau, e2i[g], HALF ? sfi[v0 + g] : base.c[1][v0 + g]);
+    }
     // L'_theta S_Phi
-    const double ltr = fma(th.ap[v], fpr, fma(th.am[v], fmr, diag * sfr[v]));
-    const double lti = fma(th.ap[v], fpi, fma(th.am[v], fmi, diag * sfi[v]));
-    // bracket B
-    double br = bre * dfr;
-    br = fma(-bim2, dfi, br);
-    br = fma(a0, e2r, br);
-    br = fma(-aim, e2i, br);
-    br = fma(cl, ltr, br);
-    br = fma(-g1, sfi[v], br);
-    double bi = bre * dfi;
-    bi = fma(bim2, dfr, bi);
-    bi = fma(a0, e2i, bi);
-    bi = fma(aim, e2r, bi);
-    bi = fma(cl, lti, bi);
-    bi = fma(g1, sfr[v], bi);
-    const double tr = fma(b2d, dpr, Q * br), ti = fma(b2d, dpi, Q * bi);
-    out.c[2][v] = fma(tau, tr, HALF ? spr : base.c[2][v]);
-    out.c[3][v] = fma(tau, ti, HALF ? spi : base.c[3][v]);
+    FORG { ltr[g] = diag[g] * sfr[v0 + g]; lti[g] = diag[g] * sfi[v0 + g]; }
+    FORG { ltr[g] = fma(th.am[v0 + g], nlr[v0 + g], ltr[g]); lti[g] = fma(th.am[v0 + g], nli[v0 + g], lti[g]); }
+    FORG { ltr[g] = fma(th.ap[v0 + g], nrr[v0 + g], ltr[g]); lti[g] = fma(th.ap[v0 + g], nri[v0 + g], lti[g]); }
+    // bracket B (same order of operations for every G: results do not depend on the grouping)
+    FORG { br[g] = bre[g] * dfr[g]; bi[g] = bre[g] * dfi[g]; }
+    FORG { br[g] = fma(-bim2, dfi[g], br[g]); bi[g] = fma(bim2, dfr[g], bi[g]); }
+    FORG { br[g] = fma(a0, e2r[g], br[g]); bi[g] = fma(a0, e2i[g], bi[g]); }
+    FORG { br[g] = fma(-aim[g], e2i[g], br[g]); bi[g] = fma(aim[g], e2r[g], bi[g]); }
+    FORG { br[g] = fma(cl, ltr[g], br[g]); bi[g] = fma(cl, lti[g], bi[g]); }
+    FORG { br[g] = fma(-g1, sfi[v0 + g], br[g]); bi[g] = fma(g1, sfr[v0 + g], bi[g]); }
+    FORG { br[g] = fma(b2d[g], dpr[g], Q[g] * br[g]); bi[g] = fma(b2d[g], dpi[g], Q[g] * bi[g]); }
+    FORG {
+      out.c[2][v0 + g] = fma(tau, br[g], HALF ? spr[g] : base.c[2][v0 + g]);
+      out.c[3][v0 + g] = fma(tau, bi[g], HALF ? spi[g] : base.c[3][v0 + g]);
+    }
+#undef FORG
   }
 }
 
@@ -263,9 +269,9 @@ struct StageSource {
   double gth[V];    // g(theta_j - theta_p) inside |j - jp| <= W, else 0
 };
 
-template <int V>
+template <int V, int MAP = 0>
 __device__ __forceinline__ void setup_source(StageSource<V>& s, const StepParams& p, int mode, long long ks,
-                                             bool half, int row_lo, int row_hi, int j0) {
+                                             bool half, int row_lo, int row_hi, int lane) {
   s.on = false;
   if (!p.has_source) return;
   const double xp = p.xp[ks], thp = p.thp[ks];
@@ -282,7 +288,7 @@ __device__ __forceinline__ void setup_source(StageSource<V>& s, const StepParams
   s.aim = p.amp_im[(size_t)mode * p.n_samples + ks];
 #pragma unroll
   for (int q = 0; q < V; ++q) {
-    const int j = j0 + q;
+    const int j = col_of<V, MAP>(lane, q);
     const double th = __dmul_rn((double)j + 0.5, p.dth);
     s.gth[q] = (j < p.n_theta && abs(j - jp) <= p.W) ? gauss_dev(th - thp, p.sigma_th) : 0.0;
   }
@@ -305,16 +311,17 @@ __device__ __forceinline__ void add_source(Row<V>& out, const StageSource<V>& s,
 }
 
 // Waveform tap of the INPUT state (sample n): w = sum_j W_j [(1-f) Phi_{i0,j} + f Phi_{i0+1,j}].
-template <int V>
+template <int V, int MAP = 0>
 __device__ __forceinline__ void tap(const Row<V>& lo, const Row<V>& hi, const StepParams& p, int i, int mode,
-                                    long long n, int j0, int lane) {
+                                    long long n, int lane) {
   for (int q = 0; q < p.n_obs; ++q) {
     if (p.obs[q].i0 != i) continue;
     const double f = p.obs[q].f;
     double wr = 0.0, wi = 0.0;
 #pragma unroll
     for (int v = 0; v < V; ++v) {
-      const double wt = (j0 + v < p.n_theta) ? __ldg(p.obs[q].weights + j0 + v) : 0.0;
+      const int j = col_of<V, MAP>(lane, v);
+      const double wt = (j < p.n_theta) ? __ldg(p.obs[q].weights + j) : 0.0;
       wr = fma(wt, fma(f, hi.c[0][v], (1.0 - f) * lo.c[0][v]), wr);
       wi = fma(wt, fma(f, hi.c[1][v], (1.0 - f) * lo.c[1][v]), wi);
     }
@@ -407,21 +414,6 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
   const int slab = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   const int mode = blockIdx.y;
   const int nth = p.n_theta, nr = p.n_r;
-#if TEUK_TT_SMEM
-  __shared__ __align__(16) double s_tt[TT_N * 32 * V];
-  {
-    constexpr int PW = V >= 2 ? 2 : 1, NP = V / PW;
-    const double* tb = p.ttab + (size_t)mode * TT_N * nth;
-    for (int t = threadIdx.x; t < TT_N * 32 * V; t += blockDim.x) {
-      const int k = t / (32 * V), r = t - k * 32 * V;      // table, position inside the table
-      const int q = r / (32 * PW), l = (r / PW) % 32, w = r % PW;
-      const int j = l * V + q * PW + w;                    // column owned by lane l
-      s_tt[t] = (j < nth) ? tb[k * nth + j] : 0.0;
-      (void)NP;
-    }
-    __syncthreads();
-  }
-#endif
   if (slab >= p.n_slabs) return;
   const int r0 = 1 + slab * p.slab_rows;             // first interior node of this slab
   const int r1 = min(r0 + p.slab_rows, nr - 1);      // one past the last
@@ -455,10 +447,6 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
   }
 
   ThetaTab<V> th;
-#if TEUK_TT_SMEM
-  th.base = s_tt;
-  th.lane = lane;
-#else
   {
     const double* tb = p.ttab + (size_t)mode * TT_N * nth;
 #pragma unroll
@@ -471,10 +459,9 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
       th.vals.d0[v] = ok ? tb[TT_D0 * nth + j0 + v] : 0.0;
     }
   }
-#endif
   StageSource<V> src_h, src_f;   // half stage: sample 2n at half points; full stage: 2n+1 at nodes
-  setup_source<V>(src_h, p, mode, 2 * n, true, r0 - 1, r1 - 1, j0);
-  setup_source<V>(src_f, p, mode, 2 * n + 1, false, r0, r1 - 1, j0);
+  setup_source<V>(src_h, p, mode, 2 * n, true, r0 - 1, r1 - 1, lane);
+  setup_source<V>(src_f, p, mode, 2 * n + 1, false, r0, r1 - 1, lane);
   const bool do_tap = p.tap_enable && p.n_obs > 0 && n >= 1;
   const double tau_h = 0.5 * p.dt, tau_f = 0.25 * p.dt, tdx = 2.0 / p.dx;
 
@@ -482,7 +469,7 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
   load_row<V, VEC>(ua, uin + (size_t)(r0 - 1) * row_stride, nth, j0);
   load_row<V, VEC>(ub, uin + (size_t)r0 * row_stride, nth, j0);
   load_row<V, VEC>(uc, uin + (size_t)(r0 + 1) * row_stride, nth, j0);
-  if (do_tap && r0 == 1) tap<V>(ua, ub, p, 0, mode, n, j0, lane);
+  if (do_tap && r0 == 1) tap<V>(ua, ub, p, 0, mode, n, lane);
   lw_stage<V, true>(ua, ub, ua, rtab + (size_t)(2 * (r0 - 1) + 1) * RT_N, th, tau_h, tdx, hp);
   add_source<V>(hp, src_h, p, r0 - 1, true);
 
@@ -503,7 +490,7 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
       if (i + RT_CH < r1)
         stage_rtab_chunk(rt_buf + ((c + 1) & 1) * RT_CHUNK_DOUBLES, rtab, 2 * (i + RT_CH), 2 * nr - 1, lane);
     }
-    if (do_tap) tap<V>(A, B, p, i, mode, n, j0, lane);
+    if (do_tap) tap<V>(A, B, p, i, mode, n, lane);
     lw_stage<V, true>(A, B, A, rt_cur + (2 * o + 1) * RT_N, th, tau_h, tdx, Hn);
     add_source<V>(Hn, src_h, p, i, true);
     if (VEC) {
@@ -574,6 +561,239 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
   }
 }
 
+// ================================================================================================
+// Shared-memory-resident variant (variant 1).  Same arithmetic per point as teuk_step_kernel (the
+// two produce bitwise identical fields), different residency: only u^n_i lives in registers across
+// iterations; u^n_{i+1} is read from its TMA landing slot where it is used, and the half-step row
+// 2u^{n+1/2}_{i-1/2} lives in a per-warp shared-memory slot.  That brings the kernel under 168
+// registers, i.e. 12 instead of 8 warps per SM, which is what the fixed-latency `wait` stalls of the
+// register-resident kernel ask for (profiles/r1_step_kernel_full.md).  Lane <-> column mapping MAP 1.
+namespace {
+
+template <int V, bool EVEN>
+__device__ __forceinline__ void piece_load(Row<V>& u, const double* row, int nth, int lane) {
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    if (V == 1) {
+      u.c[c][0] = (lane < nth) ? row[c * nth + lane] : 0.0;
+    } else {
+#pragma unroll
+      for (int q = 0; q < V / 2; ++q) {
+        const int j = q * 64 + 2 * lane;
+        if (EVEN) {
+          double2 t = make_double2(0.0, 0.0);
+          if (j < nth) t = *reinterpret_cast<const double2*>(row + c * nth + j);
+          u.c[c][2 * q] = t.x;
+          u.c[c][2 * q + 1] = t.y;
+        } else {
+          u.c[c][2 * q] = (j < nth) ? row[c * nth + j] : 0.0;
+          u.c[c][2 * q + 1] = (j + 1 < nth) ? row[c * nth + j + 1] : 0.0;
+        }
+      }
+    }
+  }
+}
+
+template <int V, bool EVEN>
+__device__ __forceinline__ void piece_store_global(const Row<V>& u, double* __restrict__ row, int nth, int lane) {
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    if (V == 1) {
+      if (lane < nth) __stcs(row + c * nth + lane, u.c[c][0]);
+    } else {
+#pragma unroll
+      for (int q = 0; q < V / 2; ++q) {
+        const int j = q * 64 + 2 * lane;
+        if (EVEN) {
+          if (j < nth) __stcs(reinterpret_cast<double2*>(row + c * nth + j), make_double2(u.c[c][2 * q], u.c[c][2 * q + 1]));
+        } else {
+          if (j < nth) __stcs(row + c * nth + j, u.c[c][2 * q]);
+          if (j + 1 < nth) __stcs(row + c * nth + j + 1, u.c[c][2 * q + 1]);
+        }
+      }
+    }
+  }
+}
+
+// private half-row slot: [comp][piece][lane] 16-byte entries (V = 1: [comp][lane] doubles)
+template <int V>
+__device__ __forceinline__ void hslot_store(const Row<V>& h, double* slot, int lane) {
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    if (V == 1) {
+      slot[c * 32 + lane] = h.c[c][0];
+    } else {
+#pragma unroll
+      for (int q = 0; q < V / 2; ++q)
+        *reinterpret_cast<double2*>(slot + ((c * (V / 2) + q) * 32 + lane) * 2) = make_double2(h.c[c][2 * q], h.c[c][2 * q + 1]);
+    }
+  }
+}
+template <int V>
+__device__ __forceinline__ void hslot_load(Row<V>& h, const double* slot, int lane) {
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    if (V == 1) {
+      h.c[c][0] = slot[c * 32 + lane];
+    } else {
+#pragma unroll
+      for (int q = 0; q < V / 2; ++q) {
+        const double2 t = *reinterpret_cast<const double2*>(slot + ((c * (V / 2) + q) * 32 + lane) * 2);
+        h.c[c][2 * q] = t.x;
+        h.c[c][2 * q + 1] = t.y;
+      }
+    }
+  }
+}
+
+}  // namespace
+
+#ifndef TEUK_SMEM_MIN_BLOCKS
+#define TEUK_SMEM_MIN_BLOCKS 3
+#endif
+
+template <int V, bool EVEN>
+__global__ void __launch_bounds__(128, TEUK_SMEM_MIN_BLOCKS) teuk_step_smem_kernel(const __grid_constant__ StepParams p) {
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  const int slab = blockIdx.x * (blockDim.x >> 5) + wib;
+  const int mode = blockIdx.y;
+  if (slab >= p.n_slabs) return;
+  const int nth = p.n_theta, nr = p.n_r;
+  const int r0 = 1 + slab * p.slab_rows;
+  const int r1 = min(r0 + p.slab_rows, nr - 1);
+  const size_t row_stride = (size_t)4 * nth;
+  const double* __restrict__ uin = p.uin + (size_t)mode * nr * row_stride;
+  double* __restrict__ uout = p.uout + (size_t)mode * nr * row_stride;
+  const double* __restrict__ rtab = p.rtab + (size_t)mode * (2 * nr - 1) * RT_N;
+  const long long n = *p.d_base + p.k;
+
+  __shared__ __align__(16) double s_rt[4][2][RT_CHUNK_DOUBLES];
+  __shared__ __align__(8) unsigned long long s_bar[4][2];
+  extern __shared__ __align__(128) unsigned char s_dyn[];  // per warp: 2 row slots + 1 half-row slot
+  const size_t warp_doubles = 2 * row_stride + (size_t)4 * 32 * V;
+  double* const slot0 = reinterpret_cast<double*>(s_dyn) + (size_t)wib * warp_doubles;
+  double* const hslot = slot0 + 2 * row_stride;
+  double* const rt_buf = &s_rt[wib][0][0];
+  unsigned long long* const bars = &s_bar[wib][0];
+  const unsigned row_bytes = (unsigned)(row_stride * sizeof(double));
+  // row q uses slot q & 1; its k-th use of the slot has mbarrier parity k & 1
+  auto slot_of = [&](int q) { return slot0 + (size_t)(q & 1) * row_stride; };
+  auto issue = [&](int q) { tma_load_row(slot_of(q), uin + (size_t)q * row_stride, row_bytes, &bars[q & 1]); };
+  auto wait_row = [&](int q) { mbar_wait(&bars[q & 1], (unsigned)((q - (r0 - 1)) >> 1) & 1u); };
+
+  if (lane == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    issue(r0 - 1);
+    issue(r0);
+  }
+  __syncwarp();
+  stage_rtab_chunk(rt_buf, rtab, 2 * r0, 2 * nr - 1, lane);
+
+  ThetaTab<V> th;
+  {
+    const double* tb = p.ttab + (size_t)mode * TT_N * nth;
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const int j = col_of<V, 1>(lane, v);
+      const bool ok = j < nth;
+      th.vals.s2[v] = ok ? tb[TT_S2 * nth + j] : 0.0;
+      th.vals.cs[v] = ok ? tb[TT_COS * nth + j] : 0.0;
+      th.vals.ap[v] = ok ? tb[TT_AP * nth + j] : 0.0;
+      th.vals.am[v] = ok ? tb[TT_AM * nth + j] : 0.0;
+      th.vals.d0[v] = ok ? tb[TT_D0 * nth + j] : 0.0;
+    }
+  }
+  StageSource<V> src_h, src_f;
+  setup_source<V, 1>(src_h, p, mode, 2 * n, true, r0 - 1, r1 - 1, lane);
+  setup_source<V, 1>(src_f, p, mode, 2 * n + 1, false, r0, r1 - 1, lane);
+  const bool do_tap = p.tap_enable && p.n_obs > 0 && n >= 1;
+  const double tau_h = 0.5 * p.dt, tau_f = 0.25 * p.dt, tdx = 2.0 / p.dx;
+
+  Row<V> A, out;
+  {  // prologue: half step at (r0-1)+1/2
+    Row<V> B, H;
+    wait_row(r0 - 1);
+    wait_row(r0);
+    piece_load<V, EVEN>(A, slot_of(r0 - 1), nth, lane);
+    piece_load<V, EVEN>(B, slot_of(r0), nth, lane);
+    if (do_tap && r0 == 1) tap<V, 1>(A, B, p, 0, mode, n, lane);
+    lw_stage<V, true, 1>(A, B, A, rtab + (size_t)(2 * (r0 - 1) + 1) * RT_N, th, tau_h, tdx, H, lane);
+    add_source<V>(H, src_h, p, r0 - 1, true);
+    hslot_store<V>(H, hslot, lane);
+    A = B;
+    __syncwarp();
+    if (lane == 0) issue(r0 + 1);   // into the slot of row r0-1, read by every lane above
+    wait_row(r0 + 1);
+  }
+
+  const double* rt_cur = rt_buf;
+  for (int i = r0; i < r1; ++i) {
+    // A = u^n_i (registers); u^n_{i+1} has landed in slot (i+1)&1; hslot = 2 u^{n+1/2}_{i-1/2}
+    __syncwarp();
+    if (lane == 0 && i + 2 <= r1) issue(i + 2);   // slot i&1: row i was copied into A by every lane
+    const int o = (i - r0) & (RT_CH - 1);
+    if (o == 0) {
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+      __syncwarp();
+      const int c = (i - r0) / RT_CH;
+      rt_cur = rt_buf + (c & 1) * RT_CHUNK_DOUBLES;
+      if (i + RT_CH < r1)
+        stage_rtab_chunk(rt_buf + ((c + 1) & 1) * RT_CHUNK_DOUBLES, rtab, 2 * (i + RT_CH), 2 * nr - 1, lane);
+    }
+    Row<V> Hn;
+    {
+      Row<V> B;
+      piece_load<V, EVEN>(B, slot_of(i + 1), nth, lane);
+      if (do_tap) tap<V, 1>(A, B, p, i, mode, n, lane);
+      lw_stage<V, true, 1>(A, B, A, rt_cur + (2 * o + 1) * RT_N, th, tau_h, tdx, Hn, lane);
+      add_source<V>(Hn, src_h, p, i, true);
+    }
+    {
+      Row<V> Hp;
+      hslot_load<V>(Hp, hslot, lane);
+      lw_stage<V, false, 1>(Hp, Hn, A, rt_cur + (2 * o) * RT_N, th, tau_f, tdx, out, lane);
+      add_source<V>(out, src_f, p, i, false);
+    }
+    piece_store_global<V, EVEN>(out, uout + (size_t)i * row_stride, nth, lane);
+    hslot_store<V>(Hn, hslot, lane);
+    piece_load<V, EVEN>(A, slot_of(i + 1), nth, lane);   // u^n_{i+1} becomes the register row
+    if (i + 2 <= r1) wait_row(i + 2);
+  }
+
+  if (r0 == 1) {
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+      for (int v = 0; v < V; ++v) out.c[c][v] = 0.0;
+    piece_store_global<V, EVEN>(out, uout, nth, lane);
+  }
+  if (r1 == nr - 1) {
+    Row<V> L, K;
+    piece_load<V, EVEN>(L, uin + (size_t)(nr - 1) * row_stride, nth, lane);
+    piece_load<V, EVEN>(K, uin + (size_t)(nr - 2) * row_stride, nth, lane);
+    const double eps = __ldg(rtab + (size_t)(2 * (nr - 1)) * RT_N + RT_EPS);
+    ThetaVals<V> tv;
+    th.get(tv);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      if (p.outer_bc == 0) {
+        const double b = rsqrt_near_one(fma(-eps, tv.s2[v], 1.0));
+        out.c[0][v] = L.c[0][v] - p.dt * b * (L.c[0][v] - K.c[0][v]) / p.dx;
+        out.c[1][v] = L.c[1][v] - p.dt * b * (L.c[1][v] - K.c[1][v]) / p.dx;
+      } else {
+        out.c[0][v] = 0.0;
+        out.c[1][v] = 0.0;
+      }
+      out.c[2][v] = 0.0;
+      out.c[3][v] = 0.0;
+    }
+    piece_store_global<V, EVEN>(out, uout + (size_t)(nr - 1) * row_stride, nth, lane);
+  }
+}
+
 // Tap of the CURRENT state at the end of a teuk_step call (the in-kernel tap records the input
 // level of each iteration, so the last level needs one tiny launch).  One warp per (mode, observer).
 __global__ void teuk_flush_tap_kernel(const __grid_constant__ StepParams p) {
@@ -590,8 +810,8 @@ __global__ void teuk_flush_tap_kernel(const __grid_constant__ StepParams p) {
   const int vreq = (nth + 31) / 32;
   const int V = vreq <= 1 ? 1 : (vreq <= 2 ? 2 : (vreq <= 4 ? 4 : 8));
   for (int v = 0; v < V; ++v) {
-    const int j = lane * V + v;
-    if (j >= nth) break;
+    const int j = (p.variant == 1 && V > 1) ? (v >> 1) * 64 + 2 * lane + (v & 1) : lane * V + v;
+    if (j >= nth) continue;
     const double wt = p.obs[q].weights[j];
     wr = fma(wt, fma(f, hi[j], (1.0 - f) * lo[j]), wr);
     wi = fma(wt, fma(f, hi[nth + j], (1.0 - f) * lo[nth + j]), wi);
@@ -658,8 +878,40 @@ static cudaError_t launch_v(const StepParams& p, cudaStream_t st) {
   return cudaGetLastError();
 }
 
+template <int V>
+static cudaError_t launch_smem_v(const StepParams& p, cudaStream_t st) {
+  const int warps_per_block = 4;
+  dim3 grid((p.n_slabs + warps_per_block - 1) / warps_per_block, p.n_modes), block(32 * warps_per_block);
+  const size_t dyn = (size_t)warps_per_block * (2 * 4 * (size_t)p.n_theta + 4 * 32 * V) * sizeof(double);
+  const int dyn_max = (int)((size_t)warps_per_block * (2 * 4 * 32 * V + 4 * 32 * V) * sizeof(double));
+  if (p.n_theta % 2 == 0 || V == 1) {
+    static bool attr_set = false;
+    if (!attr_set) {
+      cudaError_t e = cudaFuncSetAttribute(teuk_step_smem_kernel<V, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max);
+      if (e != cudaSuccess) return e;
+      attr_set = true;
+    }
+    teuk_step_smem_kernel<V, true><<<grid, block, dyn, st>>>(p);
+  } else {
+    static bool attr_set = false;
+    if (!attr_set) {
+      cudaError_t e = cudaFuncSetAttribute(teuk_step_smem_kernel<V, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max);
+      if (e != cudaSuccess) return e;
+      attr_set = true;
+    }
+    teuk_step_smem_kernel<V, false><<<grid, block, dyn, st>>>(p);
+  }
+  return cudaGetLastError();
+}
+
 cudaError_t teuk_launch_step(const StepParams& p, cudaStream_t st) {
   const int v = (p.n_theta + 31) / 32;
+  if (p.variant == 1) {
+    if (v <= 1) return launch_smem_v<1>(p, st);
+    if (v <= 2) return launch_smem_v<2>(p, st);
+    if (v <= 4) return launch_smem_v<4>(p, st);
+    return launch_smem_v<8>(p, st);
+  }
   if (v <= 1) return launch_v<1>(p, st);
   if (v <= 2) return launch_v<2>(p, st);
   if (v <= 4) return launch_v<4>(p, st);

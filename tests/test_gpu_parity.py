@@ -243,3 +243,33 @@ def test_nonfinite_sentinel(teuk):
         g.extract(cfg.rs_min + 200 * cfg.dx + 0.01)
     assert e.value.code == teuk.TEUK_ENONFINITE
     g.close()
+
+
+@pytest.mark.parametrize("n_theta", [8, 32, 45, 64, 100, 128, 131, 200, 256])
+def test_kernel_variants_agree_bitwise(orc, teuk, n_theta):
+    """The register-resident and the shared-memory-resident kernels do the same arithmetic per point:
+    fields must agree bit for bit; waveforms differ only in the summation order over theta."""
+    cfg = SMALL[3].scaled(name="kv%d" % n_theta, n_r=333, n_theta=n_theta, dt_over_dx=0.02, steps=40, modes=(2, 3))
+    out = []
+    for kernel in (0, 1):
+        g = teuk.Solver.from_config(cfg)
+        g.set_option("kernel", kernel)
+        g.set_initial(*wl.random_state(cfg, 9))
+        g.set_source(wl.orbit_table(cfg, n_steps=40))
+        g.add_observer(30.0, wl.observer_weights(cfg))
+        g.step(7)
+        g.step(33)
+        out.append((g.get_state(), g.extract(30.0)))
+        g.close()
+    for a, b in zip(out[0][0], out[1][0]):
+        assert np.array_equal(a, b)
+    assert rel_l2(out[1][1][1], out[0][1][1]) < 1e-13
+
+
+@pytest.mark.parametrize("cfg", SMALL, ids=[c.name for c in SMALL])
+def test_smem_kernel_parity(orc, teuk, cfg):
+    res = run_pair(orc, teuk, cfg, min(cfg.steps, 300), options={"kernel": 1})
+    check_pair(res)
+    for slab in (1, 5):
+        res = run_pair(orc, teuk, cfg, 4, initial=wl.random_state(cfg, 31), options={"kernel": 1, "slab_rows": slab})
+        check_pair(res, tol=1e-12)
