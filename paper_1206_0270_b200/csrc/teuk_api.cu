@@ -16,6 +16,8 @@
 // kernels / launchers defined in the other translation units
 cudaError_t teuk_launch_tables(double* rtab, double* ttab, const int* d_m, int n_modes, int n_r, int n_theta,
                                double rs_min, double dx, double dth, double M, double a, cudaStream_t st);
+cudaError_t teuk_launch_coef2d(double* c2d, const double* rtab, const double* ttab, int n_modes, int n_r,
+                               int n_theta, double dx, cudaStream_t st);
 cudaError_t teuk_launch_step(const StepParams& p, cudaStream_t st);
 cudaError_t teuk_launch_flush_tap(const StepParams& p, cudaStream_t st);
 cudaError_t teuk_launch_bump(long long* d_base, long long inc, cudaStream_t st);
@@ -143,6 +145,7 @@ void fill_params(const teuk_solver* s, StepParams* p, int in_buf, int k, int tap
   p->rtab = s->d_rtab;
   p->ttab = s->d_ttab;
   p->coef2d = s->d_coef2d;
+  p->coef_mode = s->coef_mode;
   p->n_r = s->n_r;
   p->n_theta = s->n_theta;
   p->n_modes = s->n_modes;
@@ -616,7 +619,15 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
   } else if (!strcmp(key, "stream")) {
     s->stream = value ? (cudaStream_t)(uintptr_t)value : s->own_stream;
   } else if (!strcmp(key, "coef_mode")) {
-    if (value != 0) return fail(s, TEUK_EINVAL, "coef_mode 1 (streamed 2D coefficient planes) is not built in this round");
+    if (value != 0 && value != 1) return fail(s, TEUK_EINVAL, "coef_mode must be 0 or 1");
+    if (value == 1 && s->variant != 0) return fail(s, TEUK_EINVAL, "coef_mode 1 needs kernel 0");
+    if (value == 1 && !s->d_coef2d) {
+      const size_t bytes = (size_t)s->n_modes * (2 * (size_t)s->n_r - 1) * 8 * s->n_theta * sizeof(double);
+      CK(cudaMalloc((void**)&s->d_coef2d, bytes), "coef_mode: alloc of the 2D coefficient planes");
+      CK(teuk_launch_coef2d(s->d_coef2d, s->d_rtab, s->d_ttab, s->n_modes, s->n_r, s->n_theta, s->dx, s->stream),
+         "coef_mode: plane kernel");
+      s->launches += 1;
+    }
     s->coef_mode = (int)value;
   } else if (!strcmp(key, "slab_rows")) {
     if (value < 0 || value > (1 << 30)) return fail(s, TEUK_EINVAL, "slab_rows out of range");
@@ -625,6 +636,7 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
     s->use_graph = value ? 1 : 0;
   } else if (!strcmp(key, "kernel")) {
     if (value != 0 && value != 1) return fail(s, TEUK_EINVAL, "kernel must be 0 (register-resident) or 1 (shared-memory-resident)");
+    if (value == 1 && s->coef_mode != 0) return fail(s, TEUK_EINVAL, "kernel 1 needs coef_mode 0");
     s->variant = (int)value;
   } else {
     return fail(s, TEUK_EINVAL, "teuk_set_option: unknown key");

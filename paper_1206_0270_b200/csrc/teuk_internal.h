@@ -55,7 +55,8 @@ struct StepParams {
   double* uout;
   const double* rtab;
   const double* ttab;
-  const double* coef2d;   // coef_mode 1: [n_modes][2 n_r - 1][8][n_theta] (b,kre,kim,are,aim,gre,gim,cL)
+  const double* coef2d;   // coef_mode 1: [n_modes][2 n_r - 1][8][n_theta] streamed coefficient planes
+  int coef_mode;
   int n_r, n_theta, n_modes;
   int slab_rows, n_slabs;
   int variant;            // 0 = register-resident kernel, 1 = shared-memory-resident kernel

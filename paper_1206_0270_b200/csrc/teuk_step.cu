@@ -60,6 +60,30 @@ struct ThetaTab {
   __device__ __forceinline__ void get(ThetaVals<V>& t) const { t = vals; }
 };
 
+// theta tables read from a block-shared copy [TT_N][n_theta_pad] under lane mapping MAP 1: the two-column
+// piece of lane l starts at column q*64 + 2l, so a warp-wide 16-byte load is bank-conflict free.
+template <int V>
+struct ThetaTabShared {
+  const double* base;   // shared memory, row stride `stride` doubles, zero padded to 32*V columns
+  int stride, lane;
+  __device__ __forceinline__ void get(ThetaVals<V>& t) const {
+    double* dst[TT_N] = {t.s2, t.cs, t.ap, t.am, t.d0};
+#pragma unroll
+    for (int k = 0; k < TT_N; ++k) {
+      if (V == 1) {
+        dst[k][0] = base[k * stride + lane];
+      } else {
+#pragma unroll
+        for (int q = 0; q < V / 2; ++q) {
+          const double2 w = *reinterpret_cast<const double2*>(base + k * stride + q * 64 + 2 * lane);
+          dst[k][2 * q] = w.x;
+          dst[k][2 * q + 1] = w.y;
+        }
+      }
+    }
+  }
+};
+
 // 1/sqrt(x) for x in (0.9, 1]: MUFU.RSQ64H seed (rel. error < 2^-20) + one third-order step
 // y <- y + y e (1/2 + 3/8 e), e = 1 - x y^2  (error ~ e^3): no range checks, no branch.
 __device__ __forceinline__ double rsqrt_near_one(double x);
@@ -184,9 +208,9 @@ __device__ __forceinline__ void theta_neighbours(const double (&f)[V], double (&
 // ---- one Lax-Wendroff stage at one radial location ------------------------------------------
 // HALF: A = u^n_i, B = u^n_{i+1}, out = 2 u^{n+1/2}_{i+1/2}             (Eq. 3, tau = dt/2)
 // else: A = H_{i-1/2}, B = H_{i+1/2} (doubled), out = u^{n+1}_i, base = u^n_i   (Eq. 4, tau = dt/4)
-template <int V, bool HALF, int MAP = 0>
+template <int V, bool HALF, int MAP = 0, class TT = ThetaTab<V>>
 __device__ __forceinline__ void lw_stage(const Row<V>& A, const Row<V>& B, const Row<V>& base,
-                                         const double* __restrict__ rec, const ThetaTab<V>& tht,
+                                         const double* __restrict__ rec, const TT& tht,
                                          double tau, double two_over_dx, Row<V>& out, int lane = 0) {
   ThetaVals<V> th;
   tht.get(th);
@@ -248,6 +272,81 @@ __device__ __forceinline__ void lw_stage(const Row<V>& A, const Row<V>& B, const
       out.c[3][v0 + g] = fma(tau, bi[g], HALF ? spi[g] : base.c[3][v0 + g]);
     }
 #undef FORG
+  }
+}
+
+// ---- coef_mode 1: the same stage with the eight 2D coefficient planes STREAMED from HBM ----------
+// (comparison arm for the bytes-vs-flops choice: +128 B per point per iteration, -26 FP64 instructions).
+// `loc` points at this location's [8][n_theta] planes (see teuk_coef2d_kernel); textbook form
+// R = b dPi + kappa dPhi + alpha Pi + gamma Phi + cL L_theta Phi in the scaled variables S, D.
+template <int V, bool HALF, bool VEC>
+__device__ __forceinline__ void lw_stage_planes(const Row<V>& A, const Row<V>& B, const Row<V>& base,
+                                                const double* __restrict__ loc, const ThetaTab<V>& tht, double tau,
+                                                Row<V>& out, int nth, int j0) {
+  ThetaVals<V> th;
+  tht.get(th);
+  double cf[8][V];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    const double* q = loc + (size_t)k * nth + j0;
+    if (VEC && j0 < nth) {
+      if (V == 1) {
+        cf[k][0] = __ldcs(q);
+      } else if (V % 4 == 0) {
+#pragma unroll
+        for (int v = 0; v < V; v += 4) ld256(q + v, cf[k][v], cf[k][v + 1], cf[k][v + 2], cf[k][v + 3]);
+      } else {
+#pragma unroll
+        for (int v = 0; v < V; v += 2) {
+          const double2 t = __ldcs(reinterpret_cast<const double2*>(q + v));
+          cf[k][v] = t.x;
+          cf[k][v + 1] = t.y;
+        }
+      }
+    } else {
+#pragma unroll
+      for (int v = 0; v < V; ++v) cf[k][v] = (j0 + v < nth) ? __ldcs(q + v) : 0.0;
+    }
+  }
+  double sfr[V], sfi[V];
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    sfr[v] = A.c[0][v] + B.c[0][v];
+    sfi[v] = A.c[1][v] + B.c[1][v];
+  }
+  double nlr[V], nrr[V], nli[V], nri[V];
+  theta_neighbours<V, 0>(sfr, nlr, nrr, 0);
+  theta_neighbours<V, 0>(sfi, nli, nri, 0);
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    const double dfr = B.c[0][v] - A.c[0][v], dfi = B.c[1][v] - A.c[1][v];
+    const double spr = A.c[2][v] + B.c[2][v], spi = A.c[3][v] + B.c[3][v];
+    const double dpr = B.c[2][v] - A.c[2][v], dpi = B.c[3][v] - A.c[3][v];
+    const double b2d = cf[0][v], kre = cf[1][v], kim = cf[2][v], are = cf[3][v], aim = cf[4][v];
+    const double gre = cf[5][v], gim = cf[6][v], cl = cf[7][v];
+    const double e2r = fma(-b2d, dfr, spr), e2i = fma(-b2d, dfi, spi);
+    out.c[0][v] = fma(tau, e2r, HALF ? sfr[v] : base.c[0][v]);
+    out.c[1][v] = fma(tau, e2i, HALF ? sfi[v] : base.c[1][v]);
+    const double ltr = fma(th.ap[v], nrr[v], fma(th.am[v], nlr[v], th.d0[v] * sfr[v]));
+    const double lti = fma(th.ap[v], nri[v], fma(th.am[v], nli[v], th.d0[v] * sfi[v]));
+    double br = kre * dfr;
+    br = fma(-kim, dfi, br);
+    br = fma(are, spr, br);
+    br = fma(-aim, spi, br);
+    br = fma(cl, ltr, br);
+    br = fma(gre, sfr[v], br);
+    br = fma(-gim, sfi[v], br);
+    br = fma(b2d, dpr, br);
+    double bi = kre * dfi;
+    bi = fma(kim, dfr, bi);
+    bi = fma(are, spi, bi);
+    bi = fma(aim, spr, bi);
+    bi = fma(cl, lti, bi);
+    bi = fma(gre, sfi[v], bi);
+    bi = fma(gim, sfr[v], bi);
+    bi = fma(b2d, dpi, bi);
+    out.c[2][v] = fma(tau, br, HALF ? spr : base.c[2][v]);
+    out.c[3][v] = fma(tau, bi, HALF ? spi : base.c[3][v]);
   }
 }
 
@@ -408,7 +507,7 @@ __device__ __forceinline__ void stage_rtab_chunk(double* sbuf, const double* __r
   asm volatile("cp.async.commit_group;" ::: "memory");
 }
 
-template <int V, bool VEC>
+template <int V, bool VEC, int CM>
 __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const __grid_constant__ StepParams p) {
   const int lane = threadIdx.x & 31;
   const int slab = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -470,7 +569,13 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
   load_row<V, VEC>(ub, uin + (size_t)r0 * row_stride, nth, j0);
   load_row<V, VEC>(uc, uin + (size_t)(r0 + 1) * row_stride, nth, j0);
   if (do_tap && r0 == 1) tap<V>(ua, ub, p, 0, mode, n, lane);
-  lw_stage<V, true>(ua, ub, ua, rtab + (size_t)(2 * (r0 - 1) + 1) * RT_N, th, tau_h, tdx, hp);
+  const double* __restrict__ planes = nullptr;   // coef_mode 1: [2 nr - 1][8][nth] of this mode
+  if (CM == 1) planes = p.coef2d + (size_t)mode * (2 * nr - 1) * 8 * nth;
+  const size_t loc_stride = (size_t)8 * nth;
+  if (CM == 1)
+    lw_stage_planes<V, true, VEC>(ua, ub, ua, planes + (size_t)(2 * (r0 - 1) + 1) * loc_stride, th, tau_h, hp, nth, j0);
+  else
+    lw_stage<V, true>(ua, ub, ua, rtab + (size_t)(2 * (r0 - 1) + 1) * RT_N, th, tau_h, tdx, hp);
   add_source<V>(hp, src_h, p, r0 - 1, true);
 
   const double* rt_cur = rt_buf;
@@ -491,7 +596,17 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
         stage_rtab_chunk(rt_buf + ((c + 1) & 1) * RT_CHUNK_DOUBLES, rtab, 2 * (i + RT_CH), 2 * nr - 1, lane);
     }
     if (do_tap) tap<V>(A, B, p, i, mode, n, lane);
-    lw_stage<V, true>(A, B, A, rt_cur + (2 * o + 1) * RT_N, th, tau_h, tdx, Hn);
+    if (CM == 1) {
+      // pull the next iteration's two coefficient rows (2 x 8 planes) towards L2 while this one computes
+      if (i + 1 < r1) {
+        const char* nxt = reinterpret_cast<const char*>(planes + (size_t)(2 * (i + 1)) * loc_stride);
+        for (unsigned off = lane * 128u; off < 2u * (unsigned)loc_stride * 8u; off += 32u * 128u)
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(nxt + off));
+      }
+      lw_stage_planes<V, true, VEC>(A, B, A, planes + (size_t)(2 * i + 1) * loc_stride, th, tau_h, Hn, nth, j0);
+    } else {
+      lw_stage<V, true>(A, B, A, rt_cur + (2 * o + 1) * RT_N, th, tau_h, tdx, Hn);
+    }
     add_source<V>(Hn, src_h, p, i, true);
     if (VEC) {
       // B (row i+1, read from slot (i+1)&1 at the end of the last iteration) has been consumed by
@@ -501,7 +616,10 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
         tma_load_row(slot0 + (size_t)((i + 3) & 1) * row_stride, uin + (size_t)(i + 3) * row_stride, row_bytes,
                      &bars[(i + 3) & 1]);
     }
-    lw_stage<V, false>(Hp, Hn, A, rt_cur + (2 * o) * RT_N, th, tau_f, tdx, out);
+    if (CM == 1)
+      lw_stage_planes<V, false, VEC>(Hp, Hn, A, planes + (size_t)(2 * i) * loc_stride, th, tau_f, out, nth, j0);
+    else
+      lw_stage<V, false>(Hp, Hn, A, rt_cur + (2 * o) * RT_N, th, tau_f, tdx, out);
     add_source<V>(out, src_f, p, i, false);
     store_row<V, VEC>(out, uout + (size_t)i * row_stride, nth, j0);
     if (VEC) {
@@ -651,14 +769,25 @@ __device__ __forceinline__ void hslot_load(Row<V>& h, const double* slot, int la
 #ifndef TEUK_SMEM_MIN_BLOCKS
 #define TEUK_SMEM_MIN_BLOCKS 3
 #endif
+#ifndef TEUK_SMEM_TT
+#define TEUK_SMEM_TT 0   // 1: theta tables of the shared-memory-resident kernel in shared memory too (no gain measured)
+#endif
 
 template <int V, bool EVEN>
 __global__ void __launch_bounds__(128, TEUK_SMEM_MIN_BLOCKS) teuk_step_smem_kernel(const __grid_constant__ StepParams p) {
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const int slab = blockIdx.x * (blockDim.x >> 5) + wib;
   const int mode = blockIdx.y;
-  if (slab >= p.n_slabs) return;
   const int nth = p.n_theta, nr = p.n_r;
+#if TEUK_SMEM_TT
+  __shared__ __align__(16) double s_tt[TT_N * 32 * V];
+  for (int t = threadIdx.x; t < TT_N * 32 * V; t += blockDim.x) {
+    const int k = t / (32 * V), j = t - k * 32 * V;
+    s_tt[t] = (j < nth) ? p.ttab[((size_t)mode * TT_N + k) * nth + j] : 0.0;
+  }
+  __syncthreads();
+#endif
+  if (slab >= p.n_slabs) return;
   const int r0 = 1 + slab * p.slab_rows;
   const int r1 = min(r0 + p.slab_rows, nr - 1);
   const size_t row_stride = (size_t)4 * nth;
@@ -692,6 +821,13 @@ __global__ void __launch_bounds__(128, TEUK_SMEM_MIN_BLOCKS) teuk_step_smem_kern
   __syncwarp();
   stage_rtab_chunk(rt_buf, rtab, 2 * r0, 2 * nr - 1, lane);
 
+#if TEUK_SMEM_TT
+  ThetaTabShared<V> th;
+  th.base = s_tt;
+  th.stride = 32 * V;
+  th.lane = lane;
+  typedef ThetaTabShared<V> TTab;
+#else
   ThetaTab<V> th;
   {
     const double* tb = p.ttab + (size_t)mode * TT_N * nth;
@@ -706,6 +842,8 @@ __global__ void __launch_bounds__(128, TEUK_SMEM_MIN_BLOCKS) teuk_step_smem_kern
       th.vals.d0[v] = ok ? tb[TT_D0 * nth + j] : 0.0;
     }
   }
+  typedef ThetaTab<V> TTab;
+#endif
   StageSource<V> src_h, src_f;
   setup_source<V, 1>(src_h, p, mode, 2 * n, true, r0 - 1, r1 - 1, lane);
   setup_source<V, 1>(src_f, p, mode, 2 * n + 1, false, r0, r1 - 1, lane);
@@ -720,7 +858,7 @@ __global__ void __launch_bounds__(128, TEUK_SMEM_MIN_BLOCKS) teuk_step_smem_kern
     piece_load<V, EVEN>(A, slot_of(r0 - 1), nth, lane);
     piece_load<V, EVEN>(B, slot_of(r0), nth, lane);
     if (do_tap && r0 == 1) tap<V, 1>(A, B, p, 0, mode, n, lane);
-    lw_stage<V, true, 1>(A, B, A, rtab + (size_t)(2 * (r0 - 1) + 1) * RT_N, th, tau_h, tdx, H, lane);
+    lw_stage<V, true, 1, TTab>(A, B, A, rtab + (size_t)(2 * (r0 - 1) + 1) * RT_N, th, tau_h, tdx, H, lane);
     add_source<V>(H, src_h, p, r0 - 1, true);
     hslot_store<V>(H, hslot, lane);
     A = B;
@@ -748,13 +886,13 @@ __global__ void __launch_bounds__(128, TEUK_SMEM_MIN_BLOCKS) teuk_step_smem_kern
       Row<V> B;
       piece_load<V, EVEN>(B, slot_of(i + 1), nth, lane);
       if (do_tap) tap<V, 1>(A, B, p, i, mode, n, lane);
-      lw_stage<V, true, 1>(A, B, A, rt_cur + (2 * o + 1) * RT_N, th, tau_h, tdx, Hn, lane);
+      lw_stage<V, true, 1, TTab>(A, B, A, rt_cur + (2 * o + 1) * RT_N, th, tau_h, tdx, Hn, lane);
       add_source<V>(Hn, src_h, p, i, true);
     }
     {
       Row<V> Hp;
       hslot_load<V>(Hp, hslot, lane);
-      lw_stage<V, false, 1>(Hp, Hn, A, rt_cur + (2 * o) * RT_N, th, tau_f, tdx, out, lane);
+      lw_stage<V, false, 1, TTab>(Hp, Hn, A, rt_cur + (2 * o) * RT_N, th, tau_f, tdx, out, lane);
       add_source<V>(out, src_f, p, i, false);
     }
     piece_store_global<V, EVEN>(out, uout + (size_t)i * row_stride, nth, lane);
@@ -862,19 +1000,26 @@ template <int V>
 static cudaError_t launch_v(const StepParams& p, cudaStream_t st) {
   const int warps_per_block = 4;
   dim3 grid((p.n_slabs + warps_per_block - 1) / warps_per_block, p.n_modes), block(32 * warps_per_block);
-  if (p.n_theta % V == 0) {
-    const size_t dyn = (size_t)warps_per_block * 2 * 4 * p.n_theta * sizeof(double);
-    static bool attr_set = false;   // per instantiation
-    if (!attr_set) {
-      cudaError_t e = cudaFuncSetAttribute(teuk_step_kernel<V, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           (int)((size_t)warps_per_block * 2 * 4 * 32 * V * sizeof(double)));
-      if (e != cudaSuccess) return e;
-      attr_set = true;
-    }
-    teuk_step_kernel<V, true><<<grid, block, dyn, st>>>(p);
+  const bool vec = p.n_theta % V == 0;
+  const size_t dyn = vec ? (size_t)warps_per_block * 2 * 4 * p.n_theta * sizeof(double) : 0;
+  const int dyn_max = (int)((size_t)warps_per_block * 2 * 4 * 32 * V * sizeof(double));
+#define TEUK_LAUNCH(VECF, CMF)                                                                               \
+  do {                                                                                                       \
+    static bool attr_set = false;                                                                            \
+    if (!attr_set) {                                                                                         \
+      cudaError_t e = cudaFuncSetAttribute(teuk_step_kernel<V, VECF, CMF>,                                   \
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max);            \
+      if (e != cudaSuccess) return e;                                                                        \
+      attr_set = true;                                                                                       \
+    }                                                                                                        \
+    teuk_step_kernel<V, VECF, CMF><<<grid, block, dyn, st>>>(p);                                             \
+  } while (0)
+  if (p.coef_mode == 1) {
+    if (vec) TEUK_LAUNCH(true, 1); else TEUK_LAUNCH(false, 1);
   } else {
-    teuk_step_kernel<V, false><<<grid, block, 0, st>>>(p);
+    if (vec) TEUK_LAUNCH(true, 0); else TEUK_LAUNCH(false, 0);
   }
+#undef TEUK_LAUNCH
   return cudaGetLastError();
 }
 

@@ -129,9 +129,11 @@ __global__ void teuk_ttab_kernel(double* __restrict__ ttab, const int* __restric
   base[TT_D0 * n_theta + j] = d0;
 }
 
-// coef_mode 1: the eight full 2D coefficient values per location ("matrices D and S"
-// stored per grid point), assembled from the same 1D tables: b, Re/Im kappa, Re/Im alpha,
-// Re/Im gamma, cL.  Layout [mode][p][8][n_theta].
+// coef_mode 1: eight full 2D coefficient planes per location, i.e. the paper's stored "matrices D and S"
+// (PAPER.md:102), assembled once from the 1D tables and then STREAMED by the step kernel instead of being
+// rebuilt.  Layout [mode][p][8][n_theta]; planes (prescaled so the kernel needs no assembly at all):
+//   0: (2/dx) b   1,2: (2/dx) Re/Im kappa   3,4: Re/Im alpha   5: -cL Gr (r-part of Re gamma; the theta
+//   part rides on the D0 table together with the pole ghosts)   6: Im gamma   7: cL.
 __global__ void teuk_coef2d_kernel(double* __restrict__ c2d, const double* __restrict__ rtab,
                                    const double* __restrict__ ttab, int n_modes, int n_r, int n_theta,
                                    double dx) {
@@ -145,23 +147,27 @@ __global__ void teuk_coef2d_kernel(double* __restrict__ c2d, const double* __res
   const double* rec = rtab + qp * RT_N;
   const double* tb = ttab + (size_t)q * TT_N * n_theta;
   const double s2 = tb[TT_S2 * n_theta + j], cs = tb[TT_COS * n_theta + j];
-  const double Q = 1.0 / (1.0 - rec[RT_EPS] * s2);
-  const double b = sqrt(Q);
-  const double hdx = 0.5 * dx;
+  const double b = rsqrt(1.0 - rec[RT_EPS] * s2);
+  const double Q = b * b;
+  const double b2d = b * (2.0 / dx);
   const double are = Q * rec[RT_A0], aim = Q * (rec[RT_A1] + rec[RT_A2] * cs);
-  const double bre = Q * rec[RT_BRE] * hdx, bim = Q * rec[RT_BIM] * hdx;
-  const double bbx = Q * Q * s2 * rec[RT_X32] * hdx;
-  // Gtheta is recovered from the un-folded diagonal: D0 = -2/dth^2 - Gtheta (+ ghost term), so the
-  // 2D planes keep gamma itself and the step kernel applies the ghosts through A+-, D0 as usual.
   double* out = c2d + (qp * 8) * n_theta + j;
-  out[0 * (size_t)n_theta] = b;
-  out[1 * (size_t)n_theta] = bre - are * b - bbx;   // Re kappa = Re beta - Re alpha b - b b_x
-  out[2 * (size_t)n_theta] = bim - aim * b;         // Im kappa
-  out[3 * (size_t)n_theta] = are;
-  out[4 * (size_t)n_theta] = aim;
-  out[5 * (size_t)n_theta] = -Q * rec[RT_CL] * rec[RT_GR];  // r-part of Re gamma (theta part rides on D0)
-  out[6 * (size_t)n_theta] = Q * rec[RT_G1];
-  out[7 * (size_t)n_theta] = Q * rec[RT_CL];
+  const size_t st = (size_t)n_theta;
+  out[0 * st] = b2d;
+  out[1 * st] = Q * rec[RT_BRE] - are * b2d - Q * Q * s2 * rec[RT_X32];  // (2/dx)(Re beta - Re alpha b - b b_x)
+  out[2 * st] = Q * rec[RT_BIM] - aim * b2d;                             // (2/dx)(Im beta - Im alpha b)
+  out[3 * st] = are;
+  out[4 * st] = aim;
+  out[5 * st] = -Q * rec[RT_CL] * rec[RT_GR];
+  out[6 * st] = Q * rec[RT_G1];
+  out[7 * st] = Q * rec[RT_CL];
+}
+
+cudaError_t teuk_launch_coef2d(double* c2d, const double* rtab, const double* ttab, int n_modes, int n_r,
+                               int n_theta, double dx, cudaStream_t st) {
+  const size_t total = (size_t)n_modes * (2 * (size_t)n_r - 1) * n_theta;
+  teuk_coef2d_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(c2d, rtab, ttab, n_modes, n_r, n_theta, dx);
+  return cudaGetLastError();
 }
 
 // ---- host-side launcher (called from teuk_api.cu) --------------------------------------------

@@ -273,3 +273,19 @@ def test_smem_kernel_parity(orc, teuk, cfg):
     for slab in (1, 5):
         res = run_pair(orc, teuk, cfg, 4, initial=wl.random_state(cfg, 31), options={"kernel": 1, "slab_rows": slab})
         check_pair(res, tol=1e-12)
+
+
+@pytest.mark.parametrize("cfg", SMALL, ids=[c.name for c in SMALL])
+def test_streamed_coefficient_planes_parity(orc, teuk, cfg):
+    """coef_mode 1 (the stored-matrices arm of the bytes-vs-flops comparison) against the oracle."""
+    res = run_pair(orc, teuk, cfg, min(cfg.steps, 200), options={"coef_mode": 1})
+    check_pair(res)
+    res = run_pair(orc, teuk, cfg, 3, initial=wl.random_state(cfg, 41), options={"coef_mode": 1, "slab_rows": 7})
+    check_pair(res, tol=1e-12)
+
+
+@pytest.mark.parametrize("n_theta", [20, 45, 64, 100, 128, 256])
+def test_streamed_coefficient_planes_theta_sizes(orc, teuk, n_theta):
+    cfg = SMALL[3].scaled(name="cm%d" % n_theta, n_r=150, n_theta=n_theta, dt_over_dx=0.02, steps=8, modes=(2, 1))
+    res = run_pair(orc, teuk, cfg, 8, initial=wl.random_state(cfg, n_theta), options={"coef_mode": 1})
+    check_pair(res, tol=1e-11)
