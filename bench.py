@@ -263,6 +263,7 @@ def main():
         barrier()
         ms = e0.elapsed_time(e1)
         launches = g.stat("launches") - l0
+        slab_rows = g.stat("slab_rows")
         clocks = sampler.stop() if rank == 0 else None
         ms = max_over_ranks(ms, "cuda", world)
         value = world * cfg.n_pts * K / (ms * 1e-3) / 1e9
@@ -304,7 +305,7 @@ def main():
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfg.name, "grid": [cfg.n_r, cfg.n_theta], "modes": list(cfg.modes), "a": cfg.a,
-                       "dt": cfg.dt, "source": cfg.source, "coef_mode": args.coef_mode, "observers": list(cfg.observers),
+                       "dt": cfg.dt, "source": cfg.source, "coef_mode": args.coef_mode, "slab_rows": int(slab_rows), "observers": list(cfg.observers),
                        "state_mb": 4 * cfg.n_pts * 8 / 1e6, "parallelism": "replicas x%d" % world,
                        "l2": "inputs larger than L2 (two 537 MB state copies stream through a 126 MB L2)"
                        if 4 * cfg.n_pts * 8 > 2.5e8 else "state fits in L2: not an HBM measurement"},

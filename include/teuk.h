@@ -83,7 +83,8 @@ int teuk_set_initial(teuk_solver *s, const double *phi_re, const double *phi_im,
 /* Install (copy to the device) the trajectory table; NULL = source-free.  Host pointers. */
 int teuk_set_source(teuk_solver *s, const teuk_orbit *orbit);
 
-/* Enqueue n >= 0 iterations.  No host synchronisation, no full-grid host transfer; observers are
+/* Enqueue n >= 0 iterations.  No host synchronisation (except the one-time slab-length measurement of
+ * the first call, see "autotune"), no full-grid host transfer; observers are
  * tapped on the device after every iteration (sample time t = n_done*dt).  TEUK_EINVAL if a
  * source is installed and its table is too short. */
 int teuk_step(teuk_solver *s, int64_t n);
@@ -109,14 +110,16 @@ int teuk_get_state(teuk_solver *s, double *phi_re, double *phi_im, double *pi_re
  *   "stream"        a cudaStream_t cast to int64 (0 = back to the solver's own stream)
  *   "coef_mode"     0 = coefficients recomputed on the fly from 1D tables (default),
  *                   1 = coefficients streamed from precomputed 2D FP64 planes
- *   "slab_rows"     rows of r* marched by one warp (0 = automatic)
+ *   "slab_rows"     rows of r* marched by one warp (0 = automatic: measured once at the first teuk_step,
+ *                   which then waits for a few untimed-by-the-caller trial launches into scratch memory)
+ *   "autotune"      1 = measure the slab length (default), 0 = use the two-wave heuristic
  *   "graph"         1 = replay the iteration through a CUDA graph (default), 0 = plain launches
  *   "kernel"        0 = register-resident marching kernel, 1 = shared-memory-resident marching kernel
  *                   (same arithmetic, bitwise identical fields; they differ in on-chip residency) */
 int teuk_set_option(teuk_solver *s, const char *key, int64_t value);
 
 /* Read-only counters: "steps" (iterations done), "launches" (kernels launched so far),
- * "n_pts" (n_modes*n_r*n_theta), "state_bytes" (one copy of the fields). */
+ * "n_pts" (n_modes*n_r*n_theta), "state_bytes" (one copy of the fields), "slab_rows" (in use). */
 int teuk_get_stat(const teuk_solver *s, const char *key, int64_t *value);
 
 /* Wait for all work enqueued on the solver's stream. */

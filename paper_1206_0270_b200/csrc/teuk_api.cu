@@ -57,7 +57,8 @@ struct teuk_solver {
   int n_r, n_theta, n_modes;
   int m[TEUK_MAX_MODES];
   // options
-  int outer_bc, coef_mode, slab_rows_opt, use_graph, variant;
+  int outer_bc, coef_mode, slab_rows_opt, use_graph, variant, autotune;
+  int tuned_rows;        // slab length chosen by the one-time autotune (0 = not tuned yet)
   // device
   int device, n_sms;
   cudaStream_t own_stream, stream, copy_stream;
@@ -123,20 +124,24 @@ void drop_graph(teuk_solver* s) {
     }
 }
 
-// Automatic slab length: enough warps for >= 2 waves of the resident capacity, slabs >= 16 rows.
-int auto_slab_rows(const teuk_solver* s) {
-  const int interior = s->n_r - 2;
+// Heuristic slab length (rows of r* marched by one warp): two waves of the warps that fit on the chip.
+// It seeds the autotune below and is used as is when autotuning is switched off.
+int resident_warps(const teuk_solver* s) {
   const int sms = s->n_sms > 0 ? s->n_sms : 148;
   const int v = (s->n_theta + 31) / 32;
-  const int warps_per_sm = s->variant == 1 ? 12 : (v <= 1 ? 16 : 8);
-  const long long target_warps = (long long)sms * warps_per_sm * 2;
-  long long per_mode = target_warps / s->n_modes;
-  if (per_mode < 1) per_mode = 1;
-  int rows = (int)((interior + per_mode - 1) / per_mode);
-  if (rows < 16) rows = 16;
-  if (rows > interior) rows = interior;
-  return rows;
+  return sms * (s->variant == 1 ? 12 : (v <= 1 ? 16 : 8));
 }
+
+int rows_for_waves(const teuk_solver* s, double waves) {
+  const long long interior = s->n_r - 2;
+  const double target = waves * resident_warps(s);
+  long long rows = (long long)((interior * s->n_modes + target - 1) / target);
+  if (rows < 1) rows = 1;
+  if (rows > interior) rows = interior;
+  return (int)rows;
+}
+
+int auto_slab_rows(const teuk_solver* s) { return rows_for_waves(s, 2.0); }
 
 void fill_params(const teuk_solver* s, StepParams* p, int in_buf, int k, int tap_enable) {
   memset(p, 0, sizeof(*p));
@@ -149,7 +154,7 @@ void fill_params(const teuk_solver* s, StepParams* p, int in_buf, int k, int tap
   p->n_r = s->n_r;
   p->n_theta = s->n_theta;
   p->n_modes = s->n_modes;
-  p->slab_rows = s->slab_rows_opt > 0 ? s->slab_rows_opt : auto_slab_rows(s);
+  p->slab_rows = s->slab_rows_opt > 0 ? s->slab_rows_opt : (s->tuned_rows > 0 ? s->tuned_rows : auto_slab_rows(s));
   if (p->slab_rows > s->n_r - 2) p->slab_rows = s->n_r - 2;
   p->n_slabs = (s->n_r - 2 + p->slab_rows - 1) / p->slab_rows;
   p->outer_bc = s->outer_bc;
@@ -303,7 +308,7 @@ int teuk_create(teuk_solver** out, double a, double M, const int32_t* m, int32_t
   s->dx = (grid->rs_max - grid->rs_min) / (grid->n_r - 1);
   s->dth = kPi / grid->n_theta;
   for (int q = 0; q < n_modes; ++q) s->m[q] = m[q];
-  s->outer_bc = 0; s->coef_mode = 0; s->slab_rows_opt = 0; s->use_graph = 1;
+  s->outer_bc = 0; s->coef_mode = 0; s->slab_rows_opt = 0; s->use_graph = 1; s->autotune = 1; s->tuned_rows = 0;
   s->device = dev;
   if (cudaDeviceGetAttribute(&s->n_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) s->n_sms = 148;
   snprintf(s->err, sizeof(s->err), "no error");
@@ -444,6 +449,64 @@ int build_graph(teuk_solver* s) {
   return TEUK_OK;
 }
 
+// One-time measurement of the slab length: the march of a slab is serial, so the
+// best length depends on grid size, mode count and wave quantisation.  Candidates are timed with the real
+// kernel reading the current level and writing the idle ping-pong buffer (tap off): the state, the
+// iteration counter and the recorded series are untouched, and results do not depend on the slab length.
+int tune_slab_rows(teuk_solver* s) {
+  const double waves[] = {0.95, 1.9, 2.0, 2.9, 3.9, 5.8};
+  int cand[16];
+  int nc = 0;
+  auto add = [&](int r) {
+    if (r < 1) r = 1;
+    if (r > s->n_r - 2) r = s->n_r - 2;
+    for (int q = 0; q < nc; ++q)
+      if (cand[q] == r) return;
+    if (nc < 16) cand[nc++] = r;
+  };
+  for (double w : waves) add(rows_for_waves(s, w));
+  const int base = auto_slab_rows(s);
+  if (base <= 16) { add(1); add(2); add(4); add(8); add(16); }
+  cudaEvent_t e0, e1;
+  CK(cudaEventCreate(&e0), "autotune: event");
+  CK(cudaEventCreate(&e1), "autotune: event");
+  float best = 1e30f;
+  int best_rows = base;
+  const int saved = s->slab_rows_opt;
+  for (int q = 0; q < nc; ++q) {
+    s->slab_rows_opt = cand[q];
+    StepParams p;
+    fill_params(s, &p, s->cur, (int)(s->step - s->base_on_device), 0);
+    cudaError_t e = teuk_launch_step(p, s->stream);               // warm-up
+    float ms = 0.f;
+    int reps = 3;
+    for (int pass = 0; pass < 2 && e == cudaSuccess; ++pass) {   // short kernels: second pass with 40 launches
+      e = cudaEventRecord(e0, s->stream);
+      for (int r = 0; r < reps && e == cudaSuccess; ++r) e = teuk_launch_step(p, s->stream);
+      if (e == cudaSuccess) e = cudaEventRecord(e1, s->stream);
+      if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+      if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+      s->launches += reps;
+      ms /= reps;
+      if (ms * reps > 0.3f) break;
+      reps = 40;
+    }
+    s->launches += 1;
+    if (e != cudaSuccess) {
+      s->slab_rows_opt = saved;
+      cudaEventDestroy(e0);
+      cudaEventDestroy(e1);
+      return cuda_fail(s, e, "autotune");
+    }
+    if (ms < best) { best = ms; best_rows = cand[q]; }
+  }
+  s->slab_rows_opt = saved;
+  s->tuned_rows = best_rows;
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  return TEUK_OK;
+}
+
 // Run c >= 1 iterations whose samples fit in the ring.
 int run_chunk(teuk_solver* s, long long c) {
   long long left = c;
@@ -502,6 +565,11 @@ int teuk_step(teuk_solver* s, int64_t n) {
   if (n < 0) return fail(s, TEUK_EINVAL, "teuk_step: n < 0");
   if (s->has_source && 2 * (s->step + n) > s->n_samples)
     return fail(s, TEUK_EINVAL, "teuk_step: trajectory table too short for n more iterations");
+  if (n > 0 && s->autotune && s->slab_rows_opt == 0 && s->tuned_rows == 0 && (s->base_on_device <= s->step)) {
+    const int rc = tune_slab_rows(s);
+    if (rc != TEUK_OK) return rc;
+    drop_graph(s);
+  }
   long long remaining = n;
   while (remaining > 0) {
     long long room = remaining;
@@ -634,6 +702,8 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
     s->slab_rows_opt = (int)value;
   } else if (!strcmp(key, "graph")) {
     s->use_graph = value ? 1 : 0;
+  } else if (!strcmp(key, "autotune")) {
+    s->autotune = value ? 1 : 0;
   } else if (!strcmp(key, "kernel")) {
     if (value != 0 && value != 1) return fail(s, TEUK_EINVAL, "kernel must be 0 (register-resident) or 1 (shared-memory-resident)");
     if (value == 1 && s->coef_mode != 0) return fail(s, TEUK_EINVAL, "kernel 1 needs coef_mode 0");
@@ -641,6 +711,7 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
   } else {
     return fail(s, TEUK_EINVAL, "teuk_set_option: unknown key");
   }
+  if (strcmp(key, "stream") != 0) s->tuned_rows = 0;   // launch shape may change: measure again
   drop_graph(s);
   return TEUK_OK;
 }
@@ -651,6 +722,7 @@ int teuk_get_stat(const teuk_solver* s, const char* key, int64_t* value) {
   else if (!strcmp(key, "launches")) *value = s->launches;
   else if (!strcmp(key, "n_pts")) *value = (int64_t)s->n_modes * s->n_r * s->n_theta;
   else if (!strcmp(key, "state_bytes")) *value = (int64_t)(state_doubles(s) * sizeof(double));
+  else if (!strcmp(key, "slab_rows")) *value = s->slab_rows_opt > 0 ? s->slab_rows_opt : (s->tuned_rows > 0 ? s->tuned_rows : auto_slab_rows(s));
   else return TEUK_EINVAL;
   return TEUK_OK;
 }

@@ -289,3 +289,22 @@ def test_streamed_coefficient_planes_theta_sizes(orc, teuk, n_theta):
     cfg = SMALL[3].scaled(name="cm%d" % n_theta, n_r=150, n_theta=n_theta, dt_over_dx=0.02, steps=8, modes=(2, 1))
     res = run_pair(orc, teuk, cfg, 8, initial=wl.random_state(cfg, n_theta), options={"coef_mode": 1})
     check_pair(res, tol=1e-11)
+
+
+def test_autotune_does_not_change_results(orc, teuk):
+    """The one-time slab-length measurement runs trial launches into scratch memory only."""
+    cfg = SMALL[3]
+    out = []
+    for auto in (1, 0):
+        g = teuk.Solver.from_config(cfg)
+        g.set_option("autotune", auto)
+        g.set_initial(*wl.random_state(cfg, 17))
+        g.set_source(wl.orbit_table(cfg, n_steps=60))
+        g.add_observer(30.0, wl.observer_weights(cfg))
+        g.step(60)
+        assert g.stat("steps") == 60 and g.stat("slab_rows") >= 1
+        out.append((g.get_state(), g.extract(30.0)))
+        g.close()
+    for a, b in zip(out[0][0], out[1][0]):
+        assert np.array_equal(a, b)
+    assert np.array_equal(out[0][1][1], out[1][1][1]) and len(out[0][1][0]) == 60
