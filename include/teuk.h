@@ -50,7 +50,7 @@ typedef struct teuk_solver teuk_solver; /* opaque; created and destroyed by the 
 
 typedef struct {
   double rs_min, rs_max; /* tortoise-coordinate range, rs_max > rs_min                            */
-  int32_t n_r, n_theta;  /* n_r >= 4; 4 <= n_theta <= 256                                          */
+  int32_t n_r, n_theta;  /* n_r >= 4; 4 <= n_theta <= 4096                                         */
 } teuk_grid;
 
 /* Sampled particle trajectory and source amplitude (C.6 of DESIGN.md).
@@ -109,13 +109,14 @@ int teuk_get_state(teuk_solver *s, double *phi_re, double *phi_im, double *pi_re
  *   "outer_bc"      0 = outgoing (Pi = 0, Phi upwind; default), 1 = Dirichlet as PAPER.md:104
  *   "stream"        a cudaStream_t cast to int64 (0 = back to the solver's own stream)
  *   "coef_mode"     0 = coefficients recomputed on the fly from 1D tables (default),
- *                   1 = coefficients streamed from precomputed 2D FP64 planes
+ *                   1 = coefficients streamed from precomputed 2D FP64 planes (n_theta <= 128 only)
  *   "slab_rows"     rows of r* marched by one warp (0 = automatic: measured once at the first teuk_step,
  *                   which then waits for a few untimed-by-the-caller trial launches into scratch memory)
  *   "autotune"      1 = measure the slab length (default), 0 = use the two-wave heuristic
  *   "graph"         1 = replay the iteration through a CUDA graph (default), 0 = plain launches
  *   "kernel"        0 = register-resident marching kernel, 1 = shared-memory-resident marching kernel
- *                   (same arithmetic, bitwise identical fields; they differ in on-chip residency) */
+ *                   (same arithmetic, bitwise identical fields; they differ in on-chip residency;
+ *                   kernel 1 needs n_theta <= 256) */
 int teuk_set_option(teuk_solver *s, const char *key, int64_t value);
 
 /* Read-only counters: "steps" (iterations done), "launches" (kernels launched so far),

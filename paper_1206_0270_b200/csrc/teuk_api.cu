@@ -124,18 +124,25 @@ void drop_graph(teuk_solver* s) {
     }
 }
 
+// theta segments of the register kernel: one warp spans up to 128 columns; wider grids are cut into
+// segments of <= 120 payload columns (+ 4 halo columns on each side inside the warp's 128-column window).
+int n_segments(const teuk_solver* s) {
+  if (s->variant == 1 || s->n_theta <= 128) return 1;
+  return (s->n_theta + 119) / 120;
+}
+
 // Heuristic slab length (rows of r* marched by one warp): two waves of the warps that fit on the chip.
 // It seeds the autotune below and is used as is when autotuning is switched off.
 int resident_warps(const teuk_solver* s) {
   const int sms = s->n_sms > 0 ? s->n_sms : 148;
   const int v = (s->n_theta + 31) / 32;
-  return sms * (s->variant == 1 ? 12 : (v <= 1 ? 16 : 8));
+  return sms * (s->variant == 1 ? 12 : (v <= 1 ? 16 : 8));   // measured occupancies of the kernels
 }
 
 int rows_for_waves(const teuk_solver* s, double waves) {
   const long long interior = s->n_r - 2;
   const double target = waves * resident_warps(s);
-  long long rows = (long long)((interior * s->n_modes + target - 1) / target);
+  long long rows = (long long)((interior * s->n_modes * n_segments(s) + target - 1) / target);
   if (rows < 1) rows = 1;
   if (rows > interior) rows = interior;
   return (int)rows;
@@ -157,6 +164,8 @@ void fill_params(const teuk_solver* s, StepParams* p, int in_buf, int k, int tap
   p->slab_rows = s->slab_rows_opt > 0 ? s->slab_rows_opt : (s->tuned_rows > 0 ? s->tuned_rows : auto_slab_rows(s));
   if (p->slab_rows > s->n_r - 2) p->slab_rows = s->n_r - 2;
   p->n_slabs = (s->n_r - 2 + p->slab_rows - 1) / p->slab_rows;
+  p->n_seg = n_segments(s);
+  p->seg_payload = p->n_seg > 1 ? ((s->n_theta + p->n_seg - 1) / p->n_seg + 3) / 4 * 4 : s->n_theta;
   p->outer_bc = s->outer_bc;
   p->variant = s->variant;
   p->dt = s->dt;
@@ -289,8 +298,8 @@ int teuk_create(teuk_solver** out, double a, double M, const int32_t* m, int32_t
   if (!m || !grid) return fail(nullptr, TEUK_EINVAL, "teuk_create: m or grid is NULL");
   if (!(M > 0.0) || !(fabs(a) < M)) return fail(nullptr, TEUK_EINVAL, "teuk_create: need M > 0 and |a| < M");
   if (n_modes < 1 || n_modes > TEUK_MAX_MODES) return fail(nullptr, TEUK_EINVAL, "teuk_create: n_modes must be 1..64");
-  if (grid->n_r < 4 || grid->n_theta < 4 || grid->n_theta > 256)
-    return fail(nullptr, TEUK_EINVAL, "teuk_create: need n_r >= 4 and 4 <= n_theta <= 256");
+  if (grid->n_r < 4 || grid->n_theta < 4 || grid->n_theta > 4096)
+    return fail(nullptr, TEUK_EINVAL, "teuk_create: need n_r >= 4 and 4 <= n_theta <= 4096");
   if (!(grid->rs_max > grid->rs_min) || !(dt > 0.0) || !isfinite(dt) || !isfinite(grid->rs_min) ||
       !isfinite(grid->rs_max))
     return fail(nullptr, TEUK_EINVAL, "teuk_create: need rs_max > rs_min and dt > 0");
@@ -434,10 +443,15 @@ int build_graph(teuk_solver* s) {
   cudaGraph_t graph = nullptr;
   CK(cudaStreamBeginCapture(s->own_stream, cudaStreamCaptureModeThreadLocal), "graph: begin capture");
   cudaError_t e = cudaSuccess;
+  const bool sep_tap = n_segments(s) > 1 && s->n_obs > 0;   // theta segments: the tap is its own small kernel
   for (int k = 0; k < kGraphBatch && e == cudaSuccess; ++k) {
     StepParams p;
-    fill_params(s, &p, s->cur ^ (k & 1), k, 1);
+    fill_params(s, &p, s->cur ^ (k & 1), k, sep_tap ? 0 : 1);
     e = teuk_launch_step(p, s->own_stream);
+    if (sep_tap && e == cudaSuccess) {
+      fill_params(s, &p, s->cur ^ ((k + 1) & 1), k + 1, 1);
+      e = teuk_launch_flush_tap(p, s->own_stream);
+    }
   }
   if (e == cudaSuccess) e = teuk_launch_bump(s->d_base, kGraphBatch, s->own_stream);
   cudaError_t e2 = cudaStreamEndCapture(s->own_stream, &graph);
@@ -526,7 +540,7 @@ int run_chunk(teuk_solver* s, long long c) {
       CK(cudaGraphLaunch(s->graph_exec[s->cur], s->stream), "step: graph launch");
       s->base_on_device += kGraphBatch;
       s->step += kGraphBatch;
-      s->launches += kGraphBatch + 1;
+      s->launches += kGraphBatch * (n_segments(s) > 1 && s->n_obs > 0 ? 2 : 1) + 1;
       left -= kGraphBatch;
       continue;
     }
@@ -536,14 +550,20 @@ int run_chunk(teuk_solver* s, long long c) {
       s->base_on_device = s->step;
       s->launches += 1;
     }
+    const bool sep_tap = n_segments(s) > 1 && s->n_obs > 0;
     StepParams p;
-    fill_params(s, &p, s->cur, (int)(s->step - s->base_on_device), first ? 0 : 1);
+    fill_params(s, &p, s->cur, (int)(s->step - s->base_on_device), (first || sep_tap) ? 0 : 1);
     CK(teuk_launch_step(p, s->stream), "step: launch");
     s->launches += 1;
     s->cur ^= 1;
     s->step += 1;
     left -= 1;
     first = 0;
+    if (sep_tap && left > 0) {   // the level just produced (the last one is tapped below)
+      fill_params(s, &p, s->cur, (int)(s->step - s->base_on_device), 1);
+      CK(teuk_launch_flush_tap(p, s->stream), "step: tap");
+      s->launches += 1;
+    }
   }
   if (s->n_obs > 0) {
     StepParams p;
@@ -689,6 +709,7 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
   } else if (!strcmp(key, "coef_mode")) {
     if (value != 0 && value != 1) return fail(s, TEUK_EINVAL, "coef_mode must be 0 or 1");
     if (value == 1 && s->variant != 0) return fail(s, TEUK_EINVAL, "coef_mode 1 needs kernel 0");
+    if (value == 1 && n_segments(s) > 1) return fail(s, TEUK_EINVAL, "coef_mode 1 needs n_theta <= 128");
     if (value == 1 && !s->d_coef2d) {
       const size_t bytes = (size_t)s->n_modes * (2 * (size_t)s->n_r - 1) * 8 * s->n_theta * sizeof(double);
       CK(cudaMalloc((void**)&s->d_coef2d, bytes), "coef_mode: alloc of the 2D coefficient planes");
@@ -707,6 +728,7 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
   } else if (!strcmp(key, "kernel")) {
     if (value != 0 && value != 1) return fail(s, TEUK_EINVAL, "kernel must be 0 (register-resident) or 1 (shared-memory-resident)");
     if (value == 1 && s->coef_mode != 0) return fail(s, TEUK_EINVAL, "kernel 1 needs coef_mode 0");
+    if (value == 1 && s->n_theta > 256) return fail(s, TEUK_EINVAL, "kernel 1 needs n_theta <= 256");
     s->variant = (int)value;
   } else {
     return fail(s, TEUK_EINVAL, "teuk_set_option: unknown key");

@@ -59,6 +59,7 @@ struct StepParams {
   int coef_mode;
   int n_r, n_theta, n_modes;
   int slab_rows, n_slabs;
+  int n_seg, seg_payload; // theta segments (register kernel, n_theta > 128): count and payload columns each
   int variant;            // 0 = register-resident kernel, 1 = shared-memory-resident kernel
   int outer_bc;
   double dt, dx, rs_min, dth;

@@ -115,7 +115,7 @@ __device__ __forceinline__ void load_row(Row<V>& u, const double* __restrict__ r
   for (int c = 0; c < 4; ++c) {
     const double* p = row + (size_t)c * nth + j0;
     if (VEC) {
-      if (j0 < nth) {
+      if ((unsigned)j0 < (unsigned)nth) {
         if (V == 1) {
           u.c[c][0] = __ldcs(p);
         } else if (V % 4 == 0) {
@@ -135,18 +135,20 @@ __device__ __forceinline__ void load_row(Row<V>& u, const double* __restrict__ r
       }
     } else {
 #pragma unroll
-      for (int v = 0; v < V; ++v) u.c[c][v] = (j0 + v < nth) ? __ldcs(p + v) : 0.0;
+      for (int v = 0; v < V; ++v) u.c[c][v] = ((unsigned)(j0 + v) < (unsigned)nth) ? __ldcs(p + v) : 0.0;
     }
   }
 }
 
+// Columns outside [pay_lo, pay_hi) (halo columns of a theta segment, idle lanes) are not stored.
 template <int V, bool VEC>
-__device__ __forceinline__ void store_row(const Row<V>& u, double* __restrict__ row, int nth, int j0) {
+__device__ __forceinline__ void store_row(const Row<V>& u, double* __restrict__ row, int nth, int j0, int pay_lo,
+                                          int pay_hi) {
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
     double* p = row + (size_t)c * nth + j0;
     if (VEC) {
-      if (j0 < nth) {
+      if (j0 >= pay_lo && j0 < pay_hi) {
         if (V == 1) {
           __stcs(p, u.c[c][0]);
         } else if (V % 4 == 0) {
@@ -160,7 +162,7 @@ __device__ __forceinline__ void store_row(const Row<V>& u, double* __restrict__ 
     } else {
 #pragma unroll
       for (int v = 0; v < V; ++v)
-        if (j0 + v < nth) __stcs(p + v, u.c[c][v]);
+        if (j0 + v >= pay_lo && j0 + v < pay_hi) __stcs(p + v, u.c[c][v]);
     }
   }
 }
@@ -370,7 +372,7 @@ struct StageSource {
 
 template <int V, int MAP = 0>
 __device__ __forceinline__ void setup_source(StageSource<V>& s, const StepParams& p, int mode, long long ks,
-                                             bool half, int row_lo, int row_hi, int lane) {
+                                             bool half, int row_lo, int row_hi, int lane, int col0 = 0) {
   s.on = false;
   if (!p.has_source) return;
   const double xp = p.xp[ks], thp = p.thp[ks];
@@ -387,9 +389,9 @@ __device__ __forceinline__ void setup_source(StageSource<V>& s, const StepParams
   s.aim = p.amp_im[(size_t)mode * p.n_samples + ks];
 #pragma unroll
   for (int q = 0; q < V; ++q) {
-    const int j = col_of<V, MAP>(lane, q);
+    const int j = col0 + col_of<V, MAP>(lane, q);
     const double th = __dmul_rn((double)j + 0.5, p.dth);
-    s.gth[q] = (j < p.n_theta && abs(j - jp) <= p.W) ? gauss_dev(th - thp, p.sigma_th) : 0.0;
+    s.gth[q] = ((unsigned)j < (unsigned)p.n_theta && abs(j - jp) <= p.W) ? gauss_dev(th - thp, p.sigma_th) : 0.0;
   }
 }
 
@@ -466,11 +468,11 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
 
 // shared-memory row (same [comp][n_theta] layout as HBM) -> registers
 template <int V>
-__device__ __forceinline__ void lds_row(Row<V>& u, const double* srow, int nth, int j0) {
+__device__ __forceinline__ void lds_row(Row<V>& u, const double* srow, int comp_stride, int col, bool valid) {
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
-    if (j0 < nth) {
-      const double* q = srow + c * nth + j0;
+    if (valid) {
+      const double* q = srow + c * comp_stride + col;
       if (V == 1) {
         u.c[c][0] = q[0];
       } else {
@@ -507,7 +509,11 @@ __device__ __forceinline__ void stage_rtab_chunk(double* sbuf, const double* __r
   asm volatile("cp.async.commit_group;" ::: "memory");
 }
 
-template <int V, bool VEC, int CM>
+// SEG: the theta range is split into gridDim.z segments of p.seg_payload columns (n_theta > 32 V, e.g. the
+// paper's 32000 x 304 grid).  A warp then owns a window of 32 V columns: its payload plus a
+// 4-column halo on each side, recomputed redundantly (the stencil reaches 2 columns per iteration), so no
+// exchange between warps is needed; only payload columns are stored.
+template <int V, bool VEC, int CM, bool SEG>
 __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const __grid_constant__ StepParams p) {
   const int lane = threadIdx.x & 31;
   const int slab = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -516,7 +522,11 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
   if (slab >= p.n_slabs) return;
   const int r0 = 1 + slab * p.slab_rows;             // first interior node of this slab
   const int r1 = min(r0 + p.slab_rows, nr - 1);      // one past the last
-  const int j0 = lane * V;
+  const int c_lo = SEG ? (int)blockIdx.z * p.seg_payload - 4 : 0;            // first column of the window
+  const int pay_lo = SEG ? (int)blockIdx.z * p.seg_payload : 0;
+  const int pay_hi = SEG ? min(pay_lo + p.seg_payload, nth) : nth;
+  const int j0 = c_lo + lane * V;                    // may be negative or >= nth in a segment's halo
+  const int slot_cs = SEG ? 32 * V : nth;            // component stride inside a landing slot
   const size_t row_stride = (size_t)4 * nth;
   const double* __restrict__ uin = p.uin + (size_t)mode * nr * row_stride;
   double* __restrict__ uout = p.uout + (size_t)mode * nr * row_stride;
@@ -529,8 +539,26 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
   double* const rt_buf = &s_rt[wib][0][0];
   stage_rtab_chunk(rt_buf, rtab, 2 * r0, 2 * nr - 1, lane);
   const unsigned row_bytes = (unsigned)(row_stride * sizeof(double));
-  double* const slot0 = reinterpret_cast<double*>(s_dyn) + (size_t)wib * 2 * row_stride;
+  const size_t slot_doubles = (size_t)4 * slot_cs;
+  double* const slot0 = reinterpret_cast<double*>(s_dyn) + (size_t)wib * 2 * slot_doubles;
   unsigned long long* const bars = &s_bar[wib][0];
+  // One TMA bulk copy per row (whole row), or four (one per component) for a theta segment's window.
+  const int g_lo = max(c_lo, 0), g_hi = min(c_lo + 32 * V, nth);
+  auto issue_row = [&](int q) {
+    double* dst = slot0 + (size_t)(q & 1) * slot_doubles;
+    const double* src = uin + (size_t)q * row_stride;
+    if (!SEG) {
+      tma_load_row(dst, src, row_bytes, &bars[q & 1]);
+    } else {
+      const unsigned bytes = (unsigned)((g_hi - g_lo) * sizeof(double));
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&bars[q & 1])), "r"(4u * bytes) : "memory");
+#pragma unroll
+      for (int c = 0; c < 4; ++c)
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"(smem_u32(dst + c * slot_cs + (g_lo - c_lo))), "l"(src + (size_t)c * nth + g_lo), "r"(bytes),
+                     "r"(smem_u32(&bars[q & 1])) : "memory");
+    }
+  };
   if (VEC) {
     if (lane == 0) {
       mbar_init(&bars[0], 1);
@@ -538,9 +566,7 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       // row q lands in slot q & 1; rows r0+2 and (mid-iteration r0) r0+3 are the first uses
-      if (r0 + 2 <= r1)
-        tma_load_row(slot0 + (size_t)((r0 + 2) & 1) * row_stride, uin + (size_t)(r0 + 2) * row_stride, row_bytes,
-                     &bars[(r0 + 2) & 1]);
+      if (r0 + 2 <= r1) issue_row(r0 + 2);
     }
     __syncwarp();
   }
@@ -550,7 +576,7 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
     const double* tb = p.ttab + (size_t)mode * TT_N * nth;
 #pragma unroll
     for (int v = 0; v < V; ++v) {
-      const bool ok = j0 + v < nth;
+      const bool ok = (unsigned)(j0 + v) < (unsigned)nth;
       th.vals.s2[v] = ok ? tb[TT_S2 * nth + j0 + v] : 0.0;
       th.vals.cs[v] = ok ? tb[TT_COS * nth + j0 + v] : 0.0;
       th.vals.ap[v] = ok ? tb[TT_AP * nth + j0 + v] : 0.0;
@@ -559,9 +585,9 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
     }
   }
   StageSource<V> src_h, src_f;   // half stage: sample 2n at half points; full stage: 2n+1 at nodes
-  setup_source<V>(src_h, p, mode, 2 * n, true, r0 - 1, r1 - 1, lane);
-  setup_source<V>(src_f, p, mode, 2 * n + 1, false, r0, r1 - 1, lane);
-  const bool do_tap = p.tap_enable && p.n_obs > 0 && n >= 1;
+  setup_source<V>(src_h, p, mode, 2 * n, true, r0 - 1, r1 - 1, lane, c_lo);
+  setup_source<V>(src_f, p, mode, 2 * n + 1, false, r0, r1 - 1, lane, c_lo);
+  const bool do_tap = !SEG && p.tap_enable && p.n_obs > 0 && n >= 1;   // segments: separate tap kernel
   const double tau_h = 0.5 * p.dt, tau_f = 0.25 * p.dt, tdx = 2.0 / p.dx;
 
   Row<V> ua, ub, uc, hp, hn, out;
@@ -612,20 +638,18 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
       // B (row i+1, read from slot (i+1)&1 at the end of the last iteration) has been consumed by
       // every lane: its slot may now receive row i+3.
       __syncwarp();
-      if (lane == 0 && i + 3 <= r1)
-        tma_load_row(slot0 + (size_t)((i + 3) & 1) * row_stride, uin + (size_t)(i + 3) * row_stride, row_bytes,
-                     &bars[(i + 3) & 1]);
+      if (lane == 0 && i + 3 <= r1) issue_row(i + 3);
     }
     if (CM == 1)
       lw_stage_planes<V, false, VEC>(Hp, Hn, A, planes + (size_t)(2 * i) * loc_stride, th, tau_f, out, nth, j0);
     else
       lw_stage<V, false>(Hp, Hn, A, rt_cur + (2 * o) * RT_N, th, tau_f, tdx, out);
     add_source<V>(out, src_f, p, i, false);
-    store_row<V, VEC>(out, uout + (size_t)i * row_stride, nth, j0);
+    store_row<V, VEC>(out, uout + (size_t)i * row_stride, nth, j0, pay_lo, pay_hi);
     if (VEC) {
       if (i + 2 <= r1) {
         mbar_wait(&bars[(i + 2) & 1], (unsigned)(((i + 2) - (r0 + 2)) >> 1) & 1u);
-        lds_row<V>(A, slot0 + (size_t)((i + 2) & 1) * row_stride, nth, j0);
+        lds_row<V>(A, slot0 + (size_t)((i + 2) & 1) * slot_doubles, slot_cs, lane * V, (unsigned)j0 < (unsigned)nth);
       }
     } else {
       A = ua;
@@ -654,7 +678,7 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
     for (int c = 0; c < 4; ++c)
 #pragma unroll
       for (int v = 0; v < V; ++v) out.c[c][v] = 0.0;
-    store_row<V, VEC>(out, uout, nth, j0);
+    store_row<V, VEC>(out, uout, nth, j0, pay_lo, pay_hi);
   }
   if (r1 == nr - 1) {
     load_row<V, VEC>(ub, uin + (size_t)(nr - 1) * row_stride, nth, j0);
@@ -675,7 +699,7 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
       out.c[2][v] = 0.0;
       out.c[3][v] = 0.0;
     }
-    store_row<V, VEC>(out, uout + (size_t)(nr - 1) * row_stride, nth, j0);
+    store_row<V, VEC>(out, uout + (size_t)(nr - 1) * row_stride, nth, j0, pay_lo, pay_hi);
   }
 }
 
@@ -947,8 +971,10 @@ __global__ void teuk_flush_tap_kernel(const __grid_constant__ StepParams p) {
   // same lane -> column ownership and summation order as the in-kernel tap (bitwise identical)
   const int vreq = (nth + 31) / 32;
   const int V = vreq <= 1 ? 1 : (vreq <= 2 ? 2 : (vreq <= 4 ? 4 : 8));
-  for (int v = 0; v < V; ++v) {
-    const int j = (p.variant == 1 && V > 1) ? (v >> 1) * 64 + 2 * lane + (v & 1) : lane * V + v;
+  const int n_it = p.n_seg > 1 ? (nth + 31) / 32 : V;
+  for (int v = 0; v < n_it; ++v) {
+    const int j = p.n_seg > 1 ? v * 32 + lane
+                              : ((p.variant == 1 && V > 1) ? (v >> 1) * 64 + 2 * lane + (v & 1) : lane * V + v);
     if (j >= nth) continue;
     const double wt = p.obs[q].weights[j];
     wr = fma(wt, fma(f, hi[j], (1.0 - f) * lo[j]), wr);
@@ -999,25 +1025,27 @@ __global__ void teuk_unpack_kernel(const double* __restrict__ u, Planes dst, siz
 template <int V>
 static cudaError_t launch_v(const StepParams& p, cudaStream_t st) {
   const int warps_per_block = 4;
-  dim3 grid((p.n_slabs + warps_per_block - 1) / warps_per_block, p.n_modes), block(32 * warps_per_block);
+  dim3 grid((p.n_slabs + warps_per_block - 1) / warps_per_block, p.n_modes, p.n_seg), block(32 * warps_per_block);
   const bool vec = p.n_theta % V == 0;
-  const size_t dyn = vec ? (size_t)warps_per_block * 2 * 4 * p.n_theta * sizeof(double) : 0;
   const int dyn_max = (int)((size_t)warps_per_block * 2 * 4 * 32 * V * sizeof(double));
-#define TEUK_LAUNCH(VECF, CMF)                                                                               \
+  const size_t dyn = vec ? (size_t)dyn_max : 0;
+#define TEUK_LAUNCH(VECF, CMF, SEGF)                                                                         \
   do {                                                                                                       \
     static bool attr_set = false;                                                                            \
     if (!attr_set) {                                                                                         \
-      cudaError_t e = cudaFuncSetAttribute(teuk_step_kernel<V, VECF, CMF>,                                   \
+      cudaError_t e = cudaFuncSetAttribute(teuk_step_kernel<V, VECF, CMF, SEGF>,                             \
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max);            \
       if (e != cudaSuccess) return e;                                                                        \
       attr_set = true;                                                                                       \
     }                                                                                                        \
-    teuk_step_kernel<V, VECF, CMF><<<grid, block, dyn, st>>>(p);                                             \
+    teuk_step_kernel<V, VECF, CMF, SEGF><<<grid, block, dyn, st>>>(p);                                       \
   } while (0)
-  if (p.coef_mode == 1) {
-    if (vec) TEUK_LAUNCH(true, 1); else TEUK_LAUNCH(false, 1);
+  if (p.n_seg > 1) {
+    if (vec) TEUK_LAUNCH(true, 0, true); else TEUK_LAUNCH(false, 0, true);
+  } else if (p.coef_mode == 1) {
+    if (vec) TEUK_LAUNCH(true, 1, false); else TEUK_LAUNCH(false, 1, false);
   } else {
-    if (vec) TEUK_LAUNCH(true, 0); else TEUK_LAUNCH(false, 0);
+    if (vec) TEUK_LAUNCH(true, 0, false); else TEUK_LAUNCH(false, 0, false);
   }
 #undef TEUK_LAUNCH
   return cudaGetLastError();
@@ -1059,8 +1087,7 @@ cudaError_t teuk_launch_step(const StepParams& p, cudaStream_t st) {
   }
   if (v <= 1) return launch_v<1>(p, st);
   if (v <= 2) return launch_v<2>(p, st);
-  if (v <= 4) return launch_v<4>(p, st);
-  return launch_v<8>(p, st);
+  return launch_v<4>(p, st);   // n_theta > 128: theta segments of <= 120 payload columns (p.n_seg > 1)
 }
 
 cudaError_t teuk_launch_flush_tap(const StepParams& p, cudaStream_t st) {

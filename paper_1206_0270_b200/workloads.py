@@ -80,6 +80,10 @@ CONFIGS: Dict[int, Config] = {
               16000, 64, 0.05, 50000, (50.0,), "zero", "eccentric"),
     5: Config(5, "kerr099_production_131072x128", 0.99, 1.0, (2,), -200.0, 1800.0, 131072, 128,
               0.125, 200000, (1500.0, 50.0), "zero", "inspiral"),
+    # Not a BASELINE.json config: the (r, theta) grid of the paper's own Table 1 measurement,
+    # 32000 x 304, with config 3's physics.  Exercises the theta-segmented kernel path.
+    6: Config(6, "paper_table1_grid_32000x304", 0.9, 1.0, (2,), -100.0, 1900.0, 32000, 304, 0.0125, 20000,
+              (50.0,), "zero", "circular"),
 }
 
 

@@ -214,7 +214,7 @@ def test_argument_errors(teuk):
     with pytest.raises(teuk.TeukError):
         teuk.Solver(0.5, 1.0, [2], -10, 10, 3, 32, 0.01)        # n_r < 4
     with pytest.raises(teuk.TeukError):
-        teuk.Solver(0.5, 1.0, [2], -10, 10, 64, 300, 0.01)      # n_theta > 256
+        teuk.Solver(0.5, 1.0, [2], -10, 10, 64, 5000, 0.01)     # n_theta > 4096
     cfg = SMALL[3]
     g = teuk.Solver.from_config(cfg)
     g.set_source(wl.orbit_table(cfg, n_steps=5))
@@ -284,7 +284,7 @@ def test_streamed_coefficient_planes_parity(orc, teuk, cfg):
     check_pair(res, tol=1e-12)
 
 
-@pytest.mark.parametrize("n_theta", [20, 45, 64, 100, 128, 256])
+@pytest.mark.parametrize("n_theta", [20, 45, 64, 100, 128])
 def test_streamed_coefficient_planes_theta_sizes(orc, teuk, n_theta):
     cfg = SMALL[3].scaled(name="cm%d" % n_theta, n_r=150, n_theta=n_theta, dt_over_dx=0.02, steps=8, modes=(2, 1))
     res = run_pair(orc, teuk, cfg, 8, initial=wl.random_state(cfg, n_theta), options={"coef_mode": 1})
@@ -308,3 +308,22 @@ def test_autotune_does_not_change_results(orc, teuk):
     for a, b in zip(out[0][0], out[1][0]):
         assert np.array_equal(a, b)
     assert np.array_equal(out[0][1][1], out[1][1][1]) and len(out[0][1][0]) == 60
+
+
+@pytest.mark.parametrize("n_theta", [129, 132, 200, 240, 256, 304, 360, 361, 513, 1000])
+def test_theta_segments(orc, teuk, n_theta):
+    """n_theta > 128: several warps per row, each with a 4-column halo (the paper's grid has 304 columns)."""
+    cfg = SMALL[3].scaled(name="seg%d" % n_theta, n_r=97, n_theta=n_theta, dt_over_dx=0.002, steps=10, modes=(2, 1),
+                          observers=(30.0, -29.9))
+    res = run_pair(orc, teuk, cfg, 10, initial=wl.random_state(cfg, n_theta), chunks=[1, 2, 7])
+    check_pair(res, tol=1e-11)
+    res = run_pair(orc, teuk, cfg, 40, initial=wl.random_state(cfg, n_theta + 1))     # graph replay + separate taps
+    check_pair(res, tol=1e-11)
+    assert len(res["wg"][0][0]) == 40
+
+
+def test_paper_grid_quick(orc, teuk):
+    """32000 x 304, cropped in r* so the oracle finishes in seconds."""
+    cfg = wl.CONFIGS[6].scaled(name="paper_grid_crop", n_r=2000, rs_min=-30.0, rs_max=-30.0 + 1999 * wl.CONFIGS[6].dx,
+                               steps=100)
+    check_pair(run_pair(orc, teuk, cfg, 100, observers=[50.0]))
