@@ -1031,12 +1031,14 @@ static cudaError_t launch_v(const StepParams& p, cudaStream_t st) {
   const size_t dyn = vec ? (size_t)dyn_max : 0;
 #define TEUK_LAUNCH(VECF, CMF, SEGF)                                                                         \
   do {                                                                                                       \
-    static bool attr_set = false;                                                                            \
-    if (!attr_set) {                                                                                         \
+    static bool attr_set[64] = {false};   /* per device: function attributes belong to a context */         \
+    int dev_ = 0;                                                                                            \
+    cudaGetDevice(&dev_);                                                                                    \
+    if (!attr_set[dev_ & 63]) {                                                                              \
       cudaError_t e = cudaFuncSetAttribute(teuk_step_kernel<V, VECF, CMF, SEGF>,                             \
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max);            \
       if (e != cudaSuccess) return e;                                                                        \
-      attr_set = true;                                                                                       \
+      attr_set[dev_ & 63] = true;                                                                            \
     }                                                                                                        \
     teuk_step_kernel<V, VECF, CMF, SEGF><<<grid, block, dyn, st>>>(p);                                       \
   } while (0)
@@ -1058,19 +1060,23 @@ static cudaError_t launch_smem_v(const StepParams& p, cudaStream_t st) {
   const size_t dyn = (size_t)warps_per_block * (2 * 4 * (size_t)p.n_theta + 4 * 32 * V) * sizeof(double);
   const int dyn_max = (int)((size_t)warps_per_block * (2 * 4 * 32 * V + 4 * 32 * V) * sizeof(double));
   if (p.n_theta % 2 == 0 || V == 1) {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static bool attr_set[64] = {false};   // per device
+    int dev_ = 0;
+    cudaGetDevice(&dev_);
+    if (!attr_set[dev_ & 63]) {
       cudaError_t e = cudaFuncSetAttribute(teuk_step_smem_kernel<V, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max);
       if (e != cudaSuccess) return e;
-      attr_set = true;
+      attr_set[dev_ & 63] = true;
     }
     teuk_step_smem_kernel<V, true><<<grid, block, dyn, st>>>(p);
   } else {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static bool attr_set[64] = {false};   // per device
+    int dev_ = 0;
+    cudaGetDevice(&dev_);
+    if (!attr_set[dev_ & 63]) {
       cudaError_t e = cudaFuncSetAttribute(teuk_step_smem_kernel<V, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max);
       if (e != cudaSuccess) return e;
-      attr_set = true;
+      attr_set[dev_ & 63] = true;
     }
     teuk_step_smem_kernel<V, false><<<grid, block, dyn, st>>>(p);
   }
