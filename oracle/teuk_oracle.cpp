@@ -21,7 +21,7 @@
 // tests/test_oracle_pins.py against a computer-algebra substitution into Eq. (1) (pin P1),
 // by second-order self-convergence (P2), by the Schwarzschild and Kerr l=m=2 quasinormal
 // frequencies (P3, P3b), by the (m, theta) reflection invariant (P4), a = 0 realness (P5),
-// linearity (P6) and the unit norm of the deposit (P7).  The paper prints no field values:
+// linearity (P6), the unit norm of the deposit (P7) and the edge rows' closed forms (P8).  The paper prints no field values:
 // beyond those pins the numbers this file produces are "parity unpinned" by the paper.
 //
 // Readings of silent/ambiguous passages are the A1-A12 of SURVEY.md 8(c), restated in DESIGN.md.

@@ -347,3 +347,34 @@ def test_p7_source_norm_support_and_time_levels(orc):
             assert np.all(hs[2] == 0.0) and np.all(phi_re == 0.0)
             assert np.allclose(pi_re[0][1:-1], cfg.dt * Tn.real[1:-1], rtol=1e-14, atol=0)
         o2.close()
+
+
+# ------------------------------------------------------------------------------------------ P8
+def test_p8_outer_edge_branches_and_domain_of_dependence(orc):
+    """Radial edge conditions.  One iteration moves information by one row, so after n
+    iterations the two outer-edge branches (Dirichlet as printed / outgoing, reading A6) may differ only in
+    the last n+1 rows, bit for bit elsewhere; the Dirichlet edge rows are exactly zero; with b = 1 (a = 0)
+    the outgoing edge advects Phi outwards: Phi' = Phi - dt (Phi_N - Phi_{N-1})/dx."""
+    cfg = wl.CONFIGS[1].scaled(name="edge", n_r=80, rs_min=40.0, rs_max=40.0 + 79 * 0.4, steps=12)
+    ini = wl.random_state(cfg, 3)
+    n = 12
+    out = []
+    for bc in (0, 1):
+        o = orc.OracleSolver.from_config(cfg.scaled(outer_bc=bc))
+        o.set_initial(*ini)
+        o.step(1)
+        first = o.get_state()
+        o.step(n - 1)
+        out.append((first, o.get_state()))
+        o.close()
+    (f0, s0), (f1, s1) = out
+    for a, b in zip(s0, s1):
+        assert np.array_equal(a[:, : cfg.n_r - n - 1], b[:, : cfg.n_r - n - 1])
+        assert not np.array_equal(a[:, -n:], b[:, -n:])
+    for q in range(4):
+        assert np.all(f1[q][:, 0] == 0.0) and np.all(f1[q][:, -1] == 0.0)      # Dirichlet: both edges
+        assert np.all(f0[q][:, 0] == 0.0)                                      # inner edge always
+    assert np.all(f0[2][:, -1] == 0.0) and np.all(f0[3][:, -1] == 0.0)         # outgoing: Pi = 0
+    for q in (0, 1):                                                           # a = 0: b = 1 exactly
+        exp = ini[q][:, -1] - cfg.dt * 1.0 * (ini[q][:, -1] - ini[q][:, -2]) / cfg.dx
+        assert np.allclose(f0[q][:, -1], exp, rtol=1e-14, atol=1e-15)
