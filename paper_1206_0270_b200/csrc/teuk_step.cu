@@ -587,7 +587,13 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
   StageSource<V> src_h, src_f;   // half stage: sample 2n at half points; full stage: 2n+1 at nodes
   setup_source<V>(src_h, p, mode, 2 * n, true, r0 - 1, r1 - 1, lane, c_lo);
   setup_source<V>(src_f, p, mode, 2 * n + 1, false, r0, r1 - 1, lane, c_lo);
-  const bool do_tap = !SEG && p.tap_enable && p.n_obs > 0 && n >= 1;   // segments: separate tap kernel
+  bool do_tap = !SEG && p.tap_enable && p.n_obs > 0 && n >= 1;   // segments: separate tap kernel
+  if (do_tap) {  // only the warp whose slab holds an observer's rows i0, i0+1 ever taps
+    bool mine = false;
+    for (int q = 0; q < p.n_obs; ++q) mine = mine || (p.obs[q].i0 >= r0 - 1 && p.obs[q].i0 < r1);
+    do_tap = mine;
+  }
+  const bool any_src = src_h.on || src_f.on;
   const double tau_h = 0.5 * p.dt, tau_f = 0.25 * p.dt, tdx = 2.0 / p.dx;
 
   Row<V> ua, ub, uc, hp, hn, out;
@@ -633,7 +639,7 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
     } else {
       lw_stage<V, true>(A, B, A, rt_cur + (2 * o + 1) * RT_N, th, tau_h, tdx, Hn);
     }
-    add_source<V>(Hn, src_h, p, i, true);
+    if (any_src) add_source<V>(Hn, src_h, p, i, true);
     if (VEC) {
       // B (row i+1, read from slot (i+1)&1 at the end of the last iteration) has been consumed by
       // every lane: its slot may now receive row i+3.
@@ -644,7 +650,7 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
       lw_stage_planes<V, false, VEC>(Hp, Hn, A, planes + (size_t)(2 * i) * loc_stride, th, tau_f, out, nth, j0);
     else
       lw_stage<V, false>(Hp, Hn, A, rt_cur + (2 * o) * RT_N, th, tau_f, tdx, out);
-    add_source<V>(out, src_f, p, i, false);
+    if (any_src) add_source<V>(out, src_f, p, i, false);
     store_row<V, VEC>(out, uout + (size_t)i * row_stride, nth, j0, pay_lo, pay_hi);
     if (VEC) {
       if (i + 2 <= r1) {
