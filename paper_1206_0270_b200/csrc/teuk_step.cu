@@ -44,6 +44,9 @@ struct Row {
 #ifndef TEUK_UNROLL2
 #define TEUK_UNROLL2 1
 #endif
+#ifndef TEUK_SLOTS
+#define TEUK_SLOTS 2    // TMA landing slots per warp (register kernel): rows i+2 .. i+TEUK_SLOTS+1 in flight (3, 4: no gain)
+#endif
 #ifndef TEUK_GROUP
 #define TEUK_GROUP 2    // columns processed "vertically" together inside a stage (ILP)
 #endif
@@ -533,40 +536,43 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
   const double* __restrict__ rtab = p.rtab + (size_t)mode * (2 * nr - 1) * RT_N;
   const long long n = *p.d_base + p.k;               // index of the input time level
   __shared__ __align__(16) double s_rt[4][2][RT_CHUNK_DOUBLES];
-  __shared__ __align__(8) unsigned long long s_bar[4][2];
-  extern __shared__ __align__(128) unsigned char s_dyn[];   // VEC: [warp][2 slots][4 n_theta] doubles
+  constexpr int NS = TEUK_SLOTS;
+  __shared__ __align__(8) unsigned long long s_bar[4][NS];
+  extern __shared__ __align__(128) unsigned char s_dyn[];   // VEC: [warp][TEUK_SLOTS][4 n_theta] doubles
   const int wib = threadIdx.x >> 5;
   double* const rt_buf = &s_rt[wib][0][0];
   stage_rtab_chunk(rt_buf, rtab, 2 * r0, 2 * nr - 1, lane);
   const unsigned row_bytes = (unsigned)(row_stride * sizeof(double));
   const size_t slot_doubles = (size_t)4 * slot_cs;
-  double* const slot0 = reinterpret_cast<double*>(s_dyn) + (size_t)wib * 2 * slot_doubles;
+  double* const slot0 = reinterpret_cast<double*>(s_dyn) + (size_t)wib * NS * slot_doubles;
   unsigned long long* const bars = &s_bar[wib][0];
   // One TMA bulk copy per row (whole row), or four (one per component) for a theta segment's window.
   const int g_lo = max(c_lo, 0), g_hi = min(c_lo + 32 * V, nth);
   auto issue_row = [&](int q) {
-    double* dst = slot0 + (size_t)(q & 1) * slot_doubles;
+    double* dst = slot0 + (size_t)(q % NS) * slot_doubles;
     const double* src = uin + (size_t)q * row_stride;
     if (!SEG) {
-      tma_load_row(dst, src, row_bytes, &bars[q & 1]);
+      tma_load_row(dst, src, row_bytes, &bars[q % NS]);
     } else {
       const unsigned bytes = (unsigned)((g_hi - g_lo) * sizeof(double));
-      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&bars[q & 1])), "r"(4u * bytes) : "memory");
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&bars[q % NS])), "r"(4u * bytes) : "memory");
 #pragma unroll
       for (int c = 0; c < 4; ++c)
         asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                      ::"r"(smem_u32(dst + c * slot_cs + (g_lo - c_lo))), "l"(src + (size_t)c * nth + g_lo), "r"(bytes),
-                     "r"(smem_u32(&bars[q & 1])) : "memory");
+                     "r"(smem_u32(&bars[q % NS])) : "memory");
     }
   };
   if (VEC) {
     if (lane == 0) {
-      mbar_init(&bars[0], 1);
-      mbar_init(&bars[1], 1);
+#pragma unroll
+      for (int q = 0; q < NS; ++q) mbar_init(&bars[q], 1);
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      // row q lands in slot q & 1; rows r0+2 and (mid-iteration r0) r0+3 are the first uses
-      if (r0 + 2 <= r1) issue_row(r0 + 2);
+      // row q lands in slot q % NS; rows r0+2 .. r0+NS go out now, row i+NS+1 in the middle of iteration i
+#pragma unroll
+      for (int q = 2; q <= NS; ++q)
+        if (r0 + q <= r1) issue_row(r0 + q);
     }
     __syncwarp();
   }
@@ -641,10 +647,10 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
     }
     if (any_src) add_source<V>(Hn, src_h, p, i, true);
     if (VEC) {
-      // B (row i+1, read from slot (i+1)&1 at the end of the last iteration) has been consumed by
-      // every lane: its slot may now receive row i+3.
+      // B (row i+1, copied out of slot (i+1) % NS at the end of the last iteration) has been consumed by
+      // every lane: its slot may now receive row i+NS+1.
       __syncwarp();
-      if (lane == 0 && i + 3 <= r1) issue_row(i + 3);
+      if (lane == 0 && i + NS + 1 <= r1) issue_row(i + NS + 1);
     }
     if (CM == 1)
       lw_stage_planes<V, false, VEC>(Hp, Hn, A, planes + (size_t)(2 * i) * loc_stride, th, tau_f, out, nth, j0);
@@ -654,8 +660,8 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
     store_row<V, VEC>(out, uout + (size_t)i * row_stride, nth, j0, pay_lo, pay_hi);
     if (VEC) {
       if (i + 2 <= r1) {
-        mbar_wait(&bars[(i + 2) & 1], (unsigned)(((i + 2) - (r0 + 2)) >> 1) & 1u);
-        lds_row<V>(A, slot0 + (size_t)((i + 2) & 1) * slot_doubles, slot_cs, lane * V, (unsigned)j0 < (unsigned)nth);
+        mbar_wait(&bars[(i + 2) % NS], (unsigned)((i - r0) / NS) & 1u);
+        lds_row<V>(A, slot0 + (size_t)((i + 2) % NS) * slot_doubles, slot_cs, lane * V, (unsigned)j0 < (unsigned)nth);
       }
     } else {
       A = ua;
@@ -1033,7 +1039,7 @@ static cudaError_t launch_v(const StepParams& p, cudaStream_t st) {
   const int warps_per_block = 4;
   dim3 grid((p.n_slabs + warps_per_block - 1) / warps_per_block, p.n_modes, p.n_seg), block(32 * warps_per_block);
   const bool vec = p.n_theta % V == 0;
-  const int dyn_max = (int)((size_t)warps_per_block * 2 * 4 * 32 * V * sizeof(double));
+  const int dyn_max = (int)((size_t)warps_per_block * TEUK_SLOTS * 4 * 32 * V * sizeof(double));
   const size_t dyn = vec ? (size_t)dyn_max : 0;
 #define TEUK_LAUNCH(VECF, CMF, SEGF)                                                                         \
   do {                                                                                                       \
