@@ -519,7 +519,11 @@ __device__ __forceinline__ void stage_rtab_chunk(double* sbuf, const double* __r
 template <int V, bool VEC, int CM, bool SEG>
 __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const __grid_constant__ StepParams p) {
   const int lane = threadIdx.x & 31;
-  const int slab = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  // warp index broadcast from lane 0: tells the compiler that everything derived from it (slab bounds, loop
+  // trip count, the early exit) is warp-uniform, so the warp stays provably converged: no BRA.DIV guards
+  // around the shuffles, uniform-datapath address arithmetic, larger basic blocks to schedule.
+  const int wib_u = __shfl_sync(FULL, (int)(threadIdx.x >> 5), 0);
+  const int slab = blockIdx.x * (blockDim.x >> 5) + wib_u;
   const int mode = blockIdx.y;
   const int nth = p.n_theta, nr = p.n_r;
   if (slab >= p.n_slabs) return;
@@ -539,7 +543,7 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
   constexpr int NS = TEUK_SLOTS;
   __shared__ __align__(8) unsigned long long s_bar[4][NS];
   extern __shared__ __align__(128) unsigned char s_dyn[];   // VEC: [warp][TEUK_SLOTS][4 n_theta] doubles
-  const int wib = threadIdx.x >> 5;
+  const int wib = wib_u;
   double* const rt_buf = &s_rt[wib][0][0];
   stage_rtab_chunk(rt_buf, rtab, 2 * r0, 2 * nr - 1, lane);
   const unsigned row_bytes = (unsigned)(row_stride * sizeof(double));
@@ -811,7 +815,8 @@ __device__ __forceinline__ void hslot_load(Row<V>& h, const double* slot, int la
 
 template <int V, bool EVEN>
 __global__ void __launch_bounds__(128, TEUK_SMEM_MIN_BLOCKS) teuk_step_smem_kernel(const __grid_constant__ StepParams p) {
-  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  const int wib = __shfl_sync(FULL, (int)(threadIdx.x >> 5), 0);   // provably warp-uniform (see teuk_step_kernel)
   const int slab = blockIdx.x * (blockDim.x >> 5) + wib;
   const int mode = blockIdx.y;
   const int nth = p.n_theta, nr = p.n_r;
