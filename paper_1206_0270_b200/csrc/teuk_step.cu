@@ -516,7 +516,9 @@ __device__ __forceinline__ void stage_rtab_chunk(double* sbuf, const double* __r
 // paper's 32000 x 304 grid).  A warp then owns a window of 32 V columns: its payload plus a
 // 4-column halo on each side, recomputed redundantly (the stencil reaches 2 columns per iteration), so no
 // exchange between warps is needed; only payload columns are stored.
-template <int V, bool VEC, int CM, bool SEG>
+// FULLW: n_theta == 32 V exactly (all five BASELINE.json configs): n_theta becomes a compile-time constant,
+// every lane is valid, and all per-lane bounds predicates fold away.
+template <int V, bool VEC, int CM, bool SEG, bool FULLW>
 __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const __grid_constant__ StepParams p) {
   const int lane = threadIdx.x & 31;
   // warp index broadcast from lane 0: tells the compiler that everything derived from it (slab bounds, loop
@@ -525,7 +527,7 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
   const int wib_u = __shfl_sync(FULL, (int)(threadIdx.x >> 5), 0);
   const int slab = blockIdx.x * (blockDim.x >> 5) + wib_u;
   const int mode = blockIdx.y;
-  const int nth = p.n_theta, nr = p.n_r;
+  const int nth = FULLW ? 32 * V : p.n_theta, nr = p.n_r;
   if (slab >= p.n_slabs) return;
   const int r0 = 1 + slab * p.slab_rows;             // first interior node of this slab
   const int r1 = min(r0 + p.slab_rows, nr - 1);      // one past the last
@@ -1046,25 +1048,30 @@ static cudaError_t launch_v(const StepParams& p, cudaStream_t st) {
   const bool vec = p.n_theta % V == 0;
   const int dyn_max = (int)((size_t)warps_per_block * TEUK_SLOTS * 4 * 32 * V * sizeof(double));
   const size_t dyn = vec ? (size_t)dyn_max : 0;
-#define TEUK_LAUNCH(VECF, CMF, SEGF)                                                                         \
+#define TEUK_LAUNCH(VECF, CMF, SEGF, FWF)                                                                        \
   do {                                                                                                       \
     static bool attr_set[64] = {false};   /* per device: function attributes belong to a context */         \
     int dev_ = 0;                                                                                            \
     cudaGetDevice(&dev_);                                                                                    \
     if (!attr_set[dev_ & 63]) {                                                                              \
-      cudaError_t e = cudaFuncSetAttribute(teuk_step_kernel<V, VECF, CMF, SEGF>,                             \
+      cudaError_t e = cudaFuncSetAttribute(teuk_step_kernel<V, VECF, CMF, SEGF, FWF>,                        \
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max);            \
       if (e != cudaSuccess) return e;                                                                        \
       attr_set[dev_ & 63] = true;                                                                            \
     }                                                                                                        \
-    teuk_step_kernel<V, VECF, CMF, SEGF><<<grid, block, dyn, st>>>(p);                                       \
+    teuk_step_kernel<V, VECF, CMF, SEGF, FWF><<<grid, block, dyn, st>>>(p);                                  \
   } while (0)
+  const bool fullw = p.n_theta == 32 * V;
   if (p.n_seg > 1) {
-    if (vec) TEUK_LAUNCH(true, 0, true); else TEUK_LAUNCH(false, 0, true);
+    if (vec) TEUK_LAUNCH(true, 0, true, false); else TEUK_LAUNCH(false, 0, true, false);
   } else if (p.coef_mode == 1) {
-    if (vec) TEUK_LAUNCH(true, 1, false); else TEUK_LAUNCH(false, 1, false);
+    if (fullw) TEUK_LAUNCH(true, 1, false, true);
+    else if (vec) TEUK_LAUNCH(true, 1, false, false);
+    else TEUK_LAUNCH(false, 1, false, false);
   } else {
-    if (vec) TEUK_LAUNCH(true, 0, false); else TEUK_LAUNCH(false, 0, false);
+    if (fullw) TEUK_LAUNCH(true, 0, false, true);
+    else if (vec) TEUK_LAUNCH(true, 0, false, false);
+    else TEUK_LAUNCH(false, 0, false, false);
   }
 #undef TEUK_LAUNCH
   return cudaGetLastError();
