@@ -461,6 +461,19 @@ __device__ __forceinline__ void tma_load_row(void* dst, const void* src, unsigne
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
+// same operations on precomputed 32-bit shared addresses (keeps the address conversion out of the hot loop)
+__device__ __forceinline__ void tma_load_row_u32(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_u32(unsigned bar, unsigned parity) {
+  unsigned ok;
+  do {
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  } while (!ok);
+}
 __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
   unsigned ok;
   do {
@@ -554,11 +567,13 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
   unsigned long long* const bars = &s_bar[wib][0];
   // One TMA bulk copy per row (whole row), or four (one per component) for a theta segment's window.
   const int g_lo = max(c_lo, 0), g_hi = min(c_lo + 32 * V, nth);
+  const unsigned slot0_u32 = smem_u32(slot0), bars_u32 = smem_u32(bars);
   auto issue_row = [&](int q) {
     double* dst = slot0 + (size_t)(q % NS) * slot_doubles;
     const double* src = uin + (size_t)q * row_stride;
     if (!SEG) {
-      tma_load_row(dst, src, row_bytes, &bars[q % NS]);
+      tma_load_row_u32(slot0_u32 + (unsigned)((q % NS) * slot_doubles * sizeof(double)), src, row_bytes,
+                       bars_u32 + 8u * (unsigned)(q % NS));
     } else {
       const unsigned bytes = (unsigned)((g_hi - g_lo) * sizeof(double));
       asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&bars[q % NS])), "r"(4u * bytes) : "memory");
@@ -605,7 +620,7 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
     for (int q = 0; q < p.n_obs; ++q) mine = mine || (p.obs[q].i0 >= r0 - 1 && p.obs[q].i0 < r1);
     do_tap = mine;
   }
-  const bool any_src = src_h.on || src_f.on;
+  const bool any_src = __any_sync(FULL, src_h.on || src_f.on);   // vote result: provably warp-uniform
   const double tau_h = 0.5 * p.dt, tau_f = 0.25 * p.dt, tdx = 2.0 / p.dx;
 
   Row<V> ua, ub, uc, hp, hn, out;
@@ -666,7 +681,7 @@ __global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const _
     store_row<V, VEC>(out, uout + (size_t)i * row_stride, nth, j0, pay_lo, pay_hi);
     if (VEC) {
       if (i + 2 <= r1) {
-        mbar_wait(&bars[(i + 2) % NS], (unsigned)((i - r0) / NS) & 1u);
+        mbar_wait_u32(bars_u32 + 8u * (unsigned)((i + 2) % NS), (unsigned)((i - r0) / NS) & 1u);
         lds_row<V>(A, slot0 + (size_t)((i + 2) % NS) * slot_doubles, slot_cs, lane * V, (unsigned)j0 < (unsigned)nth);
       }
     } else {
