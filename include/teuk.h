@@ -66,6 +66,11 @@ typedef struct {
   int32_t half_window;           /* W cells each side, 0 <= W <= 4096                              */
 } teuk_orbit;
 
+/* Make CUDA device `device` current for this library in the calling thread (cudaSetDevice inside the
+ * library's own CUDA runtime instance).  Optional: without it teuk_create uses the device whose context
+ * is current in the thread.  The Python binding calls it with torch's current device. */
+int teuk_select_device(int32_t device);
+
 /* Create a solver for Kerr parameters (a, M), |a| < M, M > 0, and n_modes (1..64) azimuthal
  * modes m[k] evolved together as independent fields ("decoupled"; one launch per
  * iteration covers all modes).  dt > 0 is the time step (the caller is responsible for stability:

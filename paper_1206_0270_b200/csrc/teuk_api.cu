@@ -291,6 +291,20 @@ void teuk_destroy(teuk_solver* s) {
   delete s;
 }
 
+int teuk_select_device(int32_t device) {
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    return fail(nullptr, TEUK_ECUDA, "teuk_select_device: no CUDA device (this library has no CPU fallback)");
+  }
+  if (device < 0 || device >= ndev) return fail(nullptr, TEUK_EINVAL, "teuk_select_device: no such device");
+  if (cudaSetDevice(device) != cudaSuccess) {
+    cudaGetLastError();
+    return fail(nullptr, TEUK_ECUDA, "teuk_select_device: cudaSetDevice failed");
+  }
+  return TEUK_OK;
+}
+
 int teuk_create(teuk_solver** out, double a, double M, const int32_t* m, int32_t n_modes,
                 const teuk_grid* grid, double dt) {
   if (!out) return fail(nullptr, TEUK_EINVAL, "teuk_create: out is NULL");

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("TEUK_LIB") or os.path.join(_HERE, "libteuk.so")  # TEUK_LIB: development override
 
 TEUK_OK, TEUK_EINVAL, TEUK_ENOMEM, TEUK_ECUDA, TEUK_ENONFINITE = 0, -1, -2, -3, -4
-SYMBOLS = ["teuk_create", "teuk_set_initial", "teuk_set_source", "teuk_step", "teuk_extract",
+SYMBOLS = ["teuk_select_device", "teuk_create", "teuk_set_initial", "teuk_set_source", "teuk_step", "teuk_extract",
            "teuk_get_state", "teuk_set_option", "teuk_get_stat", "teuk_sync", "teuk_destroy",
            "teuk_last_error"]
 
@@ -54,6 +54,7 @@ def load():
     vp = C.c_void_p
     L.teuk_create.argtypes = [C.POINTER(vp), C.c_double, C.c_double, C.POINTER(C.c_int32), C.c_int32,
                               C.POINTER(teuk_grid), C.c_double]
+    L.teuk_select_device.argtypes = [C.c_int32]
     L.teuk_set_initial.argtypes = [vp, vp, vp, vp, vp, C.c_int32]
     L.teuk_set_source.argtypes = [vp, C.POINTER(teuk_orbit)]
     L.teuk_step.argtypes = [vp, C.c_int64]
@@ -85,8 +86,17 @@ def _ptr(a):
 class Solver:
     """One teuk_solver handle.  Field arrays are [n_modes][n_r][n_theta] float64, theta fastest."""
 
-    def __init__(self, a, M, modes, rs_min, rs_max, n_r, n_theta, dt):
+    def __init__(self, a, M, modes, rs_min, rs_max, n_r, n_theta, dt, device=None):
         self._lib = load()
+        if device is None:
+            import sys
+            torch = sys.modules.get("torch")      # only if the caller already uses torch
+            if torch is not None and torch.cuda.is_available() and torch.cuda.is_initialized():
+                device = torch.cuda.current_device()
+        if device is not None:
+            rc = self._lib.teuk_select_device(int(device))
+            if rc != TEUK_OK:
+                raise TeukError(rc, self._lib.teuk_last_error(None).decode())
         self.modes = [int(m) for m in modes]
         self.shape = (len(self.modes), int(n_r), int(n_theta))
         self.dt = float(dt)
