@@ -467,19 +467,19 @@ __device__ __forceinline__ void tma_load_row_u32(unsigned dst, const void* src, 
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
+// Bounded spin: try_wait suspends the warp for a hardware time slice per attempt, so 2^22 failed attempts
+// are seconds, far beyond any HBM latency; a row that never arrives (a faulted TMA copy) then becomes a
+// reported CUDA error (trap -> sticky TEUK_ECUDA) instead of a hung GPU.
 __device__ __forceinline__ void mbar_wait_u32(unsigned bar, unsigned parity) {
-  unsigned ok;
+  unsigned ok, tries = 0;
   do {
     asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
                  : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (!ok && ++tries > (1u << 22)) asm volatile("trap;");
   } while (!ok);
 }
 __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
-  unsigned ok;
-  do {
-    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                 : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-  } while (!ok);
+  mbar_wait_u32(smem_u32(bar), parity);
 }
 
 // shared-memory row (same [comp][n_theta] layout as HBM) -> registers

@@ -327,3 +327,31 @@ def test_paper_grid_quick(orc, teuk):
     cfg = wl.CONFIGS[6].scaled(name="paper_grid_crop", n_r=2000, rs_min=-30.0, rs_max=-30.0 + 1999 * wl.CONFIGS[6].dx,
                                steps=100)
     check_pair(run_pair(orc, teuk, cfg, 100, observers=[50.0]))
+
+
+def test_seeded_fuzz_of_shapes_and_options(orc, teuk):
+    """Random (seeded) grid shapes, spins, mode sets, slab lengths, kernels and edge conditions: a few
+    iterations from random data each, against the oracle."""
+    rng = np.random.default_rng(20260270)
+    for case in range(24):
+        n_theta = int(rng.choice([5, 17, 32, 33, 48, 63, 64, 90, 127, 128, 130, 176, 257, 300]))
+        n_r = int(rng.integers(4, 160))
+        a = float(rng.choice([0.0, 0.3, 0.9, 0.998]))
+        modes = tuple(int(m) for m in rng.choice([-3, -2, -1, 0, 1, 2, 3, 4], size=int(rng.integers(1, 4)), replace=False))
+        lo = float(rng.uniform(-40.0, 5.0))
+        dx = float(rng.uniform(0.05, 0.5))
+        kernel = int(rng.integers(0, 2)) if n_theta <= 256 else 0
+        coef_mode = int(rng.integers(0, 2)) if (kernel == 0 and n_theta <= 128) else 0
+        opts = {"kernel": kernel, "slab_rows": int(rng.choice([0, 1, 2, 5, 9, 64])), "graph": int(rng.integers(0, 2)),
+                "outer_bc": int(rng.integers(0, 2))}
+        if coef_mode:
+            opts["coef_mode"] = 1
+        steps = int(rng.integers(1, 6))
+        cfg = wl.Config(100 + case, "fuzz%d" % case, a, 1.0, modes, lo, lo + dx * (n_r - 1), n_r, n_theta,
+                        0.01 / max(1, n_theta // 64), steps, (lo + 0.37 * dx * (n_r - 1),), "zero", "circular",
+                        outer_bc=opts["outer_bc"])
+        res = run_pair(orc, teuk, cfg, steps, initial=wl.random_state(cfg, case), options=opts)
+        try:
+            check_pair(res, tol=1e-11)
+        except AssertionError as e:
+            raise AssertionError("case %d: n_r=%d n_theta=%d a=%g modes=%s opts=%s: %s" % (case, n_r, n_theta, a, modes, opts, e))
