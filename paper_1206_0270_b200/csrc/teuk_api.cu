@@ -136,7 +136,7 @@ int n_segments(const teuk_solver* s) {
 int resident_warps(const teuk_solver* s) {
   const int sms = s->n_sms > 0 ? s->n_sms : 148;
   const int v = (s->n_theta + 31) / 32;
-  return sms * (s->variant == 1 ? 12 : (v <= 1 ? 16 : 8));   // measured occupancies of the kernels
+  return sms * (s->variant == 1 ? 12 : (v <= 1 ? 16 : (v == 2 ? 12 : 8)));   // occupancies of the kernels
 }
 
 int rows_for_waves(const teuk_solver* s, double waves) {
@@ -483,18 +483,26 @@ int build_graph(teuk_solver* s) {
 // iteration counter and the recorded series are untouched, and results do not depend on the slab length.
 int tune_slab_rows(teuk_solver* s) {
   const double waves[] = {0.95, 1.9, 2.0, 2.9, 3.9, 5.8};
-  int cand[16];
+  int cand[48];
   int nc = 0;
   auto add = [&](int r) {
     if (r < 1) r = 1;
     if (r > s->n_r - 2) r = s->n_r - 2;
     for (int q = 0; q < nc; ++q)
       if (cand[q] == r) return;
-    if (nc < 16) cand[nc++] = r;
+    if (nc < 48) cand[nc++] = r;
   };
-  for (double w : waves) add(rows_for_waves(s, w));
   const int base = auto_slab_rows(s);
-  if (base <= 16) { add(1); add(2); add(4); add(8); add(16); }
+  if (base <= 24) {
+    for (int r = 1; r <= 24; ++r) add(r);          // small grids: every short length (wave quantisation is coarse)
+  } else {
+    for (double w : waves) {
+      const int r = rows_for_waves(s, w);
+      add(r);
+      add(r + (r + 9) / 10);                       // and its +-10 % neighbours
+      add(r - (r + 9) / 10);
+    }
+  }
   cudaEvent_t e0, e1;
   CK(cudaEventCreate(&e0), "autotune: event");
   CK(cudaEventCreate(&e1), "autotune: event");
@@ -508,16 +516,17 @@ int tune_slab_rows(teuk_solver* s) {
     cudaError_t e = teuk_launch_step(p, s->stream);               // warm-up
     float ms = 0.f;
     int reps = 3;
-    for (int pass = 0; pass < 2 && e == cudaSuccess; ++pass) {   // short kernels: second pass with 40 launches
+    for (int pass = 0; pass < 4 && e == cudaSuccess; ++pass) {   // short kernels: time at least ~1 ms of launches
       e = cudaEventRecord(e0, s->stream);
       for (int r = 0; r < reps && e == cudaSuccess; ++r) e = teuk_launch_step(p, s->stream);
       if (e == cudaSuccess) e = cudaEventRecord(e1, s->stream);
       if (e == cudaSuccess) e = cudaEventSynchronize(e1);
       if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
       s->launches += reps;
+      const float total = ms;
       ms /= reps;
-      if (ms * reps > 0.3f) break;
-      reps = 40;
+      if (total > 1.0f) break;
+      reps *= 8;
     }
     s->launches += 1;
     if (e != cudaSuccess) {

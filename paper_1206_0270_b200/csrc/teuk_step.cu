@@ -531,8 +531,10 @@ __device__ __forceinline__ void stage_rtab_chunk(double* sbuf, const double* __r
 // exchange between warps is needed; only payload columns are stored.
 // FULLW: n_theta == 32 V exactly (all five BASELINE.json configs): n_theta becomes a compile-time constant,
 // every lane is valid, and all per-lane bounds predicates fold away.
+// Resident blocks per SM: V = 2 fits 160 registers without spills -> 3 blocks (12 warps; measured +5-9 %);
+// V = 4 needs all 255 registers -> 2 blocks; V = 1 lands at ~120 registers -> 4 blocks either way.
 template <int V, bool VEC, int CM, bool SEG, bool FULLW>
-__global__ void __launch_bounds__(128, TEUK_MIN_BLOCKS) teuk_step_kernel(const __grid_constant__ StepParams p) {
+__global__ void __launch_bounds__(128, (V == 2 ? 3 : TEUK_MIN_BLOCKS)) teuk_step_kernel(const __grid_constant__ StepParams p) {
   const int lane = threadIdx.x & 31;
   // warp index broadcast from lane 0: tells the compiler that everything derived from it (slab bounds, loop
   // trip count, the early exit) is warp-uniform, so the warp stays provably converged: no BRA.DIV guards
