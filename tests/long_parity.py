@@ -31,6 +31,8 @@ def main():
     ap.add_argument("--config", type=int, required=True)
     ap.add_argument("--steps", type=int, default=0)
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "long_parity.jsonl"))
+    ap.add_argument("--no-oracle", action="store_true", help="GPU only: report the rounding sensitivity")
+    ap.add_argument("--no-sensitivity", action="store_true")
     a = ap.parse_args()
     cfg = wl.CONFIGS[a.config]
     steps = a.steps or cfg.steps
@@ -50,6 +52,23 @@ def main():
     sg = g.get_state()
     wg = [g.extract(x) for x in cfg.observers]
     g.close()
+    # rounding sensitivity: the same CUDA path with differently rounded coefficients (streamed planes
+    # instead of per-point rebuilds); any two non-bit-identical implementations differ at least this much
+    sens = None
+    if cfg.n_theta <= 128 and not a.no_sensitivity:
+        g2 = Solver.from_config(cfg)
+        g2.set_option("coef_mode", 1)
+        g2.set_initial(*ini)
+        g2.set_source(orbit)
+        g2.step(steps)
+        s2 = g2.get_state()
+        g2.close()
+        sens = {"rel_l2_phi": rel(s2[0] + 1j * s2[1], sg[0] + 1j * sg[1]),
+                "rel_l2_pi": rel(s2[2] + 1j * s2[3], sg[2] + 1j * sg[3])}
+    if a.no_oracle:
+        print(json.dumps({"config": cfg.cid, "steps": steps, "gpu_gpts": cfg.n_pts * steps / t_gpu / 1e9,
+                          "sensitivity_coef_mode_0_vs_1": sens}))
+        return
     o = orc.OracleSolver.from_config(cfg)
     o.set_initial(*ini)
     o.set_source(orbit)
@@ -73,6 +92,7 @@ def main():
         "gpu_gpts": cfg.n_pts * steps / t_gpu / 1e9, "oracle_mpts": cfg.n_pts * steps / t_cpu / 1e6,
         "oracle_threads": int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1)),
         "oracle_seconds": t_cpu,
+        "sensitivity_coef_mode_0_vs_1": sens,
     }
     os.makedirs(os.path.dirname(a.out), exist_ok=True)
     with open(a.out, "a") as f:
