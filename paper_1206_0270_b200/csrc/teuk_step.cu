@@ -4,8 +4,9 @@
 // (PAPER.md:161).  Hand-written for sm_100a; no tensor cores (a stencil, not a contraction).
 //
 // Mapping: theta is the fastest index and one WARP spans the whole theta
-// range, each lane owning V = ceil(n_theta/32) contiguous columns, so the theta-neighbours of
-// the centred differences are register neighbours or one warp shuffle.  Each warp
+// range (n_theta <= 128; wider grids are cut into theta segments with a redundant halo, SEG), each
+// lane owning V = 1, 2 or 4 contiguous columns, so the theta-neighbours of the centred
+// differences are register neighbours or one warp shuffle.  Each warp
 // MARCHES along r* over a slab of rows, keeping u^n_i, u^n_{i+1} and the half-step values
 // u^{n+1/2}_{i-1/2} (Eq. 3) in registers: every row of u^n is read from HBM once (plus one halo
 // row per slab end) and every row of u^{n+1} is written once = 64 B per point per iteration, the
@@ -20,6 +21,12 @@
 //   full:  Phi' = Phi + (dt/4) E2(H)           Pi'  = Pi  + (dt/4) [ (2b/dx) D_Pi + Q B ](H) + dt T
 //   B = (2 beta^'/dx) D_Phi + alpha^ E2 + cL^ L'_theta S_Phi + i G1 S_Phi,
 // which uses kappa dPhi + alpha Pi = Q[(beta^ - Q s2 X3) dPhi + alpha^ (Pi - b dPhi)].
+//
+// Kernels in this file: teuk_step_kernel (register-resident marching kernel, the default; template flags
+// VEC = vector/TMA path, CM = coefficients rebuilt / streamed planes, SEG = theta segments, FULLW =
+// n_theta == 32 V compile-time), teuk_step_smem_kernel (same arithmetic, state in shared memory; bitwise
+// cross-check), teuk_flush_tap_kernel, pack/unpack and counter kernels.  The compile-time knobs below
+// record what was measured on config 5 (profiles/r1_step_kernel_full.md); the defaults are the winners.
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
@@ -36,13 +43,13 @@ struct Row {
 };
 
 #ifndef TEUK_MIN_BLOCKS
-#define TEUK_MIN_BLOCKS 2
+#define TEUK_MIN_BLOCKS 2   // resident blocks for V = 1, 4 (V = 2 always asks for 3); 3 with V = 4 spills: 29 GPts/s
 #endif
 #ifndef TEUK_FAST_RSQRT
-#define TEUK_FAST_RSQRT 1
+#define TEUK_FAST_RSQRT 1   // own MUFU.RSQ64H + one third-order step instead of CUDA's rsqrt(): +6 GPts/s
 #endif
 #ifndef TEUK_UNROLL2
-#define TEUK_UNROLL2 1
+#define TEUK_UNROLL2 1      // marching loop body instantiated twice with swapped roles (no register rotation): +3
 #endif
 #ifndef TEUK_SLOTS
 #define TEUK_SLOTS 2    // TMA landing slots per warp (register kernel): rows i+2 .. i+TEUK_SLOTS+1 in flight (3, 4: no gain)
