@@ -197,6 +197,7 @@ def main():
     ap.add_argument("--slab-rows", type=int, default=0)
     ap.add_argument("--graph", type=int, default=1)
     ap.add_argument("--coef-mode", type=int, default=0, help="0 rebuild coefficients (default), 1 stream 2D planes")
+    ap.add_argument("--temporal-block", type=int, default=0, help="0 library default, 1 or 2 iterations per HBM round trip")
     ap.add_argument("--kernel", type=int, default=-1, help="-1 library default, 0 register-resident, 1 smem-resident")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -239,6 +240,8 @@ def main():
             g.set_option("kernel", args.kernel)
         if args.coef_mode:
             g.set_option("coef_mode", args.coef_mode)
+        if args.temporal_block:
+            g.set_option("temporal_block", args.temporal_block)
         # synthetic state resident in HBM: seeded random data on all four planes (throughput does not
         # depend on values; zero data as in the config would let nothing but the source window move)
         gen = torch.Generator(device="cuda").manual_seed(wl.SEED_BASE + cfg.cid + rank)
@@ -305,7 +308,7 @@ def main():
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfg.name, "grid": [cfg.n_r, cfg.n_theta], "modes": list(cfg.modes), "a": cfg.a,
-                       "dt": cfg.dt, "source": cfg.source, "coef_mode": args.coef_mode, "slab_rows": int(slab_rows), "observers": list(cfg.observers),
+                       "dt": cfg.dt, "source": cfg.source, "coef_mode": args.coef_mode, "slab_rows": int(slab_rows), "temporal_block": args.temporal_block or "default", "observers": list(cfg.observers),
                        "state_mb": 4 * cfg.n_pts * 8 / 1e6, "parallelism": "replicas x%d" % world,
                        "l2": "inputs larger than L2 (two 537 MB state copies stream through a 126 MB L2)"
                        if 4 * cfg.n_pts * 8 > 2.5e8 else "state fits in L2: not an HBM measurement"},

@@ -118,6 +118,9 @@ int teuk_get_state(teuk_solver *s, double *phi_re, double *phi_im, double *pi_re
  *   "slab_rows"     rows of r* marched by one warp (0 = automatic: measured once at the first teuk_step,
  *                   which then waits for a few untimed-by-the-caller trial launches into scratch memory)
  *   "autotune"      1 = measure the slab length (default), 0 = use the two-wave heuristic
+ *   "temporal_block" 1 = one iteration per kernel launch (default), 2 = two iterations per HBM round trip
+ *                   (warp pairs; level n+1 stays in shared memory; same results bit for bit; needs kernel 0,
+ *                   coef_mode 0, n_theta <= 128)
  *   "graph"         1 = replay the iteration through a CUDA graph (default), 0 = plain launches
  *   "kernel"        0 = register-resident marching kernel, 1 = shared-memory-resident marching kernel
  *                   (same arithmetic, bitwise identical fields; they differ in on-chip residency;

@@ -19,6 +19,7 @@ cudaError_t teuk_launch_tables(double* rtab, double* ttab, const int* d_m, int n
 cudaError_t teuk_launch_coef2d(double* c2d, const double* rtab, const double* ttab, int n_modes, int n_r,
                                int n_theta, double dx, cudaStream_t st);
 cudaError_t teuk_launch_step(const StepParams& p, cudaStream_t st);
+cudaError_t teuk_launch_step_tb2(const StepParams& p, cudaStream_t st);
 cudaError_t teuk_launch_flush_tap(const StepParams& p, cudaStream_t st);
 cudaError_t teuk_launch_bump(long long* d_base, long long inc, cudaStream_t st);
 cudaError_t teuk_launch_set_base(long long* d_base, long long v, cudaStream_t st);
@@ -59,6 +60,8 @@ struct teuk_solver {
   // options
   int outer_bc, coef_mode, slab_rows_opt, use_graph, variant, autotune;
   int tuned_rows;        // slab length chosen by the one-time autotune (0 = not tuned yet)
+  int temporal_block;    // 1 = one iteration per launch, 2 = two (warp pairs, level n+1 stays on chip)
+  int tuned_rows2;       // autotuned slab length of the temporal-blocking kernel
   // device
   int device, n_sms;
   cudaStream_t own_stream, stream, copy_stream;
@@ -84,6 +87,7 @@ struct teuk_solver {
   ObsHost obs[TEUK_MAX_OBS];
   // graph
   cudaGraphExec_t graph_exec[2];  // one per ping-pong parity of `cur`
+  cudaGraphExec_t graph_exec_tb2[2];
   // stats / errors
   long long launches;
   int sticky;            // sticky CUDA failure
@@ -117,11 +121,16 @@ int cuda_fail(teuk_solver* s, cudaError_t e, const char* where) {
 size_t state_doubles(const teuk_solver* s) { return (size_t)s->n_modes * s->n_r * 4 * s->n_theta; }
 
 void drop_graph(teuk_solver* s) {
-  for (int q = 0; q < 2; ++q)
+  for (int q = 0; q < 2; ++q) {
     if (s->graph_exec[q]) {
       cudaGraphExecDestroy(s->graph_exec[q]);
       s->graph_exec[q] = nullptr;
     }
+    if (s->graph_exec_tb2[q]) {
+      cudaGraphExecDestroy(s->graph_exec_tb2[q]);
+      s->graph_exec_tb2[q] = nullptr;
+    }
+  }
 }
 
 // theta segments of the register kernel: one warp spans up to 128 columns; wider grids are cut into
@@ -139,18 +148,27 @@ int resident_warps(const teuk_solver* s) {
   return sms * (s->variant == 1 ? 12 : (v <= 1 ? 16 : (v == 2 ? 12 : 8)));   // occupancies of the kernels
 }
 
-int rows_for_waves(const teuk_solver* s, double waves) {
+// Temporal blocking is available for the register kernel with rebuilt coefficients, one theta segment and
+// whole vector chunks per lane (n_theta a multiple of V).
+bool tb2_possible(const teuk_solver* s) {
+  const int v = (s->n_theta + 31) / 32;
+  const int vsel = v <= 1 ? 1 : (v <= 2 ? 2 : 4);
+  return s->variant == 0 && s->coef_mode == 0 && n_segments(s) == 1 && s->n_theta % vsel == 0;
+}
+bool tb2_active(const teuk_solver* s) { return s->temporal_block == 2 && tb2_possible(s); }
+
+int rows_for_waves(const teuk_solver* s, double waves, int tb = 1) {
   const long long interior = s->n_r - 2;
-  const double target = waves * resident_warps(s);
+  const double target = waves * resident_warps(s) / tb;   // tb = 2: a slab occupies a pair of warps
   long long rows = (long long)((interior * s->n_modes * n_segments(s) + target - 1) / target);
   if (rows < 1) rows = 1;
   if (rows > interior) rows = interior;
   return (int)rows;
 }
 
-int auto_slab_rows(const teuk_solver* s) { return rows_for_waves(s, 2.0); }
+int auto_slab_rows(const teuk_solver* s, int tb = 1) { return rows_for_waves(s, 2.0, tb); }
 
-void fill_params(const teuk_solver* s, StepParams* p, int in_buf, int k, int tap_enable) {
+void fill_params(const teuk_solver* s, StepParams* p, int in_buf, int k, int tap_enable, int tb = 1) {
   memset(p, 0, sizeof(*p));
   p->uin = s->d_u[in_buf];
   p->uout = s->d_u[in_buf ^ 1];
@@ -161,7 +179,8 @@ void fill_params(const teuk_solver* s, StepParams* p, int in_buf, int k, int tap
   p->n_r = s->n_r;
   p->n_theta = s->n_theta;
   p->n_modes = s->n_modes;
-  p->slab_rows = s->slab_rows_opt > 0 ? s->slab_rows_opt : (s->tuned_rows > 0 ? s->tuned_rows : auto_slab_rows(s));
+  const int tuned = tb == 2 ? s->tuned_rows2 : s->tuned_rows;
+  p->slab_rows = s->slab_rows_opt > 0 ? s->slab_rows_opt : (tuned > 0 ? tuned : auto_slab_rows(s, tb));
   if (p->slab_rows > s->n_r - 2) p->slab_rows = s->n_r - 2;
   p->n_slabs = (s->n_r - 2 + p->slab_rows - 1) / p->slab_rows;
   p->n_seg = n_segments(s);
@@ -184,6 +203,7 @@ void fill_params(const teuk_solver* s, StepParams* p, int in_buf, int k, int tap
   p->d_base = s->d_base;
   p->k = k;
   p->tap_enable = tap_enable;
+  p->tap_enable2 = 1;
   p->n_obs = s->n_obs;
   p->ring_cap = kRingCap;
   p->nonfinite = s->d_nonfinite;
@@ -331,7 +351,7 @@ int teuk_create(teuk_solver** out, double a, double M, const int32_t* m, int32_t
   s->dx = (grid->rs_max - grid->rs_min) / (grid->n_r - 1);
   s->dth = kPi / grid->n_theta;
   for (int q = 0; q < n_modes; ++q) s->m[q] = m[q];
-  s->outer_bc = 0; s->coef_mode = 0; s->slab_rows_opt = 0; s->use_graph = 1; s->autotune = 1; s->tuned_rows = 0;
+  s->outer_bc = 0; s->coef_mode = 0; s->slab_rows_opt = 0; s->use_graph = 1; s->autotune = 1; s->tuned_rows = 0; s->temporal_block = 1; s->tuned_rows2 = 0;
   s->device = dev;
   if (cudaDeviceGetAttribute(&s->n_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) s->n_sms = 148;
   snprintf(s->err, sizeof(s->err), "no error");
@@ -452,26 +472,35 @@ int teuk_set_source(teuk_solver* s, const teuk_orbit* orbit) {
 
 namespace {
 
-// Capture kGraphBatch tapping iterations + the counter bump for the current ping-pong parity.
-int build_graph(teuk_solver* s) {
+// Capture kGraphBatch tapping iterations + the counter bump for the current ping-pong parity
+// (tb = 2: kGraphBatch / 2 temporal-blocking launches of two iterations each).
+int build_graph(teuk_solver* s, int tb) {
   cudaGraph_t graph = nullptr;
   CK(cudaStreamBeginCapture(s->own_stream, cudaStreamCaptureModeThreadLocal), "graph: begin capture");
   cudaError_t e = cudaSuccess;
   const bool sep_tap = n_segments(s) > 1 && s->n_obs > 0;   // theta segments: the tap is its own small kernel
-  for (int k = 0; k < kGraphBatch && e == cudaSuccess; ++k) {
-    StepParams p;
-    fill_params(s, &p, s->cur ^ (k & 1), k, sep_tap ? 0 : 1);
-    e = teuk_launch_step(p, s->own_stream);
-    if (sep_tap && e == cudaSuccess) {
-      fill_params(s, &p, s->cur ^ ((k + 1) & 1), k + 1, 1);
-      e = teuk_launch_flush_tap(p, s->own_stream);
+  if (tb == 2) {
+    for (int j = 0; j < kGraphBatch / 2 && e == cudaSuccess; ++j) {
+      StepParams p;
+      fill_params(s, &p, s->cur ^ (j & 1), 2 * j, 1, 2);
+      e = teuk_launch_step_tb2(p, s->own_stream);
+    }
+  } else {
+    for (int k = 0; k < kGraphBatch && e == cudaSuccess; ++k) {
+      StepParams p;
+      fill_params(s, &p, s->cur ^ (k & 1), k, sep_tap ? 0 : 1);
+      e = teuk_launch_step(p, s->own_stream);
+      if (sep_tap && e == cudaSuccess) {
+        fill_params(s, &p, s->cur ^ ((k + 1) & 1), k + 1, 1);
+        e = teuk_launch_flush_tap(p, s->own_stream);
+      }
     }
   }
   if (e == cudaSuccess) e = teuk_launch_bump(s->d_base, kGraphBatch, s->own_stream);
   cudaError_t e2 = cudaStreamEndCapture(s->own_stream, &graph);
   if (e != cudaSuccess) { if (graph) cudaGraphDestroy(graph); return cuda_fail(s, e, "graph: capture launch"); }
   CK(e2, "graph: end capture");
-  e = cudaGraphInstantiate(&s->graph_exec[s->cur], graph, 0);
+  e = cudaGraphInstantiate(tb == 2 ? &s->graph_exec_tb2[s->cur] : &s->graph_exec[s->cur], graph, 0);
   cudaGraphDestroy(graph);
   CK(e, "graph: instantiate");
   return TEUK_OK;
@@ -481,7 +510,7 @@ int build_graph(teuk_solver* s) {
 // best length depends on grid size, mode count and wave quantisation.  Candidates are timed with the real
 // kernel reading the current level and writing the idle ping-pong buffer (tap off): the state, the
 // iteration counter and the recorded series are untouched, and results do not depend on the slab length.
-int tune_slab_rows(teuk_solver* s) {
+int tune_slab_rows(teuk_solver* s, int tb) {
   const double waves[] = {0.95, 1.9, 2.0, 2.9, 3.9, 5.8};
   int cand[48];
   int nc = 0;
@@ -492,12 +521,12 @@ int tune_slab_rows(teuk_solver* s) {
       if (cand[q] == r) return;
     if (nc < 48) cand[nc++] = r;
   };
-  const int base = auto_slab_rows(s);
+  const int base = auto_slab_rows(s, tb);
   if (base <= 24) {
     for (int r = 1; r <= 24; ++r) add(r);          // small grids: every short length (wave quantisation is coarse)
   } else {
     for (double w : waves) {
-      const int r = rows_for_waves(s, w);
+      const int r = rows_for_waves(s, w, tb);
       add(r);
       add(r + (r + 9) / 10);                       // and its +-10 % neighbours
       add(r - (r + 9) / 10);
@@ -512,13 +541,15 @@ int tune_slab_rows(teuk_solver* s) {
   for (int q = 0; q < nc; ++q) {
     s->slab_rows_opt = cand[q];
     StepParams p;
-    fill_params(s, &p, s->cur, (int)(s->step - s->base_on_device), 0);
-    cudaError_t e = teuk_launch_step(p, s->stream);               // warm-up
+    fill_params(s, &p, s->cur, (int)(s->step - s->base_on_device), 0, tb);
+    p.tap_enable2 = 0;
+    auto launch = [&]() { return tb == 2 ? teuk_launch_step_tb2(p, s->stream) : teuk_launch_step(p, s->stream); };
+    cudaError_t e = launch();                                      // warm-up
     float ms = 0.f;
     int reps = 3;
     for (int pass = 0; pass < 4 && e == cudaSuccess; ++pass) {   // short kernels: time at least ~1 ms of launches
       e = cudaEventRecord(e0, s->stream);
-      for (int r = 0; r < reps && e == cudaSuccess; ++r) e = teuk_launch_step(p, s->stream);
+      for (int r = 0; r < reps && e == cudaSuccess; ++r) e = launch();
       if (e == cudaSuccess) e = cudaEventRecord(e1, s->stream);
       if (e == cudaSuccess) e = cudaEventSynchronize(e1);
       if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
@@ -538,7 +569,7 @@ int tune_slab_rows(teuk_solver* s) {
     if (ms < best) { best = ms; best_rows = cand[q]; }
   }
   s->slab_rows_opt = saved;
-  s->tuned_rows = best_rows;
+  if (tb == 2) s->tuned_rows2 = best_rows; else s->tuned_rows = best_rows;
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
   return TEUK_OK;
@@ -548,11 +579,13 @@ int tune_slab_rows(teuk_solver* s) {
 int run_chunk(teuk_solver* s, long long c) {
   long long left = c;
   int first = 1;
+  const bool tb2 = tb2_active(s);
   while (left > 0) {
     const bool graph_ok = s->use_graph && !first && left >= kGraphBatch;
     if (graph_ok) {
-      if (!s->graph_exec[s->cur]) {
-        const int rc = build_graph(s);
+      cudaGraphExec_t* ge = tb2 ? &s->graph_exec_tb2[s->cur] : &s->graph_exec[s->cur];
+      if (!*ge) {
+        const int rc = build_graph(s, tb2 ? 2 : 1);
         if (rc != TEUK_OK) return rc;
       }
       if (s->base_on_device != s->step) {
@@ -560,10 +593,10 @@ int run_chunk(teuk_solver* s, long long c) {
         s->base_on_device = s->step;
         s->launches += 1;
       }
-      CK(cudaGraphLaunch(s->graph_exec[s->cur], s->stream), "step: graph launch");
+      CK(cudaGraphLaunch(*ge, s->stream), "step: graph launch");
       s->base_on_device += kGraphBatch;
       s->step += kGraphBatch;
-      s->launches += kGraphBatch * (n_segments(s) > 1 && s->n_obs > 0 ? 2 : 1) + 1;
+      s->launches += (tb2 ? kGraphBatch / 2 : kGraphBatch * (n_segments(s) > 1 && s->n_obs > 0 ? 2 : 1)) + 1;
       left -= kGraphBatch;
       continue;
     }
@@ -572,6 +605,17 @@ int run_chunk(teuk_solver* s, long long c) {
       CK(teuk_launch_set_base(s->d_base, s->step, s->stream), "step: counter");
       s->base_on_device = s->step;
       s->launches += 1;
+    }
+    if (tb2 && left >= 2) {   // two iterations, level n+1 stays on chip
+      StepParams p;
+      fill_params(s, &p, s->cur, (int)(s->step - s->base_on_device), first ? 0 : 1, 2);
+      CK(teuk_launch_step_tb2(p, s->stream), "step: temporal-blocking launch");
+      s->launches += 1;
+      s->cur ^= 1;
+      s->step += 2;
+      left -= 2;
+      first = 0;
+      continue;
     }
     const bool sep_tap = n_segments(s) > 1 && s->n_obs > 0;
     StepParams p;
@@ -608,10 +652,17 @@ int teuk_step(teuk_solver* s, int64_t n) {
   if (n < 0) return fail(s, TEUK_EINVAL, "teuk_step: n < 0");
   if (s->has_source && 2 * (s->step + n) > s->n_samples)
     return fail(s, TEUK_EINVAL, "teuk_step: trajectory table too short for n more iterations");
-  if (n > 0 && s->autotune && s->slab_rows_opt == 0 && s->tuned_rows == 0 && (s->base_on_device <= s->step)) {
-    const int rc = tune_slab_rows(s);
-    if (rc != TEUK_OK) return rc;
-    drop_graph(s);
+  if (n > 0 && s->autotune && s->slab_rows_opt == 0 && (s->base_on_device <= s->step)) {
+    if (s->tuned_rows == 0) {
+      const int rc = tune_slab_rows(s, 1);
+      if (rc != TEUK_OK) return rc;
+      drop_graph(s);
+    }
+    if (tb2_active(s) && s->tuned_rows2 == 0) {
+      const int rc = tune_slab_rows(s, 2);
+      if (rc != TEUK_OK) return rc;
+      drop_graph(s);
+    }
   }
   long long remaining = n;
   while (remaining > 0) {
@@ -733,6 +784,7 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
     if (value != 0 && value != 1) return fail(s, TEUK_EINVAL, "coef_mode must be 0 or 1");
     if (value == 1 && s->variant != 0) return fail(s, TEUK_EINVAL, "coef_mode 1 needs kernel 0");
     if (value == 1 && n_segments(s) > 1) return fail(s, TEUK_EINVAL, "coef_mode 1 needs n_theta <= 128");
+    if (value == 1 && s->temporal_block == 2) return fail(s, TEUK_EINVAL, "coef_mode 1 needs temporal_block 1");
     if (value == 1 && !s->d_coef2d) {
       const size_t bytes = (size_t)s->n_modes * (2 * (size_t)s->n_r - 1) * 8 * s->n_theta * sizeof(double);
       CK(cudaMalloc((void**)&s->d_coef2d, bytes), "coef_mode: alloc of the 2D coefficient planes");
@@ -748,15 +800,23 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
     s->use_graph = value ? 1 : 0;
   } else if (!strcmp(key, "autotune")) {
     s->autotune = value ? 1 : 0;
+  } else if (!strcmp(key, "temporal_block")) {
+    if (value != 1 && value != 2) return fail(s, TEUK_EINVAL, "temporal_block must be 1 or 2");
+    s->temporal_block = (int)value;
+    if (value == 2 && !tb2_possible(s)) {
+      s->temporal_block = 1;
+      return fail(s, TEUK_EINVAL, "temporal_block 2 needs kernel 0, coef_mode 0, n_theta <= 128 and a multiple of its lane width (1, 2 or 4)");
+    }
   } else if (!strcmp(key, "kernel")) {
     if (value != 0 && value != 1) return fail(s, TEUK_EINVAL, "kernel must be 0 (register-resident) or 1 (shared-memory-resident)");
     if (value == 1 && s->coef_mode != 0) return fail(s, TEUK_EINVAL, "kernel 1 needs coef_mode 0");
     if (value == 1 && s->n_theta > 256) return fail(s, TEUK_EINVAL, "kernel 1 needs n_theta <= 256");
+    if (value == 1 && s->temporal_block == 2) return fail(s, TEUK_EINVAL, "kernel 1 needs temporal_block 1");
     s->variant = (int)value;
   } else {
     return fail(s, TEUK_EINVAL, "teuk_set_option: unknown key");
   }
-  if (strcmp(key, "stream") != 0) s->tuned_rows = 0;   // launch shape may change: measure again
+  if (strcmp(key, "stream") != 0) { s->tuned_rows = 0; s->tuned_rows2 = 0; }   // launch shape may change: measure again
   drop_graph(s);
   return TEUK_OK;
 }
@@ -767,7 +827,11 @@ int teuk_get_stat(const teuk_solver* s, const char* key, int64_t* value) {
   else if (!strcmp(key, "launches")) *value = s->launches;
   else if (!strcmp(key, "n_pts")) *value = (int64_t)s->n_modes * s->n_r * s->n_theta;
   else if (!strcmp(key, "state_bytes")) *value = (int64_t)(state_doubles(s) * sizeof(double));
-  else if (!strcmp(key, "slab_rows")) *value = s->slab_rows_opt > 0 ? s->slab_rows_opt : (s->tuned_rows > 0 ? s->tuned_rows : auto_slab_rows(s));
+  else if (!strcmp(key, "slab_rows")) {
+    const int tb = tb2_active(s) ? 2 : 1;
+    const int tuned = tb == 2 ? s->tuned_rows2 : s->tuned_rows;
+    *value = s->slab_rows_opt > 0 ? s->slab_rows_opt : (tuned > 0 ? tuned : auto_slab_rows(s, tb));
+  }
   else return TEUK_EINVAL;
   return TEUK_OK;
 }

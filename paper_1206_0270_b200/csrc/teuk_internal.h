@@ -72,7 +72,7 @@ struct StepParams {
   const long long* d_base;
   int k;
   // waveform tap of the input state (sample n, slot (n-1) % ring_cap)
-  int tap_enable, n_obs;
+  int tap_enable, tap_enable2, n_obs;   // tap_enable2: level n+1 inside a temporal-blocking launch
   long long ring_cap;
   int* nonfinite;
   ObsDev obs[TEUK_MAX_OBS];

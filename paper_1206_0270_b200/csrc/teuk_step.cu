@@ -999,6 +999,262 @@ __global__ void __launch_bounds__(128, TEUK_SMEM_MIN_BLOCKS) teuk_step_smem_kern
   }
 }
 
+// ================================================================================================
+// Temporal blocking, k = 2 ("temporal_block" = 2): two iterations per HBM round trip.
+// Every slab is worked on by a PAIR of warps of the same block.  The producer warp is the marching
+// kernel above for time level n -> n+1 on the slab's rows plus one halo row on each side, except that
+// it never stores to HBM: each finished row of level n+1 goes into a small shared-memory ring.  The
+// consumer warp marches over the same slab one level up (n+1 -> n+2), taking its input rows from the
+// ring instead of from TMA landing slots, and stores level n+2.  Level n+1 never touches HBM: 32 B per
+// point per iteration instead of 64.  Ring slots are handed over with a full/empty mbarrier pair per
+// slot (count 1: lane 0 arrives after __syncwarp).  Same stage arithmetic (lw_stage), same results bit
+// for bit as two k = 1 launches.
+namespace {
+
+constexpr int TB_RING = 4;
+
+template <int V>
+__device__ __forceinline__ void sts_row(const Row<V>& u, double* srow, int nth, int j0) {
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    if (j0 < nth) {
+      double* q = srow + c * nth + j0;
+      if (V == 1) {
+        q[0] = u.c[c][0];
+      } else {
+#pragma unroll
+        for (int v = 0; v < V; v += 2) *reinterpret_cast<double2*>(q + v) = make_double2(u.c[c][v], u.c[c][v + 1]);
+      }
+    }
+  }
+}
+
+__device__ __forceinline__ void mbar_arrive_u32(unsigned bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+
+struct Tb2Shared {
+  double* rt_buf;              // this warp's r-table chunk buffers
+  double* slot0;               // producer: TMA landing slots of this pair
+  double* ring;                // level n+1 rows, TB_RING slots of 4 n_theta doubles
+  unsigned tma_u32, full_u32, empty_u32;   // shared addresses of the barrier arrays of this pair
+};
+
+// ROLE 0: producer (reads level n from HBM, pushes level n+1 rows r0-1 .. r1 into the ring)
+// ROLE 1: consumer (pops them, stores level n+2 rows r0 .. r1-1, plus the grid-edge rows)
+template <int V, bool FULLW, int ROLE>
+__device__ __forceinline__ void tb2_warp(const StepParams& p, const Tb2Shared& sh, int lane, int mode, int r0, int r1) {
+  const int nth = FULLW ? 32 * V : p.n_theta, nr = p.n_r;
+  const int j0 = lane * V;
+  const bool lane_ok = j0 < nth;
+  const size_t row_stride = (size_t)4 * nth;
+  const double* __restrict__ uin = p.uin + (size_t)mode * nr * row_stride;
+  double* __restrict__ uout = p.uout + (size_t)mode * nr * row_stride;
+  const double* __restrict__ rtab = p.rtab + (size_t)mode * (2 * nr - 1) * RT_N;
+  const long long n = *p.d_base + p.k + ROLE;                 // time level this warp reads
+  const int m0 = ROLE == 0 ? max(r0 - 1, 1) : r0;             // interior nodes [m0, m1) this warp updates
+  const int m1 = ROLE == 0 ? min(r1 + 1, nr - 1) : r1;
+  constexpr int NS = TEUK_SLOTS;
+  const unsigned row_bytes = (unsigned)(row_stride * sizeof(double));
+  const unsigned slot0_u32 = smem_u32(sh.slot0);
+  auto issue_row = [&](int q) {
+    tma_load_row_u32(slot0_u32 + (unsigned)((q % NS) * row_stride * sizeof(double)), uin + (size_t)q * row_stride,
+                     row_bytes, sh.tma_u32 + 8u * (unsigned)(q % NS));
+  };
+  auto push = [&](const Row<V>& r, int q) {                   // row q of level n+1
+    const int seq = q - (r0 - 1), s = seq % TB_RING;
+    if (seq >= TB_RING) mbar_wait_u32(sh.empty_u32 + 8u * s, (unsigned)(seq / TB_RING - 1) & 1u);
+    sts_row<V>(r, sh.ring + (size_t)s * row_stride, nth, j0);
+    __syncwarp();
+    if (lane == 0) mbar_arrive_u32(sh.full_u32 + 8u * s);
+  };
+  auto pop = [&](Row<V>& r, int q) {
+    const int seq = q - (r0 - 1), s = seq % TB_RING;
+    mbar_wait_u32(sh.full_u32 + 8u * s, (unsigned)(seq / TB_RING) & 1u);
+    lds_row<V>(r, sh.ring + (size_t)s * row_stride, nth, j0, lane_ok);
+    __syncwarp();
+    if (lane == 0) mbar_arrive_u32(sh.empty_u32 + 8u * s);
+  };
+
+  stage_rtab_chunk(sh.rt_buf, rtab, 2 * m0, 2 * nr - 1, lane);
+  if (ROLE == 0) {
+    if (lane == 0) {
+#pragma unroll
+      for (int q = 2; q <= NS; ++q)
+        if (m0 + q <= m1) issue_row(m0 + q);
+    }
+    __syncwarp();
+  }
+  ThetaTab<V> th;
+  {
+    const double* tb = p.ttab + (size_t)mode * TT_N * nth;
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const bool ok = j0 + v < nth;
+      th.vals.s2[v] = ok ? tb[TT_S2 * nth + j0 + v] : 0.0;
+      th.vals.cs[v] = ok ? tb[TT_COS * nth + j0 + v] : 0.0;
+      th.vals.ap[v] = ok ? tb[TT_AP * nth + j0 + v] : 0.0;
+      th.vals.am[v] = ok ? tb[TT_AM * nth + j0 + v] : 0.0;
+      th.vals.d0[v] = ok ? tb[TT_D0 * nth + j0 + v] : 0.0;
+    }
+  }
+  StageSource<V> src_h, src_f;
+  setup_source<V>(src_h, p, mode, 2 * n, true, m0 - 1, m1 - 1, lane, 0);
+  setup_source<V>(src_f, p, mode, 2 * n + 1, false, m0, m1 - 1, lane, 0);
+  bool do_tap = (ROLE == 0 ? p.tap_enable : p.tap_enable2) && p.n_obs > 0 && n >= 1;
+  if (do_tap) {
+    bool mine = false;
+    for (int q = 0; q < p.n_obs; ++q) mine = mine || (p.obs[q].i0 >= r0 - 1 && p.obs[q].i0 < r1);
+    do_tap = mine;
+  }
+  const bool any_src = __any_sync(FULL, src_h.on || src_f.on);
+  const double tau_h = 0.5 * p.dt, tau_f = 0.25 * p.dt, tdx = 2.0 / p.dx;
+
+  Row<V> ua, ub, uc, hp, hn, out;
+  if (ROLE == 0) {
+    if (r0 - 1 == 0) {                                        // grid edge row 0 of level n+1: zeros
+#pragma unroll
+      for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int v = 0; v < V; ++v) out.c[c][v] = 0.0;
+      push(out, 0);
+    }
+    load_row<V, true>(ua, uin + (size_t)(m0 - 1) * row_stride, nth, j0);
+    load_row<V, true>(ub, uin + (size_t)m0 * row_stride, nth, j0);
+    load_row<V, true>(uc, uin + (size_t)(m0 + 1) * row_stride, nth, j0);
+  } else {
+    pop(ua, r0 - 1);
+    pop(ub, r0);
+    pop(uc, r0 + 1);
+  }
+  if (do_tap && r0 == 1) tap<V>(ua, ub, p, 0, mode, n, lane);     // both roles hold rows 0, 1 here when r0 == 1
+  lw_stage<V, true>(ua, ub, ua, rtab + (size_t)(2 * (m0 - 1) + 1) * RT_N, th, tau_h, tdx, hp);
+  add_source<V>(hp, src_h, p, m0 - 1, true);
+
+  const double* rt_cur = sh.rt_buf;
+  auto march = [&](const int i, Row<V>& A, Row<V>& B, Row<V>& Hp, Row<V>& Hn) {
+    const int o = (i - m0) & (RT_CH - 1);
+    if (o == 0) {
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+      __syncwarp();
+      const int c = (i - m0) / RT_CH;
+      rt_cur = sh.rt_buf + (c & 1) * RT_CHUNK_DOUBLES;
+      if (i + RT_CH < m1)
+        stage_rtab_chunk(sh.rt_buf + ((c + 1) & 1) * RT_CHUNK_DOUBLES, rtab, 2 * (i + RT_CH), 2 * nr - 1, lane);
+    }
+    if (do_tap && i >= r0 && i < r1) tap<V>(A, B, p, i, mode, n, lane);   // halo iterations belong to neighbours
+    lw_stage<V, true>(A, B, A, rt_cur + (2 * o + 1) * RT_N, th, tau_h, tdx, Hn);
+    if (any_src) add_source<V>(Hn, src_h, p, i, true);
+    if (ROLE == 0) {
+      __syncwarp();
+      if (lane == 0 && i + NS + 1 <= m1) issue_row(i + NS + 1);
+    }
+    lw_stage<V, false>(Hp, Hn, A, rt_cur + (2 * o) * RT_N, th, tau_f, tdx, out);
+    if (any_src) add_source<V>(out, src_f, p, i, false);
+    if (ROLE == 0) {
+      push(out, i);
+      if (i + 2 <= m1) {
+        mbar_wait_u32(sh.tma_u32 + 8u * (unsigned)((i + 2) % NS), (unsigned)((i - m0) / NS) & 1u);
+        lds_row<V>(A, sh.slot0 + (size_t)((i + 2) % NS) * row_stride, nth, j0, lane_ok);
+      }
+    } else {
+      store_row<V, true>(out, uout + (size_t)i * row_stride, nth, j0, 0, nth);
+      if (i + 2 <= m1) pop(A, i + 2);
+    }
+  };
+  bool tail = false;
+  {
+    int i = m0;
+    for (; i + 1 < m1; i += 2) {
+      march(i, ub, uc, hp, hn);
+      march(i + 1, uc, ub, hn, hp);
+    }
+    if (i < m1) {
+      march(i, ub, uc, hp, hn);
+      tail = true;
+    }
+  }
+  // After the loop the last call's (A, B) hold input rows m1-1 and m1: (ub, uc) if the tail ran, else (uc, ub).
+
+  if (ROLE == 1 && r0 == 1) {
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+      for (int v = 0; v < V; ++v) out.c[c][v] = 0.0;
+    store_row<V, true>(out, uout, nth, j0, 0, nth);
+  }
+  if (r1 == nr - 1) {                                         // outer grid edge at this warp's output level
+    if (ROLE == 0) {
+      load_row<V, true>(ub, uin + (size_t)(nr - 1) * row_stride, nth, j0);
+      load_row<V, true>(ua, uin + (size_t)(nr - 2) * row_stride, nth, j0);
+    } else if (tail) {
+      ua = ub;                                                // row nr-2 of level n+1
+      ub = uc;                                                // row nr-1
+    } else {
+      ua = uc;
+    }
+    const double eps = __ldg(rtab + (size_t)(2 * (nr - 1)) * RT_N + RT_EPS);
+    ThetaVals<V> tv;
+    th.get(tv);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      if (p.outer_bc == 0) {
+        const double b = rsqrt_near_one(fma(-eps, tv.s2[v], 1.0));
+        out.c[0][v] = ub.c[0][v] - p.dt * b * (ub.c[0][v] - ua.c[0][v]) / p.dx;
+        out.c[1][v] = ub.c[1][v] - p.dt * b * (ub.c[1][v] - ua.c[1][v]) / p.dx;
+      } else {
+        out.c[0][v] = 0.0;
+        out.c[1][v] = 0.0;
+      }
+      out.c[2][v] = 0.0;
+      out.c[3][v] = 0.0;
+    }
+    if (ROLE == 0) push(out, nr - 1);
+    else store_row<V, true>(out, uout + (size_t)(nr - 1) * row_stride, nth, j0, 0, nth);
+  }
+}
+
+}  // namespace
+
+template <int V, bool FULLW>
+__global__ void __launch_bounds__(128, (V == 2 ? 3 : TEUK_MIN_BLOCKS)) teuk_step_tb2_kernel(const __grid_constant__ StepParams p) {
+  const int lane = threadIdx.x & 31;
+  const int wib = __shfl_sync(FULL, (int)(threadIdx.x >> 5), 0);   // provably warp-uniform
+  const int pair = wib >> 1, role = wib & 1;
+  const int slab = blockIdx.x * 2 + pair;
+  const int mode = blockIdx.y;
+  const int nth = FULLW ? 32 * V : p.n_theta;
+  constexpr int NS = TEUK_SLOTS;
+  __shared__ __align__(16) double s_rt[4][2][RT_CHUNK_DOUBLES];
+  __shared__ __align__(8) unsigned long long s_tma[2][NS], s_full[2][TB_RING], s_empty[2][TB_RING];
+  extern __shared__ __align__(128) unsigned char s_dyn[];   // [pair][NS landing slots + TB_RING ring slots][4 n_theta]
+  if (role == 0 && lane == 0) {
+#pragma unroll
+    for (int q = 0; q < NS; ++q) mbar_init(&s_tma[pair][q], 1);
+#pragma unroll
+    for (int q = 0; q < TB_RING; ++q) {
+      mbar_init(&s_full[pair][q], 1);
+      mbar_init(&s_empty[pair][q], 1);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();                                          // barriers are initialised for both warps of a pair
+  if (slab >= p.n_slabs) return;                            // both warps of the pair leave together
+  const int r0 = 1 + slab * p.slab_rows;
+  const int r1 = min(r0 + p.slab_rows, p.n_r - 1);
+  const size_t row_doubles = (size_t)4 * nth;
+  Tb2Shared sh;
+  sh.rt_buf = &s_rt[wib][0][0];
+  sh.slot0 = reinterpret_cast<double*>(s_dyn) + (size_t)pair * (NS + TB_RING) * row_doubles;
+  sh.ring = sh.slot0 + (size_t)NS * row_doubles;
+  sh.tma_u32 = smem_u32(&s_tma[pair][0]);
+  sh.full_u32 = smem_u32(&s_full[pair][0]);
+  sh.empty_u32 = smem_u32(&s_empty[pair][0]);
+  if (role == 0) tb2_warp<V, FULLW, 0>(p, sh, lane, mode, r0, r1);
+  else tb2_warp<V, FULLW, 1>(p, sh, lane, mode, r0, r1);
+}
+
 // Tap of the CURRENT state at the end of a teuk_step call (the in-kernel tap records the input
 // level of each iteration, so the last level needs one tiny launch).  One warp per (mode, observer).
 __global__ void teuk_flush_tap_kernel(const __grid_constant__ StepParams p) {
@@ -1142,6 +1398,41 @@ cudaError_t teuk_launch_step(const StepParams& p, cudaStream_t st) {
   if (v <= 1) return launch_v<1>(p, st);
   if (v <= 2) return launch_v<2>(p, st);
   return launch_v<4>(p, st);   // n_theta > 128: theta segments of <= 120 payload columns (p.n_seg > 1)
+}
+
+template <int V>
+static cudaError_t launch_tb2_v(const StepParams& p, cudaStream_t st) {
+  dim3 grid((p.n_slabs + 1) / 2, p.n_modes), block(128);
+  const size_t dyn = (size_t)2 * (TEUK_SLOTS + TB_RING) * 4 * p.n_theta * sizeof(double);
+  const int dyn_max = (int)((size_t)2 * (TEUK_SLOTS + TB_RING) * 4 * 32 * V * sizeof(double));
+  int dev_ = 0;
+  cudaGetDevice(&dev_);
+  if (p.n_theta == 32 * V) {
+    static bool attr_set[64] = {false};
+    if (!attr_set[dev_ & 63]) {
+      cudaError_t e = cudaFuncSetAttribute(teuk_step_tb2_kernel<V, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max);
+      if (e != cudaSuccess) return e;
+      attr_set[dev_ & 63] = true;
+    }
+    teuk_step_tb2_kernel<V, true><<<grid, block, dyn, st>>>(p);
+  } else {
+    static bool attr_set[64] = {false};
+    if (!attr_set[dev_ & 63]) {
+      cudaError_t e = cudaFuncSetAttribute(teuk_step_tb2_kernel<V, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max);
+      if (e != cudaSuccess) return e;
+      attr_set[dev_ & 63] = true;
+    }
+    teuk_step_tb2_kernel<V, false><<<grid, block, dyn, st>>>(p);
+  }
+  return cudaGetLastError();
+}
+
+// Two iterations per launch (temporal blocking); needs n_theta % V == 0, one theta segment, coef_mode 0.
+cudaError_t teuk_launch_step_tb2(const StepParams& p, cudaStream_t st) {
+  const int v = (p.n_theta + 31) / 32;
+  if (v <= 1) return launch_tb2_v<1>(p, st);
+  if (v <= 2) return launch_tb2_v<2>(p, st);
+  return launch_tb2_v<4>(p, st);
 }
 
 cudaError_t teuk_launch_flush_tap(const StepParams& p, cudaStream_t st) {

@@ -355,3 +355,38 @@ def test_seeded_fuzz_of_shapes_and_options(orc, teuk):
             check_pair(res, tol=1e-11)
         except AssertionError as e:
             raise AssertionError("case %d: n_r=%d n_theta=%d a=%g modes=%s opts=%s: %s" % (case, n_r, n_theta, a, modes, opts, e))
+
+
+@pytest.mark.parametrize("n_r,n_theta", [(4, 8), (5, 32), (7, 64), (37, 128), (150, 64), (333, 128), (200, 100), (64, 20)])
+def test_temporal_blocking_is_bitwise_identical(orc, teuk, n_r, n_theta):
+    """temporal_block = 2 (warp pairs, level n+1 kept in shared memory) must reproduce temporal_block = 1
+    bit for bit: fields and waveforms, odd and even iteration counts, any chunking, graphs on and off."""
+    cfg = SMALL[3].scaled(name="tb%dx%d" % (n_r, n_theta), n_r=n_r, n_theta=n_theta, rs_min=-5.0, rs_max=-5.0 + 0.4 * (n_r - 1),
+                          dt_over_dx=0.004, steps=80, modes=(2, -1), observers=(-5.0, -5.0 + 0.4 * (n_r - 1) - 0.01))
+    W = wl.observer_weights(cfg)
+    out = []
+    for tb, graph, chunks, slab in ((1, 1, [77], 0), (2, 1, [77], 0), (2, 0, [1, 2, 3, 40, 31], 3), (2, 1, [5, 72], 1)):
+        g = teuk.Solver.from_config(cfg)
+        g.set_option("temporal_block", tb)
+        g.set_option("graph", graph)
+        if slab:
+            g.set_option("slab_rows", slab)
+        g.set_initial(*wl.random_state(cfg, 21))
+        g.set_source(wl.orbit_table(cfg, n_steps=80))
+        for x in cfg.observers:
+            g.add_observer(x, W)
+        for c in chunks:
+            g.step(c)
+        out.append((g.get_state(), [g.extract(x) for x in cfg.observers]))
+        g.close()
+    for k in (1, 2, 3):
+        for a, b in zip(out[0][0], out[k][0]):
+            assert np.array_equal(a, b), k
+        for (t0, w0), (t1, w1) in zip(out[0][1], out[k][1]):
+            assert len(t1) == 77 and np.array_equal(t0, t1) and np.array_equal(w0, w1), k
+
+
+def test_temporal_blocking_parity_with_oracle(orc, teuk):
+    for cfg in (SMALL[3], SMALL[4], SMALL[5]):
+        res = run_pair(orc, teuk, cfg, min(cfg.steps, 151), options={"temporal_block": 2})
+        check_pair(res)
