@@ -1011,7 +1011,10 @@ __global__ void __launch_bounds__(128, TEUK_SMEM_MIN_BLOCKS) teuk_step_smem_kern
 // for bit as two k = 1 launches.
 namespace {
 
-constexpr int TB_RING = 4;
+#ifndef TEUK_TB_RING
+#define TEUK_TB_RING 4
+#endif
+constexpr int TB_RING = TEUK_TB_RING;
 
 template <int V>
 __device__ __forceinline__ void sts_row(const Row<V>& u, double* srow, int nth, int j0) {
