@@ -172,9 +172,10 @@ def _pulse_run(orc, n_r, n_theta, a, m, cfl, T, shape, x_obs=50.0, rs=(-50.0, 15
     o = orc.OracleSolver(a, 1.0, [m], rs[0], rs[1], n_r, n_theta, dt)
     x = rs[0] + dx * np.arange(n_r)
     th = (np.arange(n_theta) + 0.5) * math.pi / n_theta
-    ang = {"sin2": np.sin(th) ** 2, "y22": (1 + np.cos(th)) ** 2, "y21": np.sin(th) * (1 + np.cos(th))}[shape]
+    ang = {"sin2": np.sin(th) ** 2, "y22": (1 + np.cos(th)) ** 2, "y21": np.sin(th) * (1 + np.cos(th)),
+           "y20": np.sin(th) ** 2}[shape]
     o.set_initial(np.ascontiguousarray((np.exp(-(x - 20.0) ** 2 / 4.0)[:, None] * ang[None, :])[None]))
-    harm = (1 + np.cos(th)) ** 2 if m % 2 == 0 else np.sin(th) * (1 + np.cos(th))
+    harm = {0: np.sin(th) ** 2, 1: np.sin(th) * (1 + np.cos(th)), 2: (1 + np.cos(th)) ** 2}[abs(m)]
     o.add_observer(x_obs, harm * np.sin(th) * math.pi / n_theta)
     o.step(int(round(T / dt)))
     t, w = o.waveform()
@@ -214,7 +215,7 @@ def test_p2_second_order_convergence(orc):
 
 
 # ------------------------------------------------------------------------------------------ P3
-@pytest.mark.parametrize("m,shape", [(2, "y22"), (1, "y21"), (2, "sin2")])
+@pytest.mark.parametrize("m,shape", [(2, "y22"), (1, "y21"), (2, "sin2"), (0, "y20")])
 def test_p3_schwarzschild_qnm(orc, m, shape):
     """Ringdown frequency M omega = 0.3737 - 0.0890i, independent of m for a = 0."""
     t, w = _pulse_run(orc, 1025, 32, 0.0, m, 0.08, 170.0, shape)
