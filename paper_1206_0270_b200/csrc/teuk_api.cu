@@ -523,7 +523,8 @@ int tune_slab_rows(teuk_solver* s, int tb) {
   };
   const int base = auto_slab_rows(s, tb);
   if (base <= 24) {
-    for (int r = 1; r <= 24; ++r) add(r);          // small grids: every short length (wave quantisation is coarse)
+    const int small[] = {1, 2, 3, 4, 5, 6, 7, 8, 10, 12, 14, 16, 20, 24};   // small grids: wave quantisation is coarse
+    for (int r : small) add(r);
   } else {
     for (double w : waves) {
       const int r = rows_for_waves(s, w, tb);
@@ -547,7 +548,7 @@ int tune_slab_rows(teuk_solver* s, int tb) {
     cudaError_t e = launch();                                      // warm-up
     float ms = 0.f;
     int reps = 3;
-    for (int pass = 0; pass < 4 && e == cudaSuccess; ++pass) {   // short kernels: time at least ~1 ms of launches
+    for (int pass = 0; pass < 3 && e == cudaSuccess; ++pass) {   // short kernels: time at least ~0.3 ms of launches
       e = cudaEventRecord(e0, s->stream);
       for (int r = 0; r < reps && e == cudaSuccess; ++r) e = launch();
       if (e == cudaSuccess) e = cudaEventRecord(e1, s->stream);
@@ -556,7 +557,7 @@ int tune_slab_rows(teuk_solver* s, int tb) {
       s->launches += reps;
       const float total = ms;
       ms /= reps;
-      if (total > 1.0f) break;
+      if (total > 0.3f) break;
       reps *= 8;
     }
     s->launches += 1;
