@@ -70,6 +70,10 @@ def lib():
         L.orc_get_waveform.restype = C.c_int64
         L.orc_source_field.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int32, _dp, _dp]
         L.orc_source_field.restype = None
+        L.orc_set_source_kind.argtypes = [C.c_void_p, C.c_int32]
+        L.orc_set_source_kind.restype = None
+        L.orc_delta.argtypes = [C.c_int32, C.c_double, C.c_double]
+        L.orc_delta.restype = C.c_double
         _lib = L
     return _lib
 
@@ -91,6 +95,11 @@ def coefficients(M, a, m, x, theta):
 
 def gauss(y, sigma):
     return lib().orc_gauss(y, sigma)
+
+
+def delta(kind, y, h):
+    """Discrete delta of kind 1 (two-point) or 2 (four-point) at offset y = x_i - x_p, grid spacing h."""
+    return lib().orc_delta(int(kind), float(y), float(h))
 
 
 class OracleSolver:
@@ -142,6 +151,12 @@ class OracleSolver:
         ai = self._arr(orbit["amp_im"], (len(self.modes), ns))
         lib().orc_set_source(self._h, ns, _p(xs), _p(th), _p(ar), _p(ai), float(orbit["sigma_r"]),
                              float(orbit["sigma_theta"]), int(orbit["half_window"]))
+
+    def set_source_kind(self, kind):
+        """0 Gaussian (default), 1 two-point, 2 four-point discrete delta."""
+        if kind not in (0, 1, 2):
+            raise ValueError("source kind must be 0, 1 or 2")
+        lib().orc_set_source_kind(self._h, int(kind))
 
     def add_observer(self, rs_obs, weights=None):
         w = self._arr(weights, (self.shape[2],))

@@ -21,7 +21,9 @@
 // tests/test_oracle_pins.py against a computer-algebra substitution into Eq. (1) (pin P1),
 // by second-order self-convergence (P2), by the Schwarzschild and Kerr l=m=2 quasinormal
 // frequencies (P3, P3b), by the (m, theta) reflection invariant (P4), a = 0 realness (P5),
-// linearity (P6), the unit norm of the deposit (P7) and the edge rows' closed forms (P8).  The paper prints no field values:
+// linearity (P6), the unit norm of the deposit (P7), the edge rows' closed forms (P8) and, for the
+// discrete-delta deposits, the paper's step-function construction in exact rationals and the moment /
+// interpolation conditions (P9).  The paper prints no field values:
 // beyond those pins the numbers this file produces are "parity unpinned" by the paper.
 //
 // Readings of silent/ambiguous passages are the A1-A12 of SURVEY.md 8(c), restated in DESIGN.md.
@@ -132,6 +134,28 @@ double gauss(double y, double sigma) {
   return std::exp(-y * y / (2.0 * sigma * sigma)) / (sigma * std::sqrt(2.0 * PI));
 }
 
+// Discrete delta ("define a step function on a discrete numerical grid and then apply the
+// finite-difference derivative operation on the discrete step-function").  On a grid of spacing h with the
+// particle at x_p = x_k + gamma h, 0 <= gamma < 1, the discrete step is H_{i+1/2} = 0 (i < k), 1 - gamma
+// (i = k), 1 (i > k) -- the cell averages of the step, i.e. the first difference of the sampled ramp
+// max(x - x_p, 0) -- and its difference (H_{i+1/2} - H_{i-1/2})/h is (1 - gamma)/h at x_k, gamma/h at x_{k+1},
+// 0 elsewhere: the hat function below evaluated at y = x_i - x_p.  (reading A13.)
+double delta_linear(double y, double h) {
+  const double s = std::fabs(y) / h;
+  return (s < 1.0) ? (1.0 - s) / h : 0.0;
+}
+
+// "Refined version" (details in its refs [3, 4], not in the container; reading A13): the
+// four-point delta whose weights are the cubic Lagrange interpolation weights at x_p divided by h, so that
+// sum_i d_i f(x_i) h = f(x_p) for every cubic f.  As a function of y = x_i - x_p, s = |y|/h:
+//   s < 1 : (1 - s)(1 + s)(2 - s)/2 ;   1 <= s < 2 : (1 - s)(2 - s)(3 - s)/6 ;   else 0.
+double delta_cubic(double y, double h) {
+  const double s = std::fabs(y) / h;
+  if (s < 1.0) return (1.0 - s) * (1.0 + s) * (2.0 - s) / 2.0 / h;
+  if (s < 2.0) return (1.0 - s) * (2.0 - s) * (3.0 - s) / 6.0 / h;
+  return 0.0;
+}
+
 }  // namespace
 
 namespace {
@@ -165,6 +189,7 @@ struct Oracle {
   std::vector<cplx> amp;                     // [mode][n_samples]
   double sigma_r, sigma_th;
   int W;
+  int source_kind;                           // 0 Gaussian (C.6), 1 two-point, 2 four-point discrete delta (f3)
   std::vector<Observer> obs;
 
   Oracle(double a, double M) : kerr(M, a) {}
@@ -188,10 +213,14 @@ inline cplx source_term(const Oracle& o, int k, int64_t ks, bool half, int i, in
   const double v = (xp - o.x_min) / o.dx;
   const int ip = half ? (int)std::floor(v - 0.5 + 0.5) : (int)std::floor(v + 0.5);
   const int jp = (int)std::floor(thp / o.dth - 0.5 + 0.5);
-  if (std::abs(i - ip) > o.W || std::abs(j - jp) > o.W) return cplx(0.0, 0.0);
+  // discrete deltas: the window is their support (nearest point +-1 or +-2), widths are the grid spacings
+  const int W = (o.source_kind == 0) ? o.W : o.source_kind;
+  if (std::abs(i - ip) > W || std::abs(j - jp) > W) return cplx(0.0, 0.0);
   const double xx = half ? o.xh[i] : o.x[i];
-  return o.amp[(size_t)k * o.n_samples + ks] * gauss(xx - xp, o.sigma_r) *
-         gauss(o.theta[j] - thp, o.sigma_th);
+  const cplx A = o.amp[(size_t)k * o.n_samples + ks];
+  if (o.source_kind == 1) return A * delta_linear(xx - xp, o.dx) * delta_linear(o.theta[j] - thp, o.dth);
+  if (o.source_kind == 2) return A * delta_cubic(xx - xp, o.dx) * delta_cubic(o.theta[j] - thp, o.dth);
+  return A * gauss(xx - xp, o.sigma_r) * gauss(o.theta[j] - thp, o.sigma_th);
 }
 
 // One iteration (C.5): half step Eq. (3), full step Eq. (4), radial edges, then the tap (C.7).
@@ -299,6 +328,7 @@ void orc_coefficients(double M, double a, int m, double x, double theta, double*
 }
 
 double orc_gauss(double y, double sigma) { return gauss(y, sigma); }
+double orc_delta(int32_t kind, double y, double h) { return kind == 2 ? delta_cubic(y, h) : delta_linear(y, h); }
 
 void* orc_create(double a, double M, const int32_t* m, int32_t n_modes, double rs_min, double rs_max,
                  int32_t n_r, int32_t n_theta, double dt, int32_t outer_bc) {
@@ -312,7 +342,7 @@ void* orc_create(double a, double M, const int32_t* m, int32_t n_modes, double r
   o->dth = PI / n_theta;
   o->dt = dt;
   o->step = 0;
-  o->has_source = false; o->n_samples = 0; o->W = 0; o->sigma_r = o->sigma_th = 1.0;
+  o->has_source = false; o->n_samples = 0; o->W = 0; o->sigma_r = o->sigma_th = 1.0; o->source_kind = 0;
   o->x.resize(n_r); o->xh.resize(n_r - 1); o->theta.resize(n_theta);
   for (int i = 0; i < n_r; ++i) o->x[i] = rs_min + i * o->dx;
   for (int i = 0; i < n_r - 1; ++i) o->xh[i] = o->x[i] + 0.5 * o->dx;
@@ -374,6 +404,9 @@ void orc_set_source(void* h, int64_t n_samples, const double* rs_p, const double
   for (size_t q = 0; q < o->amp.size(); ++q) o->amp[q] = cplx(amp_re[q], amp_im[q]);
   o->sigma_r = sigma_r; o->sigma_th = sigma_theta; o->W = half_window;
 }
+
+// 0 = Gaussian of C.6 (default), 1 = two-point, 2 = four-point discrete delta (f3).
+void orc_set_source_kind(void* h, int32_t kind) { ((Oracle*)h)->source_kind = kind; }
 
 // Returns the observer index, or -1 if x_obs is outside [x_0, x_{n_r-1}).  weights NULL = all ones.
 int32_t orc_add_observer(void* h, double rs_obs, const double* weights) {

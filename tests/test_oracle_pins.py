@@ -10,7 +10,10 @@ The paper prints no field values, so the oracle is pinned 
   P4  (m, theta) -> (-m, pi - theta) reflection with complex conjugation;
   P5  a = 0 keeps real data exactly real;
   P6  linearity / exact power-of-two scaling / zero stays zero;
-  P7  unit norm, support and time-level placement of the Gaussian deposit.
+  P7  unit norm, support and time-level placement of the Gaussian deposit (PAPER.md:114);
+  P8  closed forms of the radial edge rows, domain of dependence;
+  P9  discrete-delta deposits: the step-function construction in exact rationals, moment
+      conditions with their known remainders, cubic interpolation, mass / centre / support of the 2D deposit.
 """
 import math
 import os
@@ -379,3 +382,98 @@ def test_p8_outer_edge_branches_and_domain_of_dependence(orc):
     for q in (0, 1):                                                           # a = 0: b = 1 exactly
         exp = ini[q][:, -1] - cfg.dt * 1.0 * (ini[q][:, -1] - ini[q][:, -2]) / cfg.dx
         assert np.allclose(f0[q][:, -1], exp, rtol=1e-14, atol=1e-15)
+
+
+# ------------------------------------------------------------------------------------------ P9
+def test_p9_discrete_delta_is_the_difference_of_a_discrete_step(orc):
+    """PAPER.md:114: "define a step function on a discrete grid and apply the finite-difference derivative".
+    Done literally in exact rational arithmetic: ramp -> (first difference) discrete step -> (difference)
+    discrete delta; the oracle's closed form must reproduce it."""
+    from fractions import Fraction as Fr
+    h = Fr(1, 8)
+    for xp in (Fr(37, 64), Fr(5, 8), Fr(-3, 16) + Fr(1, 1024), Fr(99, 128)):
+        xs = [Fr(i) * h for i in range(-12, 13)]
+        ramp = [max(x - xp, Fr(0)) for x in xs]
+        step = [(ramp[i + 1] - ramp[i]) / h for i in range(len(xs) - 1)]            # H_{i+1/2}
+        assert all(0 <= v <= 1 for v in step) and step[0] == 0 and step[-1] == 1
+        assert sum(1 for v in step if 0 < v < 1) <= 1                                # one partial cell
+        delta = [(step[i] - step[i - 1]) / h for i in range(1, len(step))]           # at xs[1:-1]
+        for x, d in zip(xs[1:-1], delta):
+            got = orc.delta(1, float(x - xp), float(h))
+            assert got == float(d), (xp, x, got, d)                                  # dyadic inputs: exact
+        assert sum(delta) * h == 1
+        assert sum(d * x for d, x in zip(delta, xs[1:-1])) * h == xp
+
+
+@pytest.mark.parametrize("kind,order", [(1, 1), (2, 3)])
+def test_p9_discrete_delta_moments(orc, kind, order):
+    """sum_i d_i (x_i - x_p)^k h = delta_{k0} up to the order of the rule; the next moment is the known
+    non-zero remainder (so a wrong support, sign or a dropped factor fails)."""
+    rng = np.random.default_rng(909 + kind)
+    for _ in range(20):
+        h = rng.uniform(0.01, 2.0)
+        xp = rng.uniform(-3.0, 3.0)
+        k0 = math.floor(xp / h)
+        g = xp / h - k0
+        xs = (k0 + np.arange(-4, 6)) * h
+        d = np.array([orc.delta(kind, x - xp, h) for x in xs])
+        assert np.count_nonzero(d) <= 2 * kind
+        for k in range(order + 1):
+            mom = np.sum(d * (xs - xp) ** k) * h
+            assert abs(mom - (1.0 if k == 0 else 0.0)) < 1e-12 * max(1.0, h ** k), (kind, k, mom)
+        nxt = np.sum(d * (xs - xp) ** (order + 1)) * h
+        if kind == 1:
+            exp = g * (1 - g) * h * h                                 # linear interpolation remainder
+        else:
+            exp = -(g + 1) * g * (g - 1) * (g - 2) * h ** 4          # cubic Lagrange remainder of y^4
+        assert abs(nxt - exp) < 1e-11 * max(1.0, h ** 4), (kind, nxt, exp)
+
+
+def test_p9_four_point_delta_is_cubic_interpolation(orc):
+    rng = np.random.default_rng(9092)
+    h = 0.37
+    for _ in range(10):
+        xp = rng.uniform(-1, 1)
+        k0 = math.floor(xp / h)
+        xs = (k0 + np.arange(-1, 3)) * h                              # the four nodes around x_p
+        f = rng.normal(size=4)
+        lagr = np.polyval(np.polyfit(xs, f, 3), xp)                   # library cubic through the nodes
+        got = sum(orc.delta(2, x - xp, h) * fv for x, fv in zip(xs, f)) * h
+        assert abs(got - lagr) < 1e-11
+
+
+@pytest.mark.parametrize("kind", [1, 2])
+def test_p9_discrete_delta_deposit(orc, kind):
+    """The 2D deposit: mass A', centred on the particle, support 2x2 / 4x4 points, on both stage grids."""
+    cfg = wl.small_test_configs()[3].scaled(n_r=401)
+    orb = wl.orbit_table(cfg, n_steps=4)
+    orb["amp_re"] = np.full_like(orb["amp_re"], 1.5)
+    orb["amp_im"] = np.full_like(orb["amp_im"], -0.5)
+    o = orc.OracleSolver.from_config(cfg)
+    o.set_source(orb)
+    o.set_source_kind(kind)
+    x, th = wl.grid_axes(cfg)
+    for half in (False, True):
+        for ks in (0, 3):
+            T = o.source_field(0, ks, half)
+            xs = (x[:-1] + 0.5 * cfg.dx) if half else x
+            w = cfg.dx * cfg.dtheta
+            assert abs(T.sum() * w - (1.5 - 0.5j)) < 1e-12
+            assert abs((T.real * xs[:, None]).sum() * w / 1.5 - orb["rs_p"][ks]) < 1e-11
+            assert abs((T.real * th[None, :]).sum() * w / 1.5 - orb["theta_p"][ks]) < 1e-12
+            nz = np.argwhere(T != 0.0)
+            assert nz[:, 0].max() - nz[:, 0].min() <= 2 * kind - 1
+            assert nz[:, 1].max() - nz[:, 1].min() <= 2 * kind - 1
+    # evolution: the deposit enters Pi exactly as the Gaussian does (same time levels, P7)
+    ob = dict(orb)
+    ob["amp_re"] = np.zeros_like(orb["amp_re"]); ob["amp_im"] = np.zeros_like(orb["amp_im"])
+    ob["amp_re"][:, 0] = 1.0
+    o2 = orc.OracleSolver.from_config(cfg)
+    o2.set_source(ob)
+    o2.set_source_kind(kind)
+    o2.step(1)
+    o.set_source(ob)
+    Th = o.source_field(0, 0, True)
+    hs = o2.get_half()
+    assert np.allclose(hs[2][0], 0.5 * cfg.dt * Th.real, rtol=1e-14, atol=0)
+    assert np.count_nonzero(hs[2][0]) == np.count_nonzero(Th.real) > 0
