@@ -123,7 +123,7 @@ def oracle_sample_config(cfg, rows):
                       dt_over_dx=cfg.dt_over_dx, observers=(obs,))
 
 
-def time_oracle(cfg, steps, warmup, rows):
+def time_oracle(cfg, steps, warmup, rows, source_kind=0):
     """The oracle as it stands on the host cores; returns (GPts/s, threads, sample description)."""
     from oracle import oracle as orc
     c = oracle_sample_config(cfg, rows)
@@ -133,6 +133,7 @@ def time_oracle(cfg, steps, warmup, rows):
     if orbit is not None:
         # keep the full config's trajectory rate: T refers to cfg.steps * cfg.dt (c.dt == cfg.dt)
         o.set_source(orbit)
+        o.set_source_kind(source_kind)
     o.add_observer(c.observers[0], wl.observer_weights(c))
     o.step(warmup)
     t0 = time.perf_counter()
@@ -169,7 +170,7 @@ def run_reference(args, cfg, rank, world):
     if rank != 0:
         return
     rows = args.oracle_rows
-    val, dt, threads, sample = time_oracle(cfg, args.steps, args.warmup, rows)
+    val, dt, threads, sample = time_oracle(cfg, args.steps, args.warmup, rows, args.source_kind)
     c = oracle_sample_config(cfg, rows)
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
@@ -197,6 +198,7 @@ def main():
     ap.add_argument("--slab-rows", type=int, default=0)
     ap.add_argument("--graph", type=int, default=1)
     ap.add_argument("--coef-mode", type=int, default=0, help="0 rebuild coefficients (default), 1 stream 2D planes")
+    ap.add_argument("--source-kind", type=int, default=0, help="0 Gaussian deposit (the configs'), 1 / 2 discrete delta")
     ap.add_argument("--temporal-block", type=int, default=0, help="0 library default, 1 or 2 iterations per HBM round trip")
     ap.add_argument("--kernel", type=int, default=-1, help="-1 library default, 0 register-resident, 1 smem-resident")
     args = ap.parse_args()
@@ -242,6 +244,8 @@ def main():
             g.set_option("coef_mode", args.coef_mode)
         if args.temporal_block:
             g.set_option("temporal_block", args.temporal_block)
+        if args.source_kind:
+            g.set_option("source_kind", args.source_kind)
         # synthetic state resident in HBM: seeded random data on all four planes (throughput does not
         # depend on values; zero data as in the config would let nothing but the source window move)
         gen = torch.Generator(device="cuda").manual_seed(wl.SEED_BASE + cfg.cid + rank)
@@ -308,7 +312,7 @@ def main():
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfg.name, "grid": [cfg.n_r, cfg.n_theta], "modes": list(cfg.modes), "a": cfg.a,
-                       "dt": cfg.dt, "source": cfg.source, "coef_mode": args.coef_mode, "slab_rows": int(slab_rows), "temporal_block": args.temporal_block or "default", "observers": list(cfg.observers),
+                       "dt": cfg.dt, "source": cfg.source, "source_kind": args.source_kind, "coef_mode": args.coef_mode, "slab_rows": int(slab_rows), "temporal_block": args.temporal_block or "default", "observers": list(cfg.observers),
                        "state_mb": 4 * cfg.n_pts * 8 / 1e6, "parallelism": "replicas x%d" % world,
                        "l2": "inputs larger than L2 (two 537 MB state copies stream through a 126 MB L2)"
                        if 4 * cfg.n_pts * 8 > 2.5e8 else "state fits in L2: not an HBM measurement"},
@@ -322,7 +326,7 @@ def main():
                          "kernel": "teuk_step_kernel", "bytes_per_pt_step": BYTES_PER_PT_STEP},
         }
         if world == 1 and not args.no_cpu_baseline and not args.quick:
-            val, dt, threads, sample = time_oracle(cfg, 20, 3, args.oracle_rows)
+            val, dt, threads, sample = time_oracle(cfg, 20, 3, args.oracle_rows, args.source_kind)
             line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample}
         print(json.dumps(line), flush=True)
     if world > 1:

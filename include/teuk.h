@@ -112,6 +112,12 @@ int teuk_get_state(teuk_solver *s, double *phi_re, double *phi_im, double *pi_re
 
 /* Options (set before stepping):
  *   "outer_bc"      0 = outgoing (Pi = 0, Phi upwind; default), 1 = Dirichlet as PAPER.md:104
+ *   "source_kind"   deposit profile of the particle source: 0 = the Gaussian g of teuk_orbit
+ *                   (default); 1 = two-point "discrete delta" = finite-difference derivative of the discrete
+ *                   step function: weights (1-gamma)/h, gamma/h on the two grid points around the particle;
+ *                   2 = four-point discrete delta (cubic Lagrange weights / h).  For 1 and 2 the widths are the
+ *                   grid spacings (dx, dtheta) of the stage's own grid and sigma_r, sigma_theta, half_window
+ *                   of teuk_orbit are ignored.
  *   "stream"        a cudaStream_t cast to int64 (0 = back to the solver's own stream)
  *   "coef_mode"     0 = coefficients recomputed on the fly from 1D tables (default),
  *                   1 = coefficients streamed from precomputed 2D FP64 planes (n_theta <= 128 only)

@@ -74,7 +74,7 @@ struct teuk_solver {
   long long base_on_device;
   int* d_nonfinite;
   // source
-  int has_source, W;
+  int has_source, W, source_kind;
   long long n_samples;
   double *d_xp, *d_thp, *d_amp_re, *d_amp_im;
   double sigma_r, sigma_th;
@@ -192,14 +192,15 @@ void fill_params(const teuk_solver* s, StepParams* p, int in_buf, int k, int tap
   p->rs_min = s->rs_min;
   p->dth = s->dth;
   p->has_source = s->has_source;
-  p->W = s->W;
+  p->source_kind = s->source_kind;
+  p->W = s->source_kind ? s->source_kind : s->W;           // discrete deltas: the window is their support
   p->n_samples = s->n_samples;
   p->xp = s->d_xp;
   p->thp = s->d_thp;
   p->amp_re = s->d_amp_re;
   p->amp_im = s->d_amp_im;
-  p->sigma_r = s->sigma_r;
-  p->sigma_th = s->sigma_th;
+  p->sigma_r = s->source_kind ? s->dx : s->sigma_r;       // ... and their widths are the grid spacings
+  p->sigma_th = s->source_kind ? s->dth : s->sigma_th;
   p->d_base = s->d_base;
   p->k = k;
   p->tap_enable = tap_enable;
@@ -779,6 +780,9 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
   if (!strcmp(key, "outer_bc")) {
     if (value != 0 && value != 1) return fail(s, TEUK_EINVAL, "outer_bc must be 0 or 1");
     s->outer_bc = (int)value;
+  } else if (!strcmp(key, "source_kind")) {
+    if (value < 0 || value > 2) return fail(s, TEUK_EINVAL, "source_kind must be 0 (Gaussian), 1 or 2 (discrete delta)");
+    s->source_kind = (int)value;
   } else if (!strcmp(key, "stream")) {
     s->stream = value ? (cudaStream_t)(uintptr_t)value : s->own_stream;
   } else if (!strcmp(key, "coef_mode")) {

@@ -65,6 +65,7 @@ struct StepParams {
   double dt, dx, rs_min, dth;
   // source
   int has_source, W;
+  int source_kind;        // 0 Gaussian (sigma_r, sigma_th), 1 / 2 two- / four-point discrete delta (widths dx, dth)
   long long n_samples;
   const double *xp, *thp, *amp_re, *amp_im;
   double sigma_r, sigma_th;

@@ -367,6 +367,18 @@ __device__ __forceinline__ double gauss_dev(double y, double sigma) {
   return exp(-y * y / (2.0 * sigma * sigma)) / (sigma * sqrt(2.0 * 3.14159265358979323846264338327950288));
 }
 
+// Deposit profile along one axis at offset y from the particle.  kind 0: the Gaussian above, width = sigma.
+// kind 1 / 2: two-point / four-point discrete delta on a grid of spacing `width`:
+// the interpolation weight of the grid point at distance s = |y|/width, over the spacing.
+__device__ __forceinline__ double deposit_profile(int kind, double y, double width) {
+  if (kind == 0) return gauss_dev(y, width);
+  const double s = fabs(y) / width;
+  if (kind == 1) return s < 1.0 ? (1.0 - s) / width : 0.0;
+  if (s < 1.0) return (1.0 - s) * (1.0 + s) * (2.0 - s) / 2.0 / width;
+  if (s < 2.0) return (1.0 - s) * (2.0 - s) * (3.0 - s) / 6.0 / width;
+  return 0.0;
+}
+
 }  // namespace
 
 namespace {
@@ -401,7 +413,7 @@ __device__ __forceinline__ void setup_source(StageSource<V>& s, const StepParams
   for (int q = 0; q < V; ++q) {
     const int j = col0 + col_of<V, MAP>(lane, q);
     const double th = __dmul_rn((double)j + 0.5, p.dth);
-    s.gth[q] = ((unsigned)j < (unsigned)p.n_theta && abs(j - jp) <= p.W) ? gauss_dev(th - thp, p.sigma_th) : 0.0;
+    s.gth[q] = ((unsigned)j < (unsigned)p.n_theta && abs(j - jp) <= p.W) ? deposit_profile(p.source_kind, th - thp, p.sigma_th) : 0.0;
   }
 }
 
@@ -412,7 +424,7 @@ __device__ __forceinline__ void add_source(Row<V>& out, const StageSource<V>& s,
   if (!s.on || abs(i - s.ip) > p.W) return;
   double x = __dadd_rn(p.rs_min, __dmul_rn((double)i, p.dx));
   if (half) x = __dadd_rn(x, __dmul_rn(0.5, p.dx));
-  const double g = p.dt * gauss_dev(x - s.xp, p.sigma_r);
+  const double g = p.dt * deposit_profile(p.source_kind, x - s.xp, p.sigma_r);
 #pragma unroll
   for (int q = 0; q < V; ++q) {
     const double gg = g * s.gth[q];

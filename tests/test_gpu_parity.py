@@ -30,7 +30,8 @@ def rel_l2(got, ref):
     return float(np.linalg.norm(got - ref) / den)
 
 
-def run_pair(orc, teuk, cfg, steps, initial=None, observers=None, options=None, orbit_steps=None, chunks=None):
+def run_pair(orc, teuk, cfg, steps, initial=None, observers=None, options=None, orbit_steps=None, chunks=None,
+             source_kind=0):
     """Run oracle and GPU on the same inputs; return dict of states and waveforms."""
     ini = wl.initial_data(cfg) if initial is None else initial
     orbit = wl.orbit_table(cfg, n_steps=orbit_steps if orbit_steps is not None else max(steps, 1))
@@ -44,6 +45,9 @@ def run_pair(orc, teuk, cfg, steps, initial=None, observers=None, options=None, 
     g.set_initial(*ini)
     o.set_source(orbit)
     g.set_source(orbit)
+    if source_kind:
+        o.set_source_kind(source_kind)
+        g.set_option("source_kind", source_kind)
     for x in observers:
         o.add_observer(x, W)
         g.add_observer(x, W)
@@ -390,3 +394,48 @@ def test_temporal_blocking_parity_with_oracle(orc, teuk):
     for cfg in (SMALL[3], SMALL[4], SMALL[5]):
         res = run_pair(orc, teuk, cfg, min(cfg.steps, 151), options={"temporal_block": 2})
         check_pair(res)
+
+
+# ---- discrete-delta deposits ------------------------------------------
+@pytest.mark.parametrize("kind", [1, 2])
+@pytest.mark.parametrize("cfg", SMALL[3:], ids=[c.name for c in SMALL[3:]])
+def test_discrete_delta_source_parity(orc, teuk, cfg, kind):
+    res = run_pair(orc, teuk, cfg, min(cfg.steps, 200), source_kind=kind)
+    check_pair(res)
+
+
+@pytest.mark.parametrize("kind", [1, 2])
+def test_discrete_delta_source_variants(orc, teuk, kind):
+    """Same deposit in every kernel variant: theta segments, shared-memory kernel, temporal blocking, planes."""
+    cfg = SMALL[3]
+    base = run_pair(orc, teuk, cfg, 61, source_kind=kind)
+    check_pair(base)
+    for opt in ({"kernel": 1}, {"temporal_block": 2}, {"graph": 0}, {"slab_rows": 7}):
+        r = run_pair(orc, teuk, cfg, 61, source_kind=kind, options=opt)
+        for a, b in zip(base["sg"], r["sg"]):
+            assert np.array_equal(a, b), opt
+    check_pair(run_pair(orc, teuk, cfg, 61, source_kind=kind, options={"coef_mode": 1}))
+    wide = cfg.scaled(n_theta=304)
+    check_pair(run_pair(orc, teuk, wide, 40, source_kind=kind))
+
+
+def test_discrete_delta_differs_from_gaussian_and_first_step_closed_form(orc, teuk):
+    """Non-vacuity: the option changes the fields; after one iteration from zero data Pi is non-zero on the
+    few points of the deposit's support only (2 rows x 2 columns of the full stage plus the half stage's
+    neighbours), against (2W+1)^2 for the Gaussian."""
+    cfg = SMALL[3]
+    nz = {}
+    for kind in (0, 1, 2):
+        res = run_pair(orc, teuk, cfg, 1, source_kind=kind, observers=[])
+        check_pair(res, tol=1e-12)
+        nz[kind] = int(np.count_nonzero(res["sg"][2]) + np.count_nonzero(res["sg"][3]))
+    assert 0 < nz[1] < nz[2] < nz[0]
+    assert nz[1] <= 2 * 5 * 6 and nz[2] <= 2 * 7 * 8
+
+
+def test_source_kind_argument_errors(teuk):
+    g = teuk.Solver.from_config(SMALL[3])
+    for bad in (-1, 3):
+        with pytest.raises(teuk.TeukError):
+            g.set_option("source_kind", bad)
+    g.close()
