@@ -76,7 +76,8 @@ int teuk_select_device(int32_t device);
  * iteration covers all modes).  dt > 0 is the time step (the caller is responsible for stability:
  * DESIGN.md reading A1).  Allocates all device state (two copies of the fields, coefficient
  * tables), builds the coefficient tables on the device, zeroes the fields.  Uses the CUDA device
- * that is current in the calling thread.  *out is set to NULL on failure. */
+ * that is current in the calling thread; every later call on the handle runs on that device whatever
+ * device is current then, and restores the caller's current device.  *out is set to NULL on failure. */
 int teuk_create(teuk_solver **out, double a, double M, const int32_t *m, int32_t n_modes,
                 const teuk_grid *grid, double dt);
 

@@ -118,6 +118,21 @@ int cuda_fail(teuk_solver* s, cudaError_t e, const char* where) {
     if (e_ != cudaSuccess) return cuda_fail(s, e_, where); \
   } while (0)
 
+// Every entry point runs on the solver's own device and leaves the caller's current device as it found it
+// (several solvers on different GPUs may be driven from one thread).
+struct DeviceGuard {
+  int prev;
+  bool switched;
+  explicit DeviceGuard(const teuk_solver* s) : prev(-1), switched(false) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != s->device) switched = cudaSetDevice(s->device) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
 size_t state_doubles(const teuk_solver* s) { return (size_t)s->n_modes * s->n_r * 4 * s->n_theta; }
 
 void drop_graph(teuk_solver* s) {
@@ -284,7 +299,7 @@ const char* teuk_last_error(const teuk_solver* s) { return s ? s->err : g_create
 
 void teuk_destroy(teuk_solver* s) {
   if (!s) return;
-  cudaSetDevice(s->device);
+  DeviceGuard guard(s);
   if (s->stream) cudaStreamSynchronize(s->stream);
   if (s->copy_stream) cudaStreamSynchronize(s->copy_stream);
   drop_graph(s);
@@ -395,6 +410,7 @@ int teuk_create(teuk_solver** out, double a, double M, const int32_t* m, int32_t
 
 int teuk_sync(teuk_solver* s) {
   if (!s) return TEUK_EINVAL;
+  DeviceGuard guard(s);
   if (s->sticky) return TEUK_ECUDA;
   CK(cudaStreamSynchronize(s->stream), "teuk_sync");
   CK(cudaStreamSynchronize(s->copy_stream), "teuk_sync");
@@ -404,6 +420,7 @@ int teuk_sync(teuk_solver* s) {
 int teuk_set_initial(teuk_solver* s, const double* phi_re, const double* phi_im, const double* pi_re,
                      const double* pi_im, int32_t ptr_is_device) {
   if (!s) return TEUK_EINVAL;
+  DeviceGuard guard(s);
   if (s->sticky) return TEUK_ECUDA;
   const double* src[4] = {phi_re, phi_im, pi_re, pi_im};
   const size_t n_pts = (size_t)s->n_modes * s->n_r * s->n_theta;
@@ -436,6 +453,7 @@ int teuk_set_initial(teuk_solver* s, const double* phi_re, const double* phi_im,
 
 int teuk_set_source(teuk_solver* s, const teuk_orbit* orbit) {
   if (!s) return TEUK_EINVAL;
+  DeviceGuard guard(s);
   if (s->sticky) return TEUK_ECUDA;
   if (orbit) {
     if (orbit->n_samples < 2 || !orbit->rs_p || !orbit->theta_p || !orbit->amp_re || !orbit->amp_im)
@@ -650,6 +668,7 @@ extern "C" {
 
 int teuk_step(teuk_solver* s, int64_t n) {
   if (!s) return TEUK_EINVAL;
+  DeviceGuard guard(s);
   if (s->sticky) return TEUK_ECUDA;
   if (n < 0) return fail(s, TEUK_EINVAL, "teuk_step: n < 0");
   if (s->has_source && 2 * (s->step + n) > s->n_samples)
@@ -688,6 +707,7 @@ int teuk_step(teuk_solver* s, int64_t n) {
 int teuk_extract(teuk_solver* s, double rs_obs, const double* weights, double* t_out, double* w_re,
                  double* w_im, int64_t capacity, int64_t* n_written) {
   if (!s) return TEUK_EINVAL;
+  DeviceGuard guard(s);
   if (s->sticky) return TEUK_ECUDA;
   if (n_written) *n_written = 0;
   int q = -1;
@@ -754,6 +774,7 @@ int teuk_extract(teuk_solver* s, double rs_obs, const double* weights, double* t
 int teuk_get_state(teuk_solver* s, double* phi_re, double* phi_im, double* pi_re, double* pi_im,
                    int32_t ptr_is_device) {
   if (!s) return TEUK_EINVAL;
+  DeviceGuard guard(s);
   if (s->sticky) return TEUK_ECUDA;
   double* dst[4] = {phi_re, phi_im, pi_re, pi_im};
   const size_t n_pts = (size_t)s->n_modes * s->n_r * s->n_theta;
@@ -775,6 +796,7 @@ int teuk_get_state(teuk_solver* s, double* phi_re, double* phi_im, double* pi_re
 
 int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
   if (!s || !key) return TEUK_EINVAL;
+  DeviceGuard guard(s);
   if (s->sticky) return TEUK_ECUDA;
   CK(cudaStreamSynchronize(s->stream), "set_option: sync");
   if (!strcmp(key, "outer_bc")) {
