@@ -552,6 +552,9 @@ __device__ __forceinline__ void stage_rtab_chunk(double* sbuf, const double* __r
 // every lane is valid, and all per-lane bounds predicates fold away.
 // Resident blocks per SM: V = 2 fits 160 registers without spills -> 3 blocks (12 warps; measured +5-9 %);
 // V = 4 needs all 255 registers -> 2 blocks; V = 1 lands at ~120 registers -> 4 blocks either way.
+// Measured and rejected for V = 4 (config 5, same box, base 88.6-92.0 GPts/s): 9 warps per SM (96-thread
+// blocks, __maxnreg__(224): 388 B of spill stores) 69.6; bracket B accumulated in two partial sums
+// (shorter dependent chains, more spills) 89.1.
 template <int V, bool VEC, int CM, bool SEG, bool FULLW>
 __global__ void __launch_bounds__(128, (V == 2 ? 3 : TEUK_MIN_BLOCKS)) teuk_step_kernel(const __grid_constant__ StepParams p) {
   const int lane = threadIdx.x & 31;

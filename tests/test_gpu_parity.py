@@ -439,3 +439,43 @@ def test_source_kind_argument_errors(teuk):
         with pytest.raises(teuk.TeukError):
             g.set_option("source_kind", bad)
     g.close()
+
+
+# ---- maximum sizes and degenerate cases of the interface ---------------------------------------------------
+def test_maximum_theta_width(orc, teuk):
+    """n_theta = 4096, the largest the ABI accepts (35 theta segments), with the minimum n_r = 4."""
+    for n_r in (4, 9):
+        cfg = SMALL[3].scaled(name="thmax", n_r=n_r, n_theta=4096, rs_min=5.0, rs_max=5.0 + 0.01 * (n_r - 1),
+                              dt_over_dx=1e-4, steps=6, modes=(2,), observers=(5.005,), source=None)
+        res = run_pair(orc, teuk, cfg, 6, initial=wl.random_state(cfg, 4096 + n_r))
+        check_pair(res, tol=1e-11)
+
+
+def test_maximum_mode_count(orc, teuk):
+    """64 modes in one launch (gridDim.y = 64), m = -32 .. 31: both pole parities, m = 0, negative m."""
+    modes = tuple(range(-32, 32))
+    cfg = SMALL[3].scaled(name="m64", n_r=41, n_theta=32, modes=modes, dt_over_dx=0.002, steps=8,
+                          rs_min=-5.0, rs_max=35.0, observers=(10.0,), source=None)
+    res = run_pair(orc, teuk, cfg, 8, initial=wl.random_state(cfg, 64))
+    check_pair(res, tol=1e-11)
+    with pytest.raises(teuk.TeukError):
+        teuk.Solver(0.5, 1.0, list(range(65)), -10, 10, 64, 32, 0.01)
+
+
+def test_empty_calls(orc, teuk):
+    """step(0), extract before any step, get_state right after create: defined, empty, zero."""
+    cfg = SMALL[3]
+    g = teuk.Solver.from_config(cfg)
+    g.add_observer(cfg.observers[0], wl.observer_weights(cfg))
+    g.step(0)
+    t, w = g.extract(cfg.observers[0])
+    assert len(t) == 0 and w.shape == (0, cfg.n_modes)
+    assert all(np.all(a == 0.0) for a in g.get_state())
+    assert g.stat("steps") == 0
+    g.set_initial()
+    g.set_source(None)                                   # source-free, zero data: stays exactly zero
+    g.step(33)
+    assert all(np.all(a == 0.0) for a in g.get_state())
+    t, w = g.extract(cfg.observers[0])
+    assert len(t) == 33 and np.all(w == 0.0)
+    g.close()
