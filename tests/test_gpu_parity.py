@@ -351,14 +351,15 @@ def test_seeded_fuzz_of_shapes_and_options(orc, teuk):
         if coef_mode:
             opts["coef_mode"] = 1
         steps = int(rng.integers(1, 6))
+        kind = int(rng.integers(0, 3))
         cfg = wl.Config(100 + case, "fuzz%d" % case, a, 1.0, modes, lo, lo + dx * (n_r - 1), n_r, n_theta,
                         0.01 / max(1, n_theta // 64), steps, (lo + 0.37 * dx * (n_r - 1),), "zero", "circular",
                         outer_bc=opts["outer_bc"])
-        res = run_pair(orc, teuk, cfg, steps, initial=wl.random_state(cfg, case), options=opts)
+        res = run_pair(orc, teuk, cfg, steps, initial=wl.random_state(cfg, case), options=opts, source_kind=kind)
         try:
             check_pair(res, tol=1e-11)
         except AssertionError as e:
-            raise AssertionError("case %d: n_r=%d n_theta=%d a=%g modes=%s opts=%s: %s" % (case, n_r, n_theta, a, modes, opts, e))
+            raise AssertionError("case %d: n_r=%d n_theta=%d a=%g modes=%s opts=%s source_kind=%d: %s" % (case, n_r, n_theta, a, modes, opts, kind, e))
 
 
 @pytest.mark.parametrize("n_r,n_theta", [(4, 8), (5, 32), (7, 64), (37, 128), (150, 64), (333, 128), (200, 100), (64, 20)])
