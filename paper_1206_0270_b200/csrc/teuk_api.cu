@@ -20,6 +20,9 @@ cudaError_t teuk_launch_coef2d(double* c2d, const double* rtab, const double* tt
                                int n_theta, double dx, cudaStream_t st);
 cudaError_t teuk_launch_step(const StepParams& p, cudaStream_t st);
 cudaError_t teuk_launch_step_tb2(const StepParams& p, cudaStream_t st);
+cudaError_t teuk_launch_step_resident(const StepParams& p, int ncta, cudaStream_t st);
+size_t teuk_resident_smem_bytes(int n_theta, int res_rows);
+size_t teuk_resident_ll_bytes(int n_theta, int n_modes, int ncta);
 cudaError_t teuk_launch_flush_tap(const StepParams& p, cudaStream_t st);
 cudaError_t teuk_launch_bump(long long* d_base, long long inc, cudaStream_t st);
 cudaError_t teuk_launch_set_base(long long* d_base, long long v, cudaStream_t st);
@@ -62,6 +65,10 @@ struct teuk_solver {
   int tuned_rows;        // slab length chosen by the one-time autotune (0 = not tuned yet)
   int temporal_block;    // 1 = one iteration per launch, 2 = two (warp pairs, level n+1 stays on chip)
   int tuned_rows2;       // autotuned slab length of the temporal-blocking kernel
+  // resident kernel ("kernel" = 2): rows per block, blocks per mode, exchange buffer and its running tag
+  int res_rows, res_ncta, smem_optin;
+  void* d_ll;
+  unsigned ll_tag;
   // device
   int device, n_sms;
   cudaStream_t own_stream, stream, copy_stream;
@@ -171,6 +178,20 @@ bool tb2_possible(const teuk_solver* s) {
   return s->variant == 0 && s->coef_mode == 0 && n_segments(s) == 1 && s->n_theta % vsel == 0;
 }
 bool tb2_active(const teuk_solver* s) { return s->temporal_block == 2 && tb2_possible(s); }
+
+// Resident kernel (teuk_resident.cuh): at most one block per SM, every mode split over the same number of
+// blocks, each block's rows (state + half-step rows) in shared memory.  Returns false if that does not fit.
+bool resident_plan(const teuk_solver* s, int* res_rows, int* ncta) {
+  if (s->n_theta > 128 || s->coef_mode != 0 || s->n_modes > s->n_sms) return false;
+  const int interior = s->n_r - 2;
+  int per_mode = s->n_sms / s->n_modes;
+  if (per_mode > interior) per_mode = interior;
+  const int rows = (interior + per_mode - 1) / per_mode;
+  if (teuk_resident_smem_bytes(s->n_theta, rows) > (size_t)s->smem_optin) return false;
+  *res_rows = rows;
+  *ncta = (interior + rows - 1) / rows;
+  return true;
+}
 
 int rows_for_waves(const teuk_solver* s, double waves, int tb = 1) {
   const long long interior = s->n_r - 2;
@@ -316,6 +337,7 @@ void teuk_destroy(teuk_solver* s) {
   cudaFree(s->d_m);
   cudaFree(s->d_base);
   cudaFree(s->d_nonfinite);
+  cudaFree(s->d_ll);
   cudaFree(s->d_xp);
   cudaFree(s->d_thp);
   cudaFree(s->d_amp_re);
@@ -370,6 +392,7 @@ int teuk_create(teuk_solver** out, double a, double M, const int32_t* m, int32_t
   s->outer_bc = 0; s->coef_mode = 0; s->slab_rows_opt = 0; s->use_graph = 1; s->autotune = 1; s->tuned_rows = 0; s->temporal_block = 1; s->tuned_rows2 = 0;
   s->device = dev;
   if (cudaDeviceGetAttribute(&s->n_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) s->n_sms = 148;
+  if (cudaDeviceGetAttribute(&s->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) s->smem_optin = 0;
   snprintf(s->err, sizeof(s->err), "no error");
   int rc = TEUK_OK;
   do {
@@ -600,6 +623,40 @@ int run_chunk(teuk_solver* s, long long c) {
   long long left = c;
   int first = 1;
   const bool tb2 = tb2_active(s);
+  if (s->variant == 2) {   // all c iterations in one cooperative launch, state on chip in between
+    if (!s->d_ll) {
+      const size_t bytes = teuk_resident_ll_bytes(s->n_theta, s->n_modes, s->res_ncta);
+      CK(cudaMalloc(&s->d_ll, bytes), "resident: exchange buffer alloc");
+      CK(cudaMemsetAsync(s->d_ll, 0, bytes, s->stream), "resident: exchange buffer zero");
+      s->ll_tag = 0;
+    }
+    while (left > 0) {
+      const long long k = s->step - s->base_on_device;
+      if (k < 0 || k > (1LL << 30)) {
+        CK(teuk_launch_set_base(s->d_base, s->step, s->stream), "step: counter");
+        s->base_on_device = s->step;
+        s->launches += 1;
+      }
+      const long long m = left < (1LL << 30) ? left : (1LL << 30);
+      if ((unsigned long long)s->ll_tag + (unsigned long long)m >= 0xfffffff0ull) {   // tags would wrap: start over
+        CK(cudaMemsetAsync(s->d_ll, 0, teuk_resident_ll_bytes(s->n_theta, s->n_modes, s->res_ncta), s->stream),
+           "resident: exchange buffer zero");
+        s->ll_tag = 0;
+      }
+      StepParams p;
+      fill_params(s, &p, s->cur, (int)(s->step - s->base_on_device), 0);   // level s->step was tapped by the last flush
+      p.n_iter = (int)m;
+      p.res_rows = s->res_rows;
+      p.tag0 = s->ll_tag;
+      p.ll = s->d_ll;
+      CK(teuk_launch_step_resident(p, s->res_ncta, s->stream), "step: resident launch");
+      s->ll_tag += (unsigned)m;
+      s->launches += 1;
+      s->cur ^= 1;
+      s->step += m;
+      left -= m;
+    }
+  }
   while (left > 0) {
     const bool graph_ok = s->use_graph && !first && left >= kGraphBatch;
     if (graph_ok) {
@@ -673,7 +730,7 @@ int teuk_step(teuk_solver* s, int64_t n) {
   if (n < 0) return fail(s, TEUK_EINVAL, "teuk_step: n < 0");
   if (s->has_source && 2 * (s->step + n) > s->n_samples)
     return fail(s, TEUK_EINVAL, "teuk_step: trajectory table too short for n more iterations");
-  if (n > 0 && s->autotune && s->slab_rows_opt == 0 && (s->base_on_device <= s->step)) {
+  if (n > 0 && s->variant != 2 && s->autotune && s->slab_rows_opt == 0 && (s->base_on_device <= s->step)) {
     if (s->tuned_rows == 0) {
       const int rc = tune_slab_rows(s, 1);
       if (rc != TEUK_OK) return rc;
@@ -830,13 +887,20 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
   } else if (!strcmp(key, "temporal_block")) {
     if (value != 1 && value != 2) return fail(s, TEUK_EINVAL, "temporal_block must be 1 or 2");
     s->temporal_block = (int)value;
-    if (value == 2 && !tb2_possible(s)) {
+    if (value == 2 && (!tb2_possible(s) || s->variant == 2)) {
       s->temporal_block = 1;
       return fail(s, TEUK_EINVAL, "temporal_block 2 needs kernel 0, coef_mode 0, n_theta <= 128 and a multiple of its lane width (1, 2 or 4)");
     }
   } else if (!strcmp(key, "kernel")) {
-    if (value != 0 && value != 1) return fail(s, TEUK_EINVAL, "kernel must be 0 (register-resident) or 1 (shared-memory-resident)");
-    if (value == 1 && s->coef_mode != 0) return fail(s, TEUK_EINVAL, "kernel 1 needs coef_mode 0");
+    if (value < 0 || value > 2)
+      return fail(s, TEUK_EINVAL, "kernel must be 0 (register-resident), 1 (shared-memory-resident) or 2 (resident, whole state on chip)");
+    if (value != 0 && s->coef_mode != 0) return fail(s, TEUK_EINVAL, "kernels 1 and 2 need coef_mode 0");
+    if (value == 2) {
+      if (s->temporal_block == 2) return fail(s, TEUK_EINVAL, "kernel 2 needs temporal_block 1");
+      if (!resident_plan(s, &s->res_rows, &s->res_ncta))
+        return fail(s, TEUK_EINVAL, "kernel 2 needs n_theta <= 128 and a state that fits in the shared memory of one block per SM");
+      if (s->d_ll) { cudaFree(s->d_ll); s->d_ll = nullptr; }
+    }
     if (value == 1 && s->n_theta > 256) return fail(s, TEUK_EINVAL, "kernel 1 needs n_theta <= 256");
     if (value == 1 && s->temporal_block == 2) return fail(s, TEUK_EINVAL, "kernel 1 needs temporal_block 1");
     s->variant = (int)value;
@@ -854,6 +918,9 @@ int teuk_get_stat(const teuk_solver* s, const char* key, int64_t* value) {
   else if (!strcmp(key, "launches")) *value = s->launches;
   else if (!strcmp(key, "n_pts")) *value = (int64_t)s->n_modes * s->n_r * s->n_theta;
   else if (!strcmp(key, "state_bytes")) *value = (int64_t)(state_doubles(s) * sizeof(double));
+  else if (!strcmp(key, "kernel")) *value = s->variant;
+  else if (!strcmp(key, "resident_rows")) *value = s->variant == 2 ? s->res_rows : 0;
+  else if (!strcmp(key, "resident_blocks")) *value = s->variant == 2 ? (int64_t)s->res_ncta * s->n_modes : 0;
   else if (!strcmp(key, "slab_rows")) {
     const int tb = tb2_active(s) ? 2 : 1;
     const int tuned = tb == 2 ? s->tuned_rows2 : s->tuned_rows;

@@ -60,7 +60,7 @@ struct StepParams {
   int n_r, n_theta, n_modes;
   int slab_rows, n_slabs;
   int n_seg, seg_payload; // theta segments (register kernel, n_theta > 128): count and payload columns each
-  int variant;            // 0 = register-resident kernel, 1 = shared-memory-resident kernel
+  int variant;            // 0 = register-resident kernel, 1 = shared-memory-resident kernel, 2 = resident (on-chip) kernel
   int outer_bc;
   double dt, dx, rs_min, dth;
   // source
@@ -76,6 +76,12 @@ struct StepParams {
   int tap_enable, tap_enable2, n_obs;   // tap_enable2: level n+1 inside a temporal-blocking launch
   long long ring_cap;
   int* nonfinite;
+  // resident kernel ("kernel" = 2, teuk_resident.cuh): iterations per launch, rows of r* per block, tag of the
+  // input level in the block-to-block exchange buffer `ll` ([n_modes][blocks][2 sides][2 parities] rows of
+  // 16-byte {value.lo, tag, value.hi, tag} elements)
+  int n_iter, res_rows;
+  unsigned tag0;
+  void* ll;
   ObsDev obs[TEUK_MAX_OBS];
 };
 

@@ -1,0 +1,271 @@
+// teuk_resident.cuh -- "kernel" = 2: the whole state stays ON CHIP for all iterations of one launch.
+// Included by teuk_step.cu (same translation unit: it reuses lw_stage, the source deposit and the tap, so
+// fields and waveforms are bit-identical to the marching kernels).
+//
+// Why: the small grids (BASELINE.json configs 1 and 2: 0.5 and 8.4 MB of state) are not bandwidth-bound.  With
+// one launch per iteration they are bound by the launch rate (2.9 us per iteration) and by the serial march
+// of each warp (SURVEY.md 8(d) "Config 1 is launch-latency-bound.  Use a persistent kernel").  Here ONE
+// cooperative launch runs n_iter iterations (Eq. 3-4):
+//   * every block owns a contiguous range of r* rows of one mode and keeps them in shared memory for the
+//     whole launch (HBM is touched at entry and exit only);
+//   * an iteration is two block-wide phases separated by __syncthreads: phase 1 computes the half-step rows
+//     2 u^{n+1/2}_{i+1/2} (Eq. 3) into shared memory, one warp per row, phase 2 the full step (Eq. 4) in
+//     place -- no half-step value is computed twice, and a warp's dependent chain per iteration is two stages
+//     long instead of 2 x (slab length + 1);
+//   * neighbouring blocks exchange ONE row per side and iteration through L2 with a flag-in-data protocol
+//     (each 16-byte element = {value.lo, tag, value.hi, tag}, tag = iteration number; an element is valid
+//     when both tags match, so no fence and no separate flag round trip is needed).  A block computes and
+//     publishes its two edge rows FIRST in phase 2 and consumes its neighbours' rows LAST in phase 1 of the
+//     next iteration, so the L2 latency (~0.3 us) hides behind the interior rows;
+//   * pole ghosts, radial edges, source deposit and tap-on-read
+//     as in teuk_step_kernel.
+// All blocks must be co-resident (they wait on each other): the launch is cooperative and sized to at most
+// one block per SM; waits are bounded (trap -> sticky TEUK_ECUDA instead of a hung GPU).
+#ifndef TEUK_RESIDENT_CUH_
+#define TEUK_RESIDENT_CUH_
+
+namespace {
+
+__device__ __forceinline__ void ll_store(uint4* dst, double v, unsigned tag) {
+  const unsigned lo = (unsigned)__double2loint(v), hi = (unsigned)__double2hiint(v);
+  asm volatile("st.volatile.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "r"(lo), "r"(tag), "r"(hi), "r"(tag)
+               : "memory");
+}
+__device__ __forceinline__ bool ll_try_load(const uint4* src, unsigned tag, double& v) {
+  unsigned a, b, c, d;
+  asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "l"(src) : "memory");
+  v = __hiloint2double((int)c, (int)a);
+  return b == tag && d == tag;
+}
+
+// One exchange slot = one row: [4][32 V] 16-byte elements, same lane -> column ownership as the registers.
+template <int V>
+__device__ __forceinline__ void ll_publish(uint4* slot, const Row<V>& u, unsigned tag, int lane) {
+#pragma unroll
+  for (int c = 0; c < 4; ++c)
+#pragma unroll
+    for (int v = 0; v < V; ++v) ll_store(slot + c * 32 * V + lane * V + v, u.c[c][v], tag);
+}
+template <int V>
+__device__ __forceinline__ void ll_receive(const uint4* slot, Row<V>& u, unsigned tag, int lane) {
+  unsigned tries = 0;
+  for (;;) {
+    bool ok = true;
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+      for (int v = 0; v < V; ++v) ok = ll_try_load(slot + c * 32 * V + lane * V + v, tag, u.c[c][v]) && ok;
+    if (__all_sync(FULL, ok)) break;
+    if (++tries > (1u << 22)) asm volatile("trap;");   // a neighbour that never publishes: error, not a hang
+    __nanosleep(32);
+  }
+}
+
+template <int V>
+__device__ __forceinline__ uint4* ll_slot(const StepParams& p, int mode, int ncta, int cta, int side, unsigned tag) {
+  return reinterpret_cast<uint4*>(p.ll) + ((((size_t)mode * ncta + cta) * 2 + side) * 2 + (tag & 1u)) * (size_t)(4 * 32 * V);
+}
+
+}  // namespace
+
+// NW = warps per block the register budget allows (65536 / (32 NW) registers per thread); the launch may use
+// fewer (blockDim.x / 32 = min(NW, rows + 1)).
+template <int V, int NW>
+__global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __grid_constant__ StepParams p) {
+  constexpr int NP = 32 * V;        // padded row width in shared memory (columns >= n_theta stay zero)
+  constexpr int ROWD = 4 * NP;      // doubles per row
+  const int lane = threadIdx.x & 31;
+  const int w = __shfl_sync(FULL, (int)(threadIdx.x >> 5), 0);   // provably warp-uniform
+  const int nw = (int)(blockDim.x >> 5);
+  const int cta = blockIdx.x, ncta = gridDim.x, mode = blockIdx.y;
+  const int nth = p.n_theta, nr = p.n_r;
+  const int lo = 1 + cta * p.res_rows;              // interior nodes [lo, hi) belong to this block
+  const int hi = min(lo + p.res_rows, nr - 1);
+  const int rows = hi - lo;
+  const bool first = cta == 0, last = cta == ncta - 1;
+  const int j0 = lane * V;
+  const size_t row_stride = (size_t)4 * nth;
+  const double* __restrict__ uin = p.uin + (size_t)mode * nr * row_stride;
+  double* __restrict__ uout = p.uout + (size_t)mode * nr * row_stride;
+  const double* __restrict__ rtab = p.rtab + (size_t)mode * (2 * nr - 1) * RT_N;
+
+  extern __shared__ __align__(128) unsigned char s_dyn[];
+  double* const sU = reinterpret_cast<double*>(s_dyn);          // [res_rows + 2] rows: slot r = node lo - 1 + r
+  double* const sH = sU + (size_t)(p.res_rows + 2) * ROWD;      // [res_rows + 1] half rows: slot h = lo - 1 + h + 1/2
+  double* const sE = sH + (size_t)(p.res_rows + 1) * ROWD;      // new outer-edge row (last block)
+  double* const sR = sE + ROWD;                                 // r-table records of locations 2 lo - 1 + q
+
+  // ---- entry: state rows (with both neighbour rows: they serve iteration 0) and r-table records ----
+  for (int r = w; r < rows + 2; r += nw) {
+    Row<V> t;
+    load_row<V, false>(t, uin + (size_t)(lo - 1 + r) * row_stride, nth, j0);
+    sts_row<V>(t, sU + (size_t)r * ROWD, NP, j0);
+  }
+  for (int q = threadIdx.x; q < (2 * rows + 2) * RT_N; q += blockDim.x) {
+    const int loc = 2 * lo - 1 + q / RT_N;
+    if (loc <= 2 * nr - 2) sR[q] = rtab[(size_t)loc * RT_N + q % RT_N];
+  }
+  ThetaTab<V> th;
+  {
+    const double* tb = p.ttab + (size_t)mode * TT_N * nth;
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const bool ok = j0 + v < nth;
+      th.vals.s2[v] = ok ? tb[TT_S2 * nth + j0 + v] : 0.0;
+      th.vals.cs[v] = ok ? tb[TT_COS * nth + j0 + v] : 0.0;
+      th.vals.ap[v] = ok ? tb[TT_AP * nth + j0 + v] : 0.0;
+      th.vals.am[v] = ok ? tb[TT_AM * nth + j0 + v] : 0.0;
+      th.vals.d0[v] = ok ? tb[TT_D0 * nth + j0 + v] : 0.0;
+    }
+  }
+  __syncthreads();
+
+  const double tau_h = 0.5 * p.dt, tau_f = 0.25 * p.dt, tdx = 2.0 / p.dx;
+  const double src_reach = ((double)p.W + 2.0) * p.dx;   // conservative pre-test of the source window in x
+  const long long n0 = *p.d_base + p.k;                  // index of the input level of iteration 0
+
+  for (int it = 0; it < p.n_iter; ++it) {
+    const long long n = n0 + it;
+    const unsigned tag_in = p.tag0 + (unsigned)it;       // tag of the rows published during iteration it - 1
+    const bool do_tap = p.n_obs > 0 && n >= 1 && (it > 0 || p.tap_enable);
+
+    // ---- phase 1: half-step rows (Eq. 3).  Rows that need a neighbour block's row come last. ----
+    for (int t = w; t <= rows; t += nw) {
+      const int h = (t < rows - 1) ? t + 1 : (t == rows - 1 ? 0 : rows);
+      const int i = lo - 1 + h;                          // half point i + 1/2 between nodes i and i + 1
+      Row<V> A, B, Hn;
+      if (h == 0 && !first && it > 0) ll_receive<V>(ll_slot<V>(p, mode, ncta, cta - 1, 1, tag_in), A, tag_in, lane);
+      else lds_row<V>(A, sU + (size_t)h * ROWD, NP, j0, true);
+      if (h == rows && !last && it > 0) ll_receive<V>(ll_slot<V>(p, mode, ncta, cta + 1, 0, tag_in), B, tag_in, lane);
+      else lds_row<V>(B, sU + (size_t)(h + 1) * ROWD, NP, j0, true);
+      if (do_tap) tap<V>(A, B, p, i, mode, n, lane);
+      lw_stage<V, true>(A, B, A, sR + (2 * h) * RT_N, th, tau_h, tdx, Hn);
+      if (p.has_source) {
+        const double x = p.rs_min + ((double)i + 0.5) * p.dx;
+        if (fabs(x - __ldg(p.xp + 2 * n)) <= src_reach) {
+          StageSource<V> s;
+          setup_source<V>(s, p, mode, 2 * n, true, i, i, lane, 0);
+          add_source<V>(Hn, s, p, i, true);
+        }
+      }
+      sts_row<V>(Hn, sH + (size_t)h * ROWD, NP, j0);
+      if (last && h == rows) {   // outer radial edge (reading A6): A = row n_r-2, B = row n_r-1
+        const double eps = sR[(2 * rows + 1) * RT_N + RT_EPS];   // location 2 (n_r - 1)
+        ThetaVals<V> tv;
+        th.get(tv);
+        Row<V> e;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+          if (p.outer_bc == 0) {
+            const double b = rsqrt_near_one(fma(-eps, tv.s2[v], 1.0));
+            e.c[0][v] = B.c[0][v] - p.dt * b * (B.c[0][v] - A.c[0][v]) / p.dx;
+            e.c[1][v] = B.c[1][v] - p.dt * b * (B.c[1][v] - A.c[1][v]) / p.dx;
+          } else {
+            e.c[0][v] = 0.0;
+            e.c[1][v] = 0.0;
+          }
+          e.c[2][v] = 0.0;
+          e.c[3][v] = 0.0;
+        }
+        sts_row<V>(e, sE, NP, j0);
+      }
+    }
+    __syncthreads();
+
+    // ---- phase 2: full step in place (Eq. 4).  The two edge rows of the block go first and are published. ----
+    for (int t = w; t < rows; t += nw) {
+      const int r = (t == 0) ? 1 : (t == 1 ? rows : t);
+      const int i = lo - 1 + r;
+      Row<V> Hp, Hn, U0, out;
+      lds_row<V>(Hp, sH + (size_t)(r - 1) * ROWD, NP, j0, true);
+      lds_row<V>(Hn, sH + (size_t)r * ROWD, NP, j0, true);
+      lds_row<V>(U0, sU + (size_t)r * ROWD, NP, j0, true);
+      lw_stage<V, false>(Hp, Hn, U0, sR + (2 * r - 1) * RT_N, th, tau_f, tdx, out);
+      if (p.has_source) {
+        const double x = p.rs_min + (double)i * p.dx;
+        if (fabs(x - __ldg(p.xp + 2 * n + 1)) <= src_reach) {
+          StageSource<V> s;
+          setup_source<V>(s, p, mode, 2 * n + 1, false, i, i, lane, 0);
+          add_source<V>(out, s, p, i, false);
+        }
+      }
+      if (it + 1 < p.n_iter) {
+        if (r == 1 && !first) ll_publish<V>(ll_slot<V>(p, mode, ncta, cta, 0, tag_in + 1u), out, tag_in + 1u, lane);
+        if (r == rows && !last) ll_publish<V>(ll_slot<V>(p, mode, ncta, cta, 1, tag_in + 1u), out, tag_in + 1u, lane);
+      }
+      sts_row<V>(out, sU + (size_t)r * ROWD, NP, j0);
+      if (first && r == 1) {     // inner radial edge: Phi = Pi = 0
+        Row<V> z;
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+          for (int v = 0; v < V; ++v) z.c[c][v] = 0.0;
+        sts_row<V>(z, sU, NP, j0);
+      }
+      if (last && r == rows) {   // new outer-edge row, computed from level n in phase 1
+        Row<V> e;
+        lds_row<V>(e, sE, NP, j0, true);
+        sts_row<V>(e, sU + (size_t)(rows + 1) * ROWD, NP, j0);
+      }
+    }
+    __syncthreads();
+  }
+
+  // ---- exit: the block's rows of the last level go to the other ping-pong buffer ----
+  for (int r = w; r < rows + 2; r += nw) {
+    if ((r == 0 && !first) || (r == rows + 1 && !last)) continue;
+    Row<V> t;
+    lds_row<V>(t, sU + (size_t)r * ROWD, NP, j0, true);
+    store_row<V, false>(t, uout + (size_t)(lo - 1 + r) * row_stride, nth, j0, 0, nth);
+  }
+}
+
+// ---- host side ------------------------------------------------------------------------------------
+template <int V>
+constexpr int resident_max_warps() { return V == 4 ? 8 : 16; }
+
+size_t teuk_resident_smem_bytes(int n_theta, int res_rows) {
+  const int v = (n_theta + 31) / 32;
+  const int V = v <= 1 ? 1 : (v <= 2 ? 2 : 4);
+  const size_t rowd = (size_t)4 * 32 * V;
+  return ((size_t)(2 * res_rows + 4) * rowd + (size_t)(2 * res_rows + 2) * RT_N) * sizeof(double);
+}
+
+// bytes of the exchange buffer: [n_modes][ncta][2 sides][2 parities] rows of 16-byte elements
+size_t teuk_resident_ll_bytes(int n_theta, int n_modes, int ncta) {
+  const int v = (n_theta + 31) / 32;
+  const int V = v <= 1 ? 1 : (v <= 2 ? 2 : 4);
+  return (size_t)n_modes * ncta * 4 * (4 * 32 * V) * 16;
+}
+
+template <int V>
+static cudaError_t launch_resident_v(const StepParams& p, int ncta, cudaStream_t st) {
+  constexpr int NW = resident_max_warps<V>();
+  const size_t dyn = teuk_resident_smem_bytes(p.n_theta, p.res_rows);
+  static bool attr_set[64] = {false};   // per device
+  int dev_ = 0;
+  cudaGetDevice(&dev_);
+  if (!attr_set[dev_ & 63]) {
+    int optin = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev_);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(teuk_step_resident_kernel<V, NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    if (e != cudaSuccess) return e;
+    attr_set[dev_ & 63] = true;
+  }
+  int nwarps = p.res_rows + 1 < NW ? p.res_rows + 1 : NW;
+  dim3 grid(ncta, p.n_modes), block(32 * nwarps);
+  StepParams pc = p;
+  void* args[] = {&pc};
+  return cudaLaunchCooperativeKernel((const void*)teuk_step_resident_kernel<V, NW>, grid, block, args, dyn, st);
+}
+
+// n_iter iterations in one cooperative launch; the caller sized res_rows / ncta so that the state fits.
+cudaError_t teuk_launch_step_resident(const StepParams& p, int ncta, cudaStream_t st) {
+  const int v = (p.n_theta + 31) / 32;
+  if (v <= 1) return launch_resident_v<1>(p, ncta, st);
+  if (v <= 2) return launch_resident_v<2>(p, ncta, st);
+  return launch_resident_v<4>(p, ncta, st);
+}
+
+#endif

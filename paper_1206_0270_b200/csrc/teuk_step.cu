@@ -1338,6 +1338,8 @@ __global__ void teuk_unpack_kernel(const double* __restrict__ u, Planes dst, siz
     if (dst.c[c]) dst.c[c][t] = u[(row * 4 + c) * nth + j];
 }
 
+#include "teuk_resident.cuh"
+
 // ---- host-side launchers (called from teuk_api.cu) -------------------------------------------
 template <int V>
 static cudaError_t launch_v(const StepParams& p, cudaStream_t st) {
