@@ -200,7 +200,7 @@ def main():
     ap.add_argument("--coef-mode", type=int, default=0, help="0 rebuild coefficients (default), 1 stream 2D planes")
     ap.add_argument("--source-kind", type=int, default=0, help="0 Gaussian deposit (the configs'), 1 / 2 discrete delta")
     ap.add_argument("--temporal-block", type=int, default=0, help="0 library default, 1 or 2 iterations per HBM round trip")
-    ap.add_argument("--kernel", type=int, default=-1, help="-1 library default, 0 register-resident, 1 smem-resident")
+    ap.add_argument("--kernel", type=int, default=-1, help="-1 library default (automatic), 0 marching kernel, 1 smem-resident marching kernel, 2 resident (state on chip)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     cfg = wl.CONFIGS[args.config]
@@ -271,6 +271,7 @@ def main():
         ms = e0.elapsed_time(e1)
         launches = g.stat("launches") - l0
         slab_rows = g.stat("slab_rows")
+        kernel_used = g.stat("kernel")
         clocks = sampler.stop() if rank == 0 else None
         ms = max_over_ranks(ms, "cuda", world)
         value = world * cfg.n_pts * K / (ms * 1e-3) / 1e9
@@ -312,7 +313,7 @@ def main():
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfg.name, "grid": [cfg.n_r, cfg.n_theta], "modes": list(cfg.modes), "a": cfg.a,
-                       "dt": cfg.dt, "source": cfg.source, "source_kind": args.source_kind, "coef_mode": args.coef_mode, "slab_rows": int(slab_rows), "temporal_block": args.temporal_block or "default", "observers": list(cfg.observers),
+                       "dt": cfg.dt, "source": cfg.source, "source_kind": args.source_kind, "coef_mode": args.coef_mode, "slab_rows": int(slab_rows), "kernel": int(kernel_used), "temporal_block": args.temporal_block or "default", "observers": list(cfg.observers),
                        "state_mb": 4 * cfg.n_pts * 8 / 1e6, "parallelism": "replicas x%d" % world,
                        "l2": "inputs larger than L2 (two 537 MB state copies stream through a 126 MB L2)"
                        if 4 * cfg.n_pts * 8 > 2.5e8 else "state fits in L2: not an HBM measurement"},
@@ -323,7 +324,7 @@ def main():
             "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": ncu_traffic_bytes(cfg), "peak_source": peak_src,
-                         "kernel": "teuk_step_kernel", "bytes_per_pt_step": BYTES_PER_PT_STEP},
+                         "kernel": "teuk_step_resident_kernel" if kernel_used == 2 else "teuk_step_kernel", "bytes_per_pt_step": BYTES_PER_PT_STEP},
         }
         if world == 1 and not args.no_cpu_baseline and not args.quick:
             val, dt, threads, sample = time_oracle(cfg, 20, 3, args.oracle_rows, args.source_kind)

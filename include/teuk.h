@@ -129,13 +129,22 @@ int teuk_get_state(teuk_solver *s, double *phi_re, double *phi_im, double *pi_re
  *                   (warp pairs; level n+1 stays in shared memory; same results bit for bit; needs kernel 0,
  *                   coef_mode 0, n_theta <= 128)
  *   "graph"         1 = replay the iteration through a CUDA graph (default), 0 = plain launches
- *   "kernel"        0 = register-resident marching kernel, 1 = shared-memory-resident marching kernel
- *                   (same arithmetic, bitwise identical fields; they differ in on-chip residency;
- *                   kernel 1 needs n_theta <= 256) */
+ *   "kernel"        -1 = automatic (default): kernel 2 whenever it applies, else kernel 0;
+ *                   0 = register-resident marching kernel (one launch per iteration, state streamed from HBM/L2);
+ *                   1 = shared-memory-resident marching kernel (n_theta <= 256);
+ *                   2 = resident kernel: ONE cooperative launch per teuk_step call, the whole state stays in
+ *                   shared memory between iterations, neighbouring blocks exchange one row per iteration through
+ *                   L2.  Needs n_theta <= 128, coef_mode 0, temporal_block 1 and a state small enough for the
+ *                   shared memory of one block per SM (about n_modes*n_r*n_theta <= 5e5 points), else EINVAL.
+ *                   All kernels do the same arithmetic per point: fields are bitwise identical (waveforms too,
+ *                   except kernel 1, which sums over theta in another order).  An explicit "slab_rows" makes the
+ *                   automatic choice stay with kernel 0. */
 int teuk_set_option(teuk_solver *s, const char *key, int64_t value);
 
 /* Read-only counters: "steps" (iterations done), "launches" (kernels launched so far),
- * "n_pts" (n_modes*n_r*n_theta), "state_bytes" (one copy of the fields), "slab_rows" (in use). */
+ * "n_pts" (n_modes*n_r*n_theta), "state_bytes" (one copy of the fields), "slab_rows" (in use),
+ * "kernel" (the kernel the next teuk_step would run), "resident_rows" / "resident_blocks" (rows of r* per
+ * block and blocks of kernel 2, 0 if it is not in use). */
 int teuk_get_stat(const teuk_solver *s, const char *key, int64_t *value);
 
 /* Wait for all work enqueued on the solver's stream. */

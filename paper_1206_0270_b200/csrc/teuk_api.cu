@@ -66,6 +66,8 @@ struct teuk_solver {
   int temporal_block;    // 1 = one iteration per launch, 2 = two (warp pairs, level n+1 stays on chip)
   int tuned_rows2;       // autotuned slab length of the temporal-blocking kernel
   // resident kernel ("kernel" = 2): rows per block, blocks per mode, exchange buffer and its running tag
+  int kernel_opt;        // "kernel" option: -1 = automatic (resident kernel when the state fits on chip, else kernel 0)
+  int res_failed;        // automatic choice: a cooperative launch was refused once, stay with kernel 0
   int res_rows, res_ncta, smem_optin;
   void* d_ll;
   unsigned ll_tag;
@@ -191,6 +193,15 @@ bool resident_plan(const teuk_solver* s, int* res_rows, int* ncta) {
   *res_rows = rows;
   *ncta = (interior + rows - 1) / rows;
   return true;
+}
+
+// Which kernel runs the next iterations: the resident one if asked for, or, by default, whenever it applies
+// (results are bit-identical; an explicit slab length, coef_mode 1 or temporal_block 2 address kernel 0).
+bool resident_active(const teuk_solver* s, int* res_rows, int* ncta) {
+  if (s->kernel_opt != 2) {
+    if (s->kernel_opt != -1 || s->res_failed || s->temporal_block != 1 || s->slab_rows_opt > 0) return false;
+  }
+  return resident_plan(s, res_rows, ncta);
 }
 
 int rows_for_waves(const teuk_solver* s, double waves, int tb = 1) {
@@ -390,6 +401,7 @@ int teuk_create(teuk_solver** out, double a, double M, const int32_t* m, int32_t
   s->dth = kPi / grid->n_theta;
   for (int q = 0; q < n_modes; ++q) s->m[q] = m[q];
   s->outer_bc = 0; s->coef_mode = 0; s->slab_rows_opt = 0; s->use_graph = 1; s->autotune = 1; s->tuned_rows = 0; s->temporal_block = 1; s->tuned_rows2 = 0;
+  s->kernel_opt = -1;
   s->device = dev;
   if (cudaDeviceGetAttribute(&s->n_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) s->n_sms = 148;
   if (cudaDeviceGetAttribute(&s->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) s->smem_optin = 0;
@@ -623,7 +635,7 @@ int run_chunk(teuk_solver* s, long long c) {
   long long left = c;
   int first = 1;
   const bool tb2 = tb2_active(s);
-  if (s->variant == 2) {   // all c iterations in one cooperative launch, state on chip in between
+  if (resident_active(s, &s->res_rows, &s->res_ncta)) {   // all c iterations in one cooperative launch, state on chip in between
     if (!s->d_ll) {
       const size_t bytes = teuk_resident_ll_bytes(s->n_theta, s->n_modes, s->res_ncta);
       CK(cudaMalloc(&s->d_ll, bytes), "resident: exchange buffer alloc");
@@ -649,7 +661,14 @@ int run_chunk(teuk_solver* s, long long c) {
       p.res_rows = s->res_rows;
       p.tag0 = s->ll_tag;
       p.ll = s->d_ll;
-      CK(teuk_launch_step_resident(p, s->res_ncta, s->stream), "step: resident launch");
+      const cudaError_t el = teuk_launch_step_resident(p, s->res_ncta, s->stream);
+      if (el != cudaSuccess && s->kernel_opt == -1 &&
+          (el == cudaErrorCooperativeLaunchTooLarge || el == cudaErrorNotSupported || el == cudaErrorLaunchOutOfResources)) {
+        cudaGetLastError();        // the automatic choice does not apply on this device: kernel 0 from now on
+        s->res_failed = 1;
+        break;
+      }
+      CK(el, "step: resident launch");
       s->ll_tag += (unsigned)m;
       s->launches += 1;
       s->cur ^= 1;
@@ -730,7 +749,8 @@ int teuk_step(teuk_solver* s, int64_t n) {
   if (n < 0) return fail(s, TEUK_EINVAL, "teuk_step: n < 0");
   if (s->has_source && 2 * (s->step + n) > s->n_samples)
     return fail(s, TEUK_EINVAL, "teuk_step: trajectory table too short for n more iterations");
-  if (n > 0 && s->variant != 2 && s->autotune && s->slab_rows_opt == 0 && (s->base_on_device <= s->step)) {
+  int rr_ = 0, nc_ = 0;
+  if (n > 0 && !resident_active(s, &rr_, &nc_) && s->autotune && s->slab_rows_opt == 0 && (s->base_on_device <= s->step)) {
     if (s->tuned_rows == 0) {
       const int rc = tune_slab_rows(s, 1);
       if (rc != TEUK_OK) return rc;
@@ -887,23 +907,23 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
   } else if (!strcmp(key, "temporal_block")) {
     if (value != 1 && value != 2) return fail(s, TEUK_EINVAL, "temporal_block must be 1 or 2");
     s->temporal_block = (int)value;
-    if (value == 2 && (!tb2_possible(s) || s->variant == 2)) {
+    if (value == 2 && (!tb2_possible(s) || s->kernel_opt == 2)) {
       s->temporal_block = 1;
       return fail(s, TEUK_EINVAL, "temporal_block 2 needs kernel 0, coef_mode 0, n_theta <= 128 and a multiple of its lane width (1, 2 or 4)");
     }
   } else if (!strcmp(key, "kernel")) {
-    if (value < 0 || value > 2)
-      return fail(s, TEUK_EINVAL, "kernel must be 0 (register-resident), 1 (shared-memory-resident) or 2 (resident, whole state on chip)");
-    if (value != 0 && s->coef_mode != 0) return fail(s, TEUK_EINVAL, "kernels 1 and 2 need coef_mode 0");
+    if (value < -1 || value > 2)
+      return fail(s, TEUK_EINVAL, "kernel must be -1 (automatic), 0 (register-resident), 1 (shared-memory-resident) or 2 (resident, whole state on chip)");
+    if (value > 0 && s->coef_mode != 0) return fail(s, TEUK_EINVAL, "kernels 1 and 2 need coef_mode 0");
     if (value == 2) {
       if (s->temporal_block == 2) return fail(s, TEUK_EINVAL, "kernel 2 needs temporal_block 1");
       if (!resident_plan(s, &s->res_rows, &s->res_ncta))
         return fail(s, TEUK_EINVAL, "kernel 2 needs n_theta <= 128 and a state that fits in the shared memory of one block per SM");
-      if (s->d_ll) { cudaFree(s->d_ll); s->d_ll = nullptr; }
     }
     if (value == 1 && s->n_theta > 256) return fail(s, TEUK_EINVAL, "kernel 1 needs n_theta <= 256");
     if (value == 1 && s->temporal_block == 2) return fail(s, TEUK_EINVAL, "kernel 1 needs temporal_block 1");
-    s->variant = (int)value;
+    s->kernel_opt = (int)value;
+    s->variant = value < 0 ? 0 : (int)value;
   } else {
     return fail(s, TEUK_EINVAL, "teuk_set_option: unknown key");
   }
@@ -918,9 +938,13 @@ int teuk_get_stat(const teuk_solver* s, const char* key, int64_t* value) {
   else if (!strcmp(key, "launches")) *value = s->launches;
   else if (!strcmp(key, "n_pts")) *value = (int64_t)s->n_modes * s->n_r * s->n_theta;
   else if (!strcmp(key, "state_bytes")) *value = (int64_t)(state_doubles(s) * sizeof(double));
-  else if (!strcmp(key, "kernel")) *value = s->variant;
-  else if (!strcmp(key, "resident_rows")) *value = s->variant == 2 ? s->res_rows : 0;
-  else if (!strcmp(key, "resident_blocks")) *value = s->variant == 2 ? (int64_t)s->res_ncta * s->n_modes : 0;
+  else if (!strcmp(key, "kernel") || !strcmp(key, "resident_rows") || !strcmp(key, "resident_blocks")) {
+    int rr = 0, nc = 0;
+    const bool res = resident_active(s, &rr, &nc);
+    if (!strcmp(key, "kernel")) *value = res ? 2 : s->variant;
+    else if (!strcmp(key, "resident_rows")) *value = res ? rr : 0;
+    else *value = res ? (int64_t)nc * s->n_modes : 0;
+  }
   else if (!strcmp(key, "slab_rows")) {
     const int tb = tb2_active(s) ? 2 : 1;
     const int tuned = tb == 2 ? s->tuned_rows2 : s->tuned_rows;

@@ -86,20 +86,24 @@ def check_pair(res, tol=TOL, need_signal=True):
 SMALL = wl.small_test_configs()
 
 
+# "kernel" 0 = marching kernel, one launch per iteration; 2 = resident kernel, state on chip, one launch per call
+# (what the default -1 picks for grids of this size)
+@pytest.mark.parametrize("kernel", [0, 2])
 @pytest.mark.parametrize("cfg", SMALL, ids=[c.name for c in SMALL])
-def test_one_iteration_random_state(orc, teuk, cfg):
+def test_one_iteration_random_state(orc, teuk, cfg, kernel):
     """All four planes random: every term of Eq. (3)-(4), ghosts, edges and the deposit at once."""
-    res = run_pair(orc, teuk, cfg, 1, initial=wl.random_state(cfg, 100 + cfg.cid))
+    res = run_pair(orc, teuk, cfg, 1, initial=wl.random_state(cfg, 100 + cfg.cid), options={"kernel": kernel})
     check_pair(res, tol=1e-12)
-    res = run_pair(orc, teuk, cfg, 3, initial=wl.random_state(cfg, 200 + cfg.cid))
+    res = run_pair(orc, teuk, cfg, 3, initial=wl.random_state(cfg, 200 + cfg.cid), options={"kernel": kernel})
     check_pair(res, tol=1e-12)
 
 
+@pytest.mark.parametrize("kernel", [0, 2])
 @pytest.mark.parametrize("cfg", SMALL, ids=[c.name for c in SMALL])
-def test_multi_step_parity(orc, teuk, cfg):
+def test_multi_step_parity(orc, teuk, cfg, kernel):
     """The config's own data, source and observers, after its step count."""
     steps = cfg.steps
-    res = run_pair(orc, teuk, cfg, steps)
+    res = run_pair(orc, teuk, cfg, steps, options={"kernel": kernel})
     check_pair(res)
     assert len(res["wg"][0][0]) == steps
 
@@ -147,6 +151,7 @@ def test_graph_and_plain_launches_agree_bitwise(orc, teuk):
     out = []
     for graph, chunks in ((1, [150]), (0, [150]), (1, [1, 70, 33, 46])):
         g = teuk.Solver.from_config(cfg)
+        g.set_option("kernel", 0)
         g.set_option("graph", graph)
         g.set_initial(*wl.random_state(cfg, 3))
         g.set_source(wl.orbit_table(cfg, n_steps=150))
@@ -270,6 +275,78 @@ def test_kernel_variants_agree_bitwise(orc, teuk, n_theta):
     assert rel_l2(out[1][1][1], out[0][1][1]) < 1e-13
 
 
+@pytest.mark.parametrize("n_r,n_theta,modes", [(4, 8, (2,)), (5, 32, (1, 2)), (9, 45, (2,)), (150, 64, (2, -1, 0)),
+                                                (333, 128, (2,)), (700, 100, (3, 2)), (1500, 20, (2,)), (2600, 64, (2,))])
+def test_resident_kernel_is_bitwise_identical(orc, teuk, n_r, n_theta, modes):
+    """kernel 2 (state resident in shared memory, one cooperative launch per teuk_step call, block-to-block row
+    exchange through L2) against kernel 0: same stage arithmetic, so fields AND waveforms must agree bit for bit,
+    for any chunking of the calls, with observers in the first and last cell and the source window crossing
+    block boundaries.  Shapes: fewer rows than SMs, several rows per block, ragged last block, idle lanes."""
+    L = 0.4 * (n_r - 1)
+    cfg = SMALL[3].scaled(name="res%dx%d" % (n_r, n_theta), n_r=n_r, n_theta=n_theta, rs_min=-5.0, rs_max=-5.0 + L,
+                          dt_over_dx=0.004, steps=80, modes=modes, observers=(-5.0, -5.0 + L - 0.01, -5.0 + 0.37 * L))
+    W = wl.observer_weights(cfg)
+    out = []
+    for kernel, chunks in ((0, [77]), (2, [77]), (2, [1, 2, 3, 40, 31]), (-1, [5, 72])):
+        g = teuk.Solver.from_config(cfg)
+        g.set_option("kernel", kernel)
+        assert g.stat("kernel") == (0 if kernel == 0 else 2)
+        g.set_initial(*wl.random_state(cfg, 23))
+        g.set_source(wl.orbit_table(cfg, n_steps=80))
+        for x in cfg.observers:
+            g.add_observer(x, W)
+        for c in chunks:
+            g.step(c)
+        out.append((g.get_state(), [g.extract(x) for x in cfg.observers], g.stat("launches")))
+        g.close()
+    for k in (1, 2, 3):
+        for a, b in zip(out[0][0], out[k][0]):
+            assert np.array_equal(a, b), k
+        for (t0, w0), (t1, w1) in zip(out[0][1], out[k][1]):
+            assert len(t1) == 77 and np.array_equal(t0, t1) and np.array_equal(w0, w1), k
+    assert out[1][2] < out[0][2]          # one launch per call instead of one per iteration
+
+
+def test_resident_kernel_applicability(teuk):
+    """kernel 2 is refused (EINVAL, not a silent fallback) when the state does not fit on chip; the automatic
+    choice then runs kernel 0; an explicit slab length, coef_mode 1 or temporal_block 2 keep kernel 0."""
+    big = wl.CONFIGS[3]
+    g = teuk.Solver.from_config(big)
+    assert g.stat("kernel") == 0 and g.stat("resident_blocks") == 0
+    with pytest.raises(teuk.TeukError) as e:
+        g.set_option("kernel", 2)
+    assert e.value.code == teuk.TEUK_EINVAL
+    g.close()
+    g = teuk.Solver.from_config(wl.CONFIGS[2])
+    assert g.stat("kernel") == 2 and 1 <= g.stat("resident_blocks") <= 148 and g.stat("resident_rows") >= 27
+    g.set_option("slab_rows", 5)
+    assert g.stat("kernel") == 0
+    g.set_option("slab_rows", 0)
+    g.set_option("coef_mode", 1)
+    assert g.stat("kernel") == 0
+    g.set_option("coef_mode", 0)
+    g.set_option("temporal_block", 2)
+    assert g.stat("kernel") == 0
+    with pytest.raises(teuk.TeukError):
+        g.set_option("kernel", 2)
+    g.set_option("temporal_block", 1)
+    g.set_option("kernel", 2)
+    with pytest.raises(teuk.TeukError):
+        g.set_option("coef_mode", 1)
+    with pytest.raises(teuk.TeukError):
+        g.set_option("temporal_block", 2)
+    g.close()
+
+
+def test_resident_kernel_long_run_and_ring_drain(orc, teuk):
+    """More iterations than the device ring holds, in the resident kernel: one launch per ring-full of samples."""
+    cfg = wl.CONFIGS[1].scaled(name="ring2", n_r=24, n_theta=8, rs_min=10.0, rs_max=19.2, steps=40000,
+                               dt_over_dx=0.02, observers=(12.3,))
+    res = run_pair(orc, teuk, cfg, 40000, chunks=[5, 32763, 1, 7231], options={"kernel": 2})
+    check_pair(res, tol=1e-9)
+    assert len(res["wg"][0][0]) == 40000 and res["launches"] < 100
+
+
 @pytest.mark.parametrize("cfg", SMALL, ids=[c.name for c in SMALL])
 def test_smem_kernel_parity(orc, teuk, cfg):
     res = run_pair(orc, teuk, cfg, min(cfg.steps, 300), options={"kernel": 1})
@@ -301,6 +378,7 @@ def test_autotune_does_not_change_results(orc, teuk):
     out = []
     for auto in (1, 0):
         g = teuk.Solver.from_config(cfg)
+        g.set_option("kernel", 0)
         g.set_option("autotune", auto)
         g.set_initial(*wl.random_state(cfg, 17))
         g.set_source(wl.orbit_table(cfg, n_steps=60))
@@ -350,6 +428,8 @@ def test_seeded_fuzz_of_shapes_and_options(orc, teuk):
                 "outer_bc": int(rng.integers(0, 2))}
         if coef_mode:
             opts["coef_mode"] = 1
+        if kernel == 0 and case % 3 == 0:
+            opts["kernel"] = -1                 # the automatic choice (resident kernel where it applies)
         steps = int(rng.integers(1, 6))
         kind = int(rng.integers(0, 3))
         cfg = wl.Config(100 + case, "fuzz%d" % case, a, 1.0, modes, lo, lo + dx * (n_r - 1), n_r, n_theta,
