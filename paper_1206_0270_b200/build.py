@@ -8,10 +8,10 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libteuk.so")
-SOURCES = ["teuk_api.cu", "teuk_step.cu", "teuk_tables.cu"]
-HEADERS = [os.path.join(CSRC, "teuk_internal.h"), os.path.join(CSRC, "teuk_resident.cuh"), os.path.join(HERE, "..", "include", "teuk.h")]
+SOURCES = ["teuk_api.cu", "teuk_step.cu", "teuk_resident.cu", "teuk_tables.cu"]
+HEADERS = [os.path.join(CSRC, "teuk_internal.h"), os.path.join(CSRC, "teuk_stage.cuh"), os.path.join(HERE, "..", "include", "teuk.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared", "--threads", "0"]
+              "-Xcompiler", "-fPIC", "-shared"]
 
 
 def _nvcc() -> str:
@@ -21,21 +21,36 @@ def _nvcc() -> str:
     return "nvcc"
 
 
-def needs_build() -> bool:
-    if not os.path.exists(LIB):
+def _stale(target: str, deps) -> bool:
+    if not os.path.exists(target):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES] + HEADERS
+    t = os.path.getmtime(target)
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def needs_build() -> bool:
+    return _stale(LIB, [os.path.join(CSRC, s) for s in SOURCES] + HEADERS)
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
-    if force or needs_build():
-        tmp = LIB + ".tmp%d" % os.getpid()
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + \
-              [os.path.join(CSRC, s) for s in SOURCES]
-        subprocess.check_call(cmd)
-        os.replace(tmp, LIB)
+    """Compile every stale source to an object (in parallel), then link libteuk.so."""
+    if not (force or needs_build()):
+        return LIB
+    objdir = os.path.join(CSRC, "build")
+    os.makedirs(objdir, exist_ok=True)
+    flags = [f for f in NVCC_FLAGS if f != "-shared"] + (["-Xptxas", "-v"] if verbose else [])
+    jobs, objs = [], []
+    for src in SOURCES:
+        obj = os.path.join(objdir, src.replace(".cu", ".o"))
+        objs.append(obj)
+        if force or _stale(obj, [os.path.join(CSRC, src)] + HEADERS):
+            jobs.append((src, subprocess.Popen([_nvcc()] + flags + ["-c", "-o", obj, os.path.join(CSRC, src)])))
+    failed = [src for src, proc in jobs if proc.wait() != 0]
+    if failed:
+        raise subprocess.CalledProcessError(1, "nvcc -c " + " ".join(failed))
+    tmp = LIB + ".tmp%d" % os.getpid()
+    subprocess.check_call([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp] + objs)
+    os.replace(tmp, LIB)
     return LIB
 
 

@@ -181,7 +181,7 @@ bool tb2_possible(const teuk_solver* s) {
 }
 bool tb2_active(const teuk_solver* s) { return s->temporal_block == 2 && tb2_possible(s); }
 
-// Resident kernel (teuk_resident.cuh): at most one block per SM, every mode split over the same number of
+// Resident kernel (teuk_resident.cu): at most one block per SM, every mode split over the same number of
 // blocks, each block's rows (state + half-step rows) in shared memory.  Returns false if that does not fit.
 bool resident_plan(const teuk_solver* s, int* res_rows, int* ncta) {
   if (s->n_theta > 128 || s->coef_mode != 0 || s->n_modes > s->n_sms) return false;

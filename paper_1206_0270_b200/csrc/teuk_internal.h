@@ -76,7 +76,7 @@ struct StepParams {
   int tap_enable, tap_enable2, n_obs;   // tap_enable2: level n+1 inside a temporal-blocking launch
   long long ring_cap;
   int* nonfinite;
-  // resident kernel ("kernel" = 2, teuk_resident.cuh): iterations per launch, rows of r* per block, tag of the
+  // resident kernel ("kernel" = 2, teuk_resident.cu): iterations per launch, rows of r* per block, tag of the
   // input level in the block-to-block exchange buffer `ll` ([n_modes][blocks][2 sides][2 parities] rows of
   // 16-byte {value.lo, tag, value.hi, tag} elements)
   int n_iter, res_rows;

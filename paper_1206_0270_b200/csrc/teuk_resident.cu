@@ -1,6 +1,6 @@
-// teuk_resident.cuh -- "kernel" = 2: the whole state stays ON CHIP for all iterations of one launch.
-// Included by teuk_step.cu (same translation unit: it reuses lw_stage, the source deposit and the tap, so
-// fields and waveforms are bit-identical to the marching kernels).
+// teuk_resident.cu -- "kernel" = 2: the whole state stays ON CHIP for all iterations of one launch.
+// Same lw_stage, source deposit and tap as the marching kernels (teuk_stage.cuh), so fields and waveforms
+// are bit-identical to theirs.
 //
 // Why: the small grids (BASELINE.json configs 1 and 2: 0.5 and 8.4 MB of state) are not bandwidth-bound.  With
 // one launch per iteration they are bound by the launch rate (2.9 us per iteration) and by the serial march
@@ -8,21 +8,27 @@
 // cooperative launch runs n_iter iterations (Eq. 3-4):
 //   * every block owns a contiguous range of r* rows of one mode and keeps them in shared memory for the
 //     whole launch (HBM is touched at entry and exit only);
-//   * an iteration is two block-wide phases separated by __syncthreads: phase 1 computes the half-step rows
-//     2 u^{n+1/2}_{i+1/2} (Eq. 3) into shared memory, one warp per row, phase 2 the full step (Eq. 4) in
-//     place -- no half-step value is computed twice, and a warp's dependent chain per iteration is two stages
-//     long instead of 2 x (slab length + 1);
+//   * an iteration of a block is a list of 2 rows + 1 row tasks, one warp per task: first the half-step rows
+//     2 u^{n+1/2}_{i+1/2} (Eq. 3) into shared memory, then the full step (Eq. 4) in place -- no half-step value
+//     is computed twice.  Tasks are dealt to the warps round-robin across iterations and wait only for the rows
+//     they read (version counters in shared memory); there is no block-wide barrier in the time loop;
 //   * neighbouring blocks exchange ONE row per side and iteration through L2 with a flag-in-data protocol
 //     (each 16-byte element = {value.lo, tag, value.hi, tag}, tag = iteration number; an element is valid
 //     when both tags match, so no fence and no separate flag round trip is needed).  A block computes and
-//     publishes its two edge rows FIRST in phase 2 and consumes its neighbours' rows LAST in phase 1 of the
-//     next iteration, so the L2 latency (~0.3 us) hides behind the interior rows;
+//     publishes its two edge rows FIRST among the full-step tasks and consumes its neighbours' rows LAST among
+//     the half-step tasks of the next iteration, so the L2 latency (~0.7 us) hides behind the interior rows;
 //   * pole ghosts, radial edges, source deposit and tap-on-read
 //     as in teuk_step_kernel.
 // All blocks must be co-resident (they wait on each other): the launch is cooperative and sized to at most
 // one block per SM; waits are bounded (trap -> sticky TEUK_ECUDA instead of a hung GPU).
-#ifndef TEUK_RESIDENT_CUH_
-#define TEUK_RESIDENT_CUH_
+#include "teuk_stage.cuh"
+
+#ifndef TEUK_RES_FLAG_SLEEP
+#define TEUK_RES_FLAG_SLEEP 0   // ns between two polls of a version counter
+#endif
+#ifndef TEUK_RES_NW
+#define TEUK_RES_NW(V) ((V) == 4 ? 8 : 16)   // warps per block the register budget is cut for
+#endif
 
 namespace {
 
@@ -61,6 +67,24 @@ __device__ __forceinline__ void ll_receive(const uint4* slot, Row<V>& u, unsigne
   }
 }
 
+// Version counters of the rows in shared memory (one int per row): a producer warp writes its row, then lane 0
+// releases the new version; consumer warps acquire it before they read the row.  Bounded like every wait here.
+__device__ __forceinline__ void flag_set(unsigned addr, int v) {
+  asm volatile("st.release.cta.shared.s32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void flag_wait(unsigned addr, int need) {
+  unsigned tries = 0;
+  for (;;) {
+    int v;
+    asm volatile("ld.acquire.cta.shared.s32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    if (__all_sync(FULL, v >= need)) break;
+    if (++tries > (1u << 26)) asm volatile("trap;");
+#if TEUK_RES_FLAG_SLEEP > 0
+    __nanosleep(TEUK_RES_FLAG_SLEEP);
+#endif
+  }
+}
+
 template <int V>
 __device__ __forceinline__ uint4* ll_slot(const StepParams& p, int mode, int ncta, int cta, int side, unsigned tag) {
   return reinterpret_cast<uint4*>(p.ll) + ((((size_t)mode * ncta + cta) * 2 + side) * 2 + (tag & 1u)) * (size_t)(4 * 32 * V);
@@ -94,6 +118,9 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
   double* const sH = sU + (size_t)(p.res_rows + 2) * ROWD;      // [res_rows + 1] half rows: slot h = lo - 1 + h + 1/2
   double* const sE = sH + (size_t)(p.res_rows + 1) * ROWD;      // new outer-edge row (last block)
   double* const sR = sE + ROWD;                                 // r-table records of locations 2 lo - 1 + q
+  int* const sV = reinterpret_cast<int*>(sR + (size_t)(2 * p.res_rows + 2) * RT_N);   // version counters
+  const unsigned verU = smem_u32(sV);                           // [res_rows + 2]: level of row slot r, relative to entry
+  const unsigned verH = verU + 4u * (unsigned)(p.res_rows + 2); // [res_rows + 1]: iterations that wrote half row h
 
   // ---- entry: state rows (with both neighbour rows: they serve iteration 0) and r-table records ----
   for (int r = w; r < rows + 2; r += nw) {
@@ -101,6 +128,7 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
     load_row<V, false>(t, uin + (size_t)(lo - 1 + r) * row_stride, nth, j0);
     sts_row<V>(t, sU + (size_t)r * ROWD, NP, j0);
   }
+  for (int q = threadIdx.x; q < 2 * p.res_rows + 3; q += blockDim.x) sV[q] = 0;
   for (int q = threadIdx.x; q < (2 * rows + 2) * RT_N; q += blockDim.x) {
     const int loc = 2 * lo - 1 + q / RT_N;
     if (loc <= 2 * nr - 2) sR[q] = rtab[(size_t)loc * RT_N + q % RT_N];
@@ -121,26 +149,42 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
   __syncthreads();
 
   const double tau_h = 0.5 * p.dt, tau_f = 0.25 * p.dt, tdx = 2.0 / p.dx;
-  const double src_reach = ((double)p.W + 2.0) * p.dx;   // conservative pre-test of the source window in x
   const long long n0 = *p.d_base + p.k;                  // index of the input level of iteration 0
+  bool cta_taps = false;                                 // does an observer's cell [i0, i0+1] start in this block?
+  for (int q = 0; q < p.n_obs; ++q) cta_taps = cta_taps || (p.obs[q].i0 >= lo - 1 && p.obs[q].i0 <= hi - 1);
 
-  for (int it = 0; it < p.n_iter; ++it) {
+  // Task list of one iteration: T = 2 rows + 1 tasks, first the rows + 1 half-step rows (those that need a
+  // neighbour block's row LAST), then the rows full-step rows (the two edge rows of the block, which are
+  // published, FIRST).  Task g = it * T + t runs on warp g mod nw, so the load rotates over the warps, and
+  // every warp works through its tasks in increasing g.  A task waits for the rows it reads (version counters
+  // in shared memory, release/acquire), never for a block-wide barrier; every dependence points to a smaller g,
+  // so the smallest unfinished task can always run.
+  // Measured on config 2 (28 rows per block, 16 warps): two __syncthreads per iteration 4.08 us per iteration,
+  // this task list 3.63 us; a fixed chunk of rows per warp (no rotation, two hand-overs per warp) 4.6 us: what
+  // counts is the length of the serial chain of tasks per warp, see DESIGN.md 5.1d.
+  const bool has_source = p.has_source != 0;
+  const double src_reach = ((double)p.W + 2.0) * p.dx;   // conservative pre-test of the source window in x
+  const int T = 2 * rows + 1;
+  int it = 0, t = w;
+  while (t >= T) { t -= T; ++it; }
+  while (it < p.n_iter) {
     const long long n = n0 + it;
     const unsigned tag_in = p.tag0 + (unsigned)it;       // tag of the rows published during iteration it - 1
-    const bool do_tap = p.n_obs > 0 && n >= 1 && (it > 0 || p.tap_enable);
-
-    // ---- phase 1: half-step rows (Eq. 3).  Rows that need a neighbour block's row come last. ----
-    for (int t = w; t <= rows; t += nw) {
+    if (t <= rows) {
+      // ---- half-step row (Eq. 3) at i + 1/2 between nodes i and i + 1 ----
       const int h = (t < rows - 1) ? t + 1 : (t == rows - 1 ? 0 : rows);
-      const int i = lo - 1 + h;                          // half point i + 1/2 between nodes i and i + 1
+      const int i = lo - 1 + h;
       Row<V> A, B, Hn;
+      // own rows must be at level `it`; that also says the readers of the old H[h] are done (they wrote them)
+      if (h >= 1) flag_wait(verU + 4u * (unsigned)h, it);
+      if (h + 1 <= rows) flag_wait(verU + 4u * (unsigned)(h + 1), it);
       if (h == 0 && !first && it > 0) ll_receive<V>(ll_slot<V>(p, mode, ncta, cta - 1, 1, tag_in), A, tag_in, lane);
       else lds_row<V>(A, sU + (size_t)h * ROWD, NP, j0, true);
       if (h == rows && !last && it > 0) ll_receive<V>(ll_slot<V>(p, mode, ncta, cta + 1, 0, tag_in), B, tag_in, lane);
       else lds_row<V>(B, sU + (size_t)(h + 1) * ROWD, NP, j0, true);
-      if (do_tap) tap<V>(A, B, p, i, mode, n, lane);
+      if (cta_taps && n >= 1 && (it > 0 || p.tap_enable)) tap<V>(A, B, p, i, mode, n, lane);
       lw_stage<V, true>(A, B, A, sR + (2 * h) * RT_N, th, tau_h, tdx, Hn);
-      if (p.has_source) {
+      if (has_source) {
         const double x = p.rs_min + ((double)i + 0.5) * p.dx;
         if (fabs(x - __ldg(p.xp + 2 * n)) <= src_reach) {
           StageSource<V> s;
@@ -157,9 +201,9 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
 #pragma unroll
         for (int v = 0; v < V; ++v) {
           if (p.outer_bc == 0) {
-            const double b = rsqrt_near_one(fma(-eps, tv.s2[v], 1.0));
-            e.c[0][v] = B.c[0][v] - p.dt * b * (B.c[0][v] - A.c[0][v]) / p.dx;
-            e.c[1][v] = B.c[1][v] - p.dt * b * (B.c[1][v] - A.c[1][v]) / p.dx;
+            const double bb = rsqrt_near_one(fma(-eps, tv.s2[v], 1.0));
+            e.c[0][v] = B.c[0][v] - p.dt * bb * (B.c[0][v] - A.c[0][v]) / p.dx;
+            e.c[1][v] = B.c[1][v] - p.dt * bb * (B.c[1][v] - A.c[1][v]) / p.dx;
           } else {
             e.c[0][v] = 0.0;
             e.c[1][v] = 0.0;
@@ -169,19 +213,22 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
         }
         sts_row<V>(e, sE, NP, j0);
       }
-    }
-    __syncthreads();
-
-    // ---- phase 2: full step in place (Eq. 4).  The two edge rows of the block go first and are published. ----
-    for (int t = w; t < rows; t += nw) {
-      const int r = (t == 0) ? 1 : (t == 1 ? rows : t);
+      __syncwarp();
+      if (lane == 0) flag_set(verH + 4u * (unsigned)h, it + 1);
+    } else {
+      // ---- full-step row in place (Eq. 4) ----
+      const int tt = t - (rows + 1);
+      const int r = (tt == 0) ? 1 : (tt == 1 ? rows : tt);
       const int i = lo - 1 + r;
       Row<V> Hp, Hn, U0, out;
+      // both half-step rows of this iteration exist; their producers were the last readers of the old U[r]
+      flag_wait(verH + 4u * (unsigned)(r - 1), it + 1);
+      flag_wait(verH + 4u * (unsigned)r, it + 1);
       lds_row<V>(Hp, sH + (size_t)(r - 1) * ROWD, NP, j0, true);
       lds_row<V>(Hn, sH + (size_t)r * ROWD, NP, j0, true);
       lds_row<V>(U0, sU + (size_t)r * ROWD, NP, j0, true);
       lw_stage<V, false>(Hp, Hn, U0, sR + (2 * r - 1) * RT_N, th, tau_f, tdx, out);
-      if (p.has_source) {
+      if (has_source) {
         const double x = p.rs_min + (double)i * p.dx;
         if (fabs(x - __ldg(p.xp + 2 * n + 1)) <= src_reach) {
           StageSource<V> s;
@@ -197,19 +244,23 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
       if (first && r == 1) {     // inner radial edge: Phi = Pi = 0
         Row<V> z;
 #pragma unroll
-        for (int c = 0; c < 4; ++c)
+        for (int cc = 0; cc < 4; ++cc)
 #pragma unroll
-          for (int v = 0; v < V; ++v) z.c[c][v] = 0.0;
+          for (int v = 0; v < V; ++v) z.c[cc][v] = 0.0;
         sts_row<V>(z, sU, NP, j0);
       }
-      if (last && r == rows) {   // new outer-edge row, computed from level n in phase 1
+      if (last && r == rows) {   // new outer-edge row, computed from level n with the half-step row h = rows
         Row<V> e;
         lds_row<V>(e, sE, NP, j0, true);
         sts_row<V>(e, sU + (size_t)(rows + 1) * ROWD, NP, j0);
       }
+      __syncwarp();
+      if (lane == 0) flag_set(verU + 4u * (unsigned)r, it + 1);
     }
-    __syncthreads();
+    t += nw;
+    while (t >= T) { t -= T; ++it; }
   }
+  __syncthreads();
 
   // ---- exit: the block's rows of the last level go to the other ping-pong buffer ----
   for (int r = w; r < rows + 2; r += nw) {
@@ -222,13 +273,14 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
 
 // ---- host side ------------------------------------------------------------------------------------
 template <int V>
-constexpr int resident_max_warps() { return V == 4 ? 8 : 16; }
+constexpr int resident_max_warps() { return TEUK_RES_NW(V); }
 
 size_t teuk_resident_smem_bytes(int n_theta, int res_rows) {
   const int v = (n_theta + 31) / 32;
   const int V = v <= 1 ? 1 : (v <= 2 ? 2 : 4);
   const size_t rowd = (size_t)4 * 32 * V;
-  return ((size_t)(2 * res_rows + 4) * rowd + (size_t)(2 * res_rows + 2) * RT_N) * sizeof(double);
+  return ((size_t)(2 * res_rows + 4) * rowd + (size_t)(2 * res_rows + 2) * RT_N) * sizeof(double) +
+         (size_t)(2 * res_rows + 4) * sizeof(int);
 }
 
 // bytes of the exchange buffer: [n_modes][ncta][2 sides][2 parities] rows of 16-byte elements
@@ -253,7 +305,7 @@ static cudaError_t launch_resident_v(const StepParams& p, int ncta, cudaStream_t
     if (e != cudaSuccess) return e;
     attr_set[dev_ & 63] = true;
   }
-  int nwarps = p.res_rows + 1 < NW ? p.res_rows + 1 : NW;
+  const int nwarps = 2 * p.res_rows + 1 < NW ? 2 * p.res_rows + 1 : NW;
   dim3 grid(ncta, p.n_modes), block(32 * nwarps);
   StepParams pc = p;
   void* args[] = {&pc};
@@ -268,4 +320,3 @@ cudaError_t teuk_launch_step_resident(const StepParams& p, int ncta, cudaStream_
   return launch_resident_v<4>(p, ncta, st);
 }
 
-#endif

@@ -33,497 +33,7 @@
 
 #include "teuk_internal.h"
 
-namespace {
-
-constexpr unsigned FULL = 0xffffffffu;
-
-template <int V>
-struct Row {
-  double c[4][V];  // Phi_R, Phi_I, Pi_R, Pi_I for this lane's V columns
-};
-
-#ifndef TEUK_MIN_BLOCKS
-#define TEUK_MIN_BLOCKS 2   // resident blocks for V = 1, 4 (V = 2 always asks for 3); 3 with V = 4 spills: 29 GPts/s
-#endif
-#ifndef TEUK_FAST_RSQRT
-#define TEUK_FAST_RSQRT 1   // own MUFU.RSQ64H + one third-order step instead of CUDA's rsqrt(): +6 GPts/s
-#endif
-#ifndef TEUK_UNROLL2
-#define TEUK_UNROLL2 1      // marching loop body instantiated twice with swapped roles (no register rotation): +3
-#endif
-#ifndef TEUK_SLOTS
-#define TEUK_SLOTS 2    // TMA landing slots per warp (register kernel): rows i+2 .. i+TEUK_SLOTS+1 in flight (3, 4: no gain)
-#endif
-#ifndef TEUK_GROUP
-#define TEUK_GROUP 2    // columns processed "vertically" together inside a stage (ILP)
-#endif
-
-// theta-dependent factors of this lane's V columns (rows of teuk_internal.h TT_*)
-template <int V>
-struct ThetaVals {
-  double s2[V], cs[V], ap[V], am[V], d0[V];
-};
-
-template <int V>
-struct ThetaTab {
-  ThetaVals<V> vals;
-  __device__ __forceinline__ void get(ThetaVals<V>& t) const { t = vals; }
-};
-
-// theta tables read from a block-shared copy [TT_N][n_theta_pad] under lane mapping MAP 1: the two-column
-// piece of lane l starts at column q*64 + 2l, so a warp-wide 16-byte load is bank-conflict free.
-template <int V>
-struct ThetaTabShared {
-  const double* base;   // shared memory, row stride `stride` doubles, zero padded to 32*V columns
-  int stride, lane;
-  __device__ __forceinline__ void get(ThetaVals<V>& t) const {
-    double* dst[TT_N] = {t.s2, t.cs, t.ap, t.am, t.d0};
-#pragma unroll
-    for (int k = 0; k < TT_N; ++k) {
-      if (V == 1) {
-        dst[k][0] = base[k * stride + lane];
-      } else {
-#pragma unroll
-        for (int q = 0; q < V / 2; ++q) {
-          const double2 w = *reinterpret_cast<const double2*>(base + k * stride + q * 64 + 2 * lane);
-          dst[k][2 * q] = w.x;
-          dst[k][2 * q + 1] = w.y;
-        }
-      }
-    }
-  }
-};
-
-// 1/sqrt(x) for x in (0.9, 1]: MUFU.RSQ64H seed (rel. error < 2^-20) + one third-order step
-// y <- y + y e (1/2 + 3/8 e), e = 1 - x y^2  (error ~ e^3): no range checks, no branch.
-__device__ __forceinline__ double rsqrt_near_one(double x);
-__device__ __forceinline__ double rsqrt_near_one_arg(double x) { return rsqrt_near_one(x); }
-__device__ __forceinline__ double rsqrt_near_one(double x) {
-#if TEUK_FAST_RSQRT
-  double y;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  const double e = fma(-x * y, y, 1.0);
-  return fma(y * e, fma(0.375, e, 0.5), y);
-#else
-  return rsqrt(x);
-#endif
-}
-
-// ---- global <-> register rows ---------------------------------------------------------------
-__device__ __forceinline__ void ld256(const double* p, double& a, double& b, double& c, double& d) {
-  asm volatile("ld.global.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];"
-               : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
-}
-__device__ __forceinline__ void st256(double* p, double a, double b, double c, double d) {
-  asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
-}
-
-// VEC: n_theta % V == 0, so a lane's chunk is either fully valid (aligned vector access) or absent.
-template <int V, bool VEC>
-__device__ __forceinline__ void load_row(Row<V>& u, const double* __restrict__ row, int nth, int j0) {
-#pragma unroll
-  for (int c = 0; c < 4; ++c) {
-    const double* p = row + (size_t)c * nth + j0;
-    if (VEC) {
-      if ((unsigned)j0 < (unsigned)nth) {
-        if (V == 1) {
-          u.c[c][0] = __ldcs(p);
-        } else if (V % 4 == 0) {
-#pragma unroll
-          for (int v = 0; v < V; v += 4) ld256(p + v, u.c[c][v], u.c[c][v + 1], u.c[c][v + 2], u.c[c][v + 3]);
-        } else {
-#pragma unroll
-          for (int v = 0; v < V; v += 2) {
-            const double2 t = __ldcs(reinterpret_cast<const double2*>(p + v));
-            u.c[c][v] = t.x;
-            u.c[c][v + 1] = t.y;
-          }
-        }
-      } else {
-#pragma unroll
-        for (int v = 0; v < V; ++v) u.c[c][v] = 0.0;
-      }
-    } else {
-#pragma unroll
-      for (int v = 0; v < V; ++v) u.c[c][v] = ((unsigned)(j0 + v) < (unsigned)nth) ? __ldcs(p + v) : 0.0;
-    }
-  }
-}
-
-// Columns outside [pay_lo, pay_hi) (halo columns of a theta segment, idle lanes) are not stored.
-template <int V, bool VEC>
-__device__ __forceinline__ void store_row(const Row<V>& u, double* __restrict__ row, int nth, int j0, int pay_lo,
-                                          int pay_hi) {
-#pragma unroll
-  for (int c = 0; c < 4; ++c) {
-    double* p = row + (size_t)c * nth + j0;
-    if (VEC) {
-      if (j0 >= pay_lo && j0 < pay_hi) {
-        if (V == 1) {
-          __stcs(p, u.c[c][0]);
-        } else if (V % 4 == 0) {
-#pragma unroll
-          for (int v = 0; v < V; v += 4) st256(p + v, u.c[c][v], u.c[c][v + 1], u.c[c][v + 2], u.c[c][v + 3]);
-        } else {
-#pragma unroll
-          for (int v = 0; v < V; v += 2) __stcs(reinterpret_cast<double2*>(p + v), make_double2(u.c[c][v], u.c[c][v + 1]));
-        }
-      }
-    } else {
-#pragma unroll
-      for (int v = 0; v < V; ++v)
-        if (j0 + v >= pay_lo && j0 + v < pay_hi) __stcs(p + v, u.c[c][v]);
-    }
-  }
-}
-
-// ---- lane <-> column mappings ------------------------------------------------------------------
-// MAP 0 (register-resident kernel): lane owns V contiguous columns j = lane*V + v.
-// MAP 1 (shared-memory-resident kernel): lane owns V/2 two-column pieces, j = (v/2)*64 + 2*lane + (v&1)
-//        (V = 1: j = lane), so a warp-wide 16-byte access touches 512 contiguous bytes: shared-memory
-//        reads are bank-conflict free and global stores are fully coalesced.
-template <int V, int MAP>
-__device__ __forceinline__ int col_of(int lane, int v) {
-  if (MAP == 0 || V == 1) return lane * V + v;
-  return (v >> 1) * 64 + 2 * lane + (v & 1);
-}
-
-// theta-neighbours of f[v] across lanes: lf[v] = f at column-1, rt[v] = f at column+1 (values beyond
-// the poles are garbage-but-finite: their coefficients are zero, see teuk_ttab_kernel).
-template <int V, int MAP>
-__device__ __forceinline__ void theta_neighbours(const double (&f)[V], double (&lf)[V], double (&rt)[V], int lane) {
-  if (MAP == 0 || V == 1) {
-    const double l = __shfl_up_sync(FULL, f[V - 1], 1), r = __shfl_down_sync(FULL, f[0], 1);
-#pragma unroll
-    for (int v = 0; v < V; ++v) {
-      lf[v] = (v > 0) ? f[v > 0 ? v - 1 : 0] : l;
-      rt[v] = (v < V - 1) ? f[v < V - 1 ? v + 1 : 0] : r;
-    }
-  } else {
-    constexpr int NP = V / 2;
-#pragma unroll
-    for (int q = 0; q < NP; ++q) {
-      // right neighbour of (q, lane, 1): (q, lane+1, 0), or (q+1, 0, 0) for lane 31
-      const double send_r = (lane == 0 && q + 1 < NP) ? f[2 * (q + 1 < NP ? q + 1 : q)] : f[2 * q];
-      // left neighbour of (q, lane, 0): (q, lane-1, 1), or (q-1, 31, 1) for lane 0
-      const double send_l = (lane == 31 && q > 0) ? f[2 * (q > 0 ? q - 1 : 0) + 1] : f[2 * q + 1];
-      const double r = __shfl_sync(FULL, send_r, (lane + 1) & 31);
-      const double l = __shfl_sync(FULL, send_l, (lane + 31) & 31);
-      lf[2 * q] = l;
-      lf[2 * q + 1] = f[2 * q];
-      rt[2 * q] = f[2 * q + 1];
-      rt[2 * q + 1] = r;
-    }
-  }
-}
-
-// ---- one Lax-Wendroff stage at one radial location ------------------------------------------
-// HALF: A = u^n_i, B = u^n_{i+1}, out = 2 u^{n+1/2}_{i+1/2}             (Eq. 3, tau = dt/2)
-// else: A = H_{i-1/2}, B = H_{i+1/2} (doubled), out = u^{n+1}_i, base = u^n_i   (Eq. 4, tau = dt/4)
-template <int V, bool HALF, int MAP = 0, class TT = ThetaTab<V>>
-__device__ __forceinline__ void lw_stage(const Row<V>& A, const Row<V>& B, const Row<V>& base,
-                                         const double* __restrict__ rec, const TT& tht,
-                                         double tau, double two_over_dx, Row<V>& out, int lane = 0) {
-  ThetaVals<V> th;
-  tht.get(th);
-  const double2 r01 = *reinterpret_cast<const double2*>(rec + 0);
-  const double2 r23 = *reinterpret_cast<const double2*>(rec + 2);
-  const double2 r45 = *reinterpret_cast<const double2*>(rec + 4);
-  const double2 r67 = *reinterpret_cast<const double2*>(rec + 6);
-  const double2 r89 = *reinterpret_cast<const double2*>(rec + 8);
-  const double eps = r01.x, x32 = r01.y, bre2 = r23.x, bim2 = r23.y;
-  const double a0 = r45.x, a1 = r45.y, a2 = r67.x, g1 = r67.y, gr = r89.x, cl = r89.y;
-
-  double sfr[V], sfi[V];
-#pragma unroll
-  for (int v = 0; v < V; ++v) {
-    sfr[v] = A.c[0][v] + B.c[0][v];
-    sfi[v] = A.c[1][v] + B.c[1][v];
-  }
-  // theta-neighbours across lanes (pole ghosts are folded into ap/am/d0; see teuk_ttab_kernel)
-  double nlr[V], nrr[V], nli[V], nri[V];
-  theta_neighbours<V, MAP>(sfr, nlr, nrr, lane);
-  theta_neighbours<V, MAP>(sfi, nli, nri, lane);
-  // The V columns are processed in groups of G: inside a group every operation is written for all
-  // G columns back to back, so consecutive FP64 instructions are independent (DFMA latency is 8
-  // cycles at one issue per 2 cycles: a lone dependent chain leaves the pipe 3/4 idle).
-  constexpr int G = (TEUK_GROUP < V) ? TEUK_GROUP : V;
-#pragma unroll
-  for (int v0 = 0; v0 < V; v0 += G) {
-    double dfr[G], dfi[G], spr[G], spi[G], dpr[G], dpi[G], b[G], Q[G], b2d[G], aim[G], diag[G], bre[G];
-    double e2r[G], e2i[G], ltr[G], lti[G], br[G], bi[G];
-#define FORG _Pragma("unroll") for (int g = 0; g < G; ++g)
-    FORG b[g] = fma(-eps, th.s2[v0 + g], 1.0);
-    FORG b[g] = rsqrt_near_one_arg(b[g]);
-    FORG { dfr[g] = B.c[0][v0 + g] - A.c[0][v0 + g]; dfi[g] = B.c[1][v0 + g] - A.c[1][v0 + g]; }
-    FORG { spr[g] = A.c[2][v0 + g] + B.c[2][v0 + g]; spi[g] = A.c[3][v0 + g] + B.c[3][v0 + g]; }
-    FORG { dpr[g] = B.c[2][v0 + g] - A.c[2][v0 + g]; dpi[g] = B.c[3][v0 + g] - A.c[3][v0 + g]; }
-    FORG { aim[g] = fma(a2, th.cs[v0 + g], a1); diag[g] = th.d0[v0 + g] - gr; }
-    FORG { Q[g] = b[g] * b[g]; b2d[g] = b[g] * two_over_dx; }
-    FORG bre[g] = fma(-Q[g], th.s2[v0 + g] * x32, bre2);
-    // E2 = 2 (Pi - b dPhi/dx)
-    FORG { e2r[g] = fma(-b2d[g], dfr[g], spr[g]); e2i[g] = fma(-b2d[g], dfi[g], spi[g]); }
-    FORG {
-      out.c[0][v0 + g] = fma(tau, e2r[g], HALF ? sfr[v0 + g] : base.c[0][v0 + g]);
-      out.c[1][v0 + g] = fma(tau, e2i[g], HALF ? sfi[v0 + g] : base.c[1][v0 + g]);
-    }
-    // L'_theta S_Phi
-    FORG { ltr[g] = diag[g] * sfr[v0 + g]; lti[g] = diag[g] * sfi[v0 + g]; }
-    FORG { ltr[g] = fma(th.am[v0 + g], nlr[v0 + g], ltr[g]); lti[g] = fma(th.am[v0 + g], nli[v0 + g], lti[g]); }
-    FORG { ltr[g] = fma(th.ap[v0 + g], nrr[v0 + g], ltr[g]); lti[g] = fma(th.ap[v0 + g], nri[v0 + g], lti[g]); }
-    // bracket B (same order of operations for every G: results do not depend on the grouping)
-    FORG { br[g] = bre[g] * dfr[g]; bi[g] = bre[g] * dfi[g]; }
-    FORG { br[g] = fma(-bim2, dfi[g], br[g]); bi[g] = fma(bim2, dfr[g], bi[g]); }
-    FORG { br[g] = fma(a0, e2r[g], br[g]); bi[g] = fma(a0, e2i[g], bi[g]); }
-    FORG { br[g] = fma(-aim[g], e2i[g], br[g]); bi[g] = fma(aim[g], e2r[g], bi[g]); }
-    FORG { br[g] = fma(cl, ltr[g], br[g]); bi[g] = fma(cl, lti[g], bi[g]); }
-    FORG { br[g] = fma(-g1, sfi[v0 + g], br[g]); bi[g] = fma(g1, sfr[v0 + g], bi[g]); }
-    FORG { br[g] = fma(b2d[g], dpr[g], Q[g] * br[g]); bi[g] = fma(b2d[g], dpi[g], Q[g] * bi[g]); }
-    FORG {
-      out.c[2][v0 + g] = fma(tau, br[g], HALF ? spr[g] : base.c[2][v0 + g]);
-      out.c[3][v0 + g] = fma(tau, bi[g], HALF ? spi[g] : base.c[3][v0 + g]);
-    }
-#undef FORG
-  }
-}
-
-// ---- coef_mode 1: the same stage with the eight 2D coefficient planes STREAMED from HBM ----------
-// (comparison arm for the bytes-vs-flops choice: +128 B per point per iteration, -26 FP64 instructions).
-// `loc` points at this location's [8][n_theta] planes (see teuk_coef2d_kernel); textbook form
-// R = b dPi + kappa dPhi + alpha Pi + gamma Phi + cL L_theta Phi in the scaled variables S, D.
-template <int V, bool HALF, bool VEC>
-__device__ __forceinline__ void lw_stage_planes(const Row<V>& A, const Row<V>& B, const Row<V>& base,
-                                                const double* __restrict__ loc, const ThetaTab<V>& tht, double tau,
-                                                Row<V>& out, int nth, int j0) {
-  ThetaVals<V> th;
-  tht.get(th);
-  double cf[8][V];
-#pragma unroll
-  for (int k = 0; k < 8; ++k) {
-    const double* q = loc + (size_t)k * nth + j0;
-    if (VEC && j0 < nth) {
-      if (V == 1) {
-        cf[k][0] = __ldcs(q);
-      } else if (V % 4 == 0) {
-#pragma unroll
-        for (int v = 0; v < V; v += 4) ld256(q + v, cf[k][v], cf[k][v + 1], cf[k][v + 2], cf[k][v + 3]);
-      } else {
-#pragma unroll
-        for (int v = 0; v < V; v += 2) {
-          const double2 t = __ldcs(reinterpret_cast<const double2*>(q + v));
-          cf[k][v] = t.x;
-          cf[k][v + 1] = t.y;
-        }
-      }
-    } else {
-#pragma unroll
-      for (int v = 0; v < V; ++v) cf[k][v] = (j0 + v < nth) ? __ldcs(q + v) : 0.0;
-    }
-  }
-  double sfr[V], sfi[V];
-#pragma unroll
-  for (int v = 0; v < V; ++v) {
-    sfr[v] = A.c[0][v] + B.c[0][v];
-    sfi[v] = A.c[1][v] + B.c[1][v];
-  }
-  double nlr[V], nrr[V], nli[V], nri[V];
-  theta_neighbours<V, 0>(sfr, nlr, nrr, 0);
-  theta_neighbours<V, 0>(sfi, nli, nri, 0);
-#pragma unroll
-  for (int v = 0; v < V; ++v) {
-    const double dfr = B.c[0][v] - A.c[0][v], dfi = B.c[1][v] - A.c[1][v];
-    const double spr = A.c[2][v] + B.c[2][v], spi = A.c[3][v] + B.c[3][v];
-    const double dpr = B.c[2][v] - A.c[2][v], dpi = B.c[3][v] - A.c[3][v];
-    const double b2d = cf[0][v], kre = cf[1][v], kim = cf[2][v], are = cf[3][v], aim = cf[4][v];
-    const double gre = cf[5][v], gim = cf[6][v], cl = cf[7][v];
-    const double e2r = fma(-b2d, dfr, spr), e2i = fma(-b2d, dfi, spi);
-    out.c[0][v] = fma(tau, e2r, HALF ? sfr[v] : base.c[0][v]);
-    out.c[1][v] = fma(tau, e2i, HALF ? sfi[v] : base.c[1][v]);
-    const double ltr = fma(th.ap[v], nrr[v], fma(th.am[v], nlr[v], th.d0[v] * sfr[v]));
-    const double lti = fma(th.ap[v], nri[v], fma(th.am[v], nli[v], th.d0[v] * sfi[v]));
-    double br = kre * dfr;
-    br = fma(-kim, dfi, br);
-    br = fma(are, spr, br);
-    br = fma(-aim, spi, br);
-    br = fma(cl, ltr, br);
-    br = fma(gre, sfr[v], br);
-    br = fma(-gim, sfi[v], br);
-    br = fma(b2d, dpr, br);
-    double bi = kre * dfi;
-    bi = fma(kim, dfr, bi);
-    bi = fma(are, spi, bi);
-    bi = fma(aim, spr, bi);
-    bi = fma(cl, lti, bi);
-    bi = fma(gre, sfi[v], bi);
-    bi = fma(gim, sfr[v], bi);
-    bi = fma(b2d, dpi, bi);
-    out.c[2][v] = fma(tau, br, HALF ? spr : base.c[2][v]);
-    out.c[3][v] = fma(tau, bi, HALF ? spi : base.c[3][v]);
-  }
-}
-
-// g(y; sigma) = exp(-y^2/(2 sigma^2)) / (sigma sqrt(2 pi))
-__device__ __forceinline__ double gauss_dev(double y, double sigma) {
-  return exp(-y * y / (2.0 * sigma * sigma)) / (sigma * sqrt(2.0 * 3.14159265358979323846264338327950288));
-}
-
-// Deposit profile along one axis at offset y from the particle.  kind 0: the Gaussian above, width = sigma.
-// kind 1 / 2: two-point / four-point discrete delta on a grid of spacing `width`:
-// the interpolation weight of the grid point at distance s = |y|/width, over the spacing.
-__device__ __forceinline__ double deposit_profile(int kind, double y, double width) {
-  if (kind == 0) return gauss_dev(y, width);
-  const double s = fabs(y) / width;
-  if (kind == 1) return s < 1.0 ? (1.0 - s) / width : 0.0;
-  if (s < 1.0) return (1.0 - s) * (1.0 + s) * (2.0 - s) / 2.0 / width;
-  if (s < 2.0) return (1.0 - s) * (2.0 - s) * (3.0 - s) / 6.0 / width;
-  return 0.0;
-}
-
-}  // namespace
-
-namespace {
-
-// Source bookkeeping of one stage for one warp: window test and the theta Gaussian per column.
-template <int V>
-struct StageSource {
-  bool on;          // the window of this stage intersects this slab
-  int ip;           // centre row index (nodes: i, half points: i + 1/2 -> i)
-  double xp, are, aim;
-  double gth[V];    // g(theta_j - theta_p) inside |j - jp| <= W, else 0
-};
-
-template <int V, int MAP = 0>
-__device__ __forceinline__ void setup_source(StageSource<V>& s, const StepParams& p, int mode, long long ks,
-                                             bool half, int row_lo, int row_hi, int lane, int col0 = 0) {
-  s.on = false;
-  if (!p.has_source) return;
-  const double xp = p.xp[ks], thp = p.thp[ks];
-  // identical rounding decisions to the definition: i_p = round((x_p - x_min)/dx [- 1/2]),
-  // j_p = round(theta_p/dtheta - 1/2), round(z) = floor(z + 1/2); division and adds only.
-  const double v = __ddiv_rn(__dsub_rn(xp, p.rs_min), p.dx);
-  const int ip = half ? (int)floor(__dadd_rn(__dsub_rn(v, 0.5), 0.5)) : (int)floor(__dadd_rn(v, 0.5));
-  const int jp = (int)floor(__dadd_rn(__dsub_rn(__ddiv_rn(thp, p.dth), 0.5), 0.5));
-  if (ip + p.W < row_lo || ip - p.W > row_hi) return;
-  s.on = true;
-  s.ip = ip;
-  s.xp = xp;
-  s.are = p.amp_re[(size_t)mode * p.n_samples + ks];
-  s.aim = p.amp_im[(size_t)mode * p.n_samples + ks];
-#pragma unroll
-  for (int q = 0; q < V; ++q) {
-    const int j = col0 + col_of<V, MAP>(lane, q);
-    const double th = __dmul_rn((double)j + 0.5, p.dth);
-    s.gth[q] = ((unsigned)j < (unsigned)p.n_theta && abs(j - jp) <= p.W) ? deposit_profile(p.source_kind, th - thp, p.sigma_th) : 0.0;
-  }
-}
-
-// out.Pi += dt * A' g(x - x_p) g(theta - theta_p) on row `i` of this stage's grid.
-template <int V>
-__device__ __forceinline__ void add_source(Row<V>& out, const StageSource<V>& s, const StepParams& p, int i,
-                                           bool half) {
-  if (!s.on || abs(i - s.ip) > p.W) return;
-  double x = __dadd_rn(p.rs_min, __dmul_rn((double)i, p.dx));
-  if (half) x = __dadd_rn(x, __dmul_rn(0.5, p.dx));
-  const double g = p.dt * deposit_profile(p.source_kind, x - s.xp, p.sigma_r);
-#pragma unroll
-  for (int q = 0; q < V; ++q) {
-    const double gg = g * s.gth[q];
-    out.c[2][q] = fma(s.are, gg, out.c[2][q]);
-    out.c[3][q] = fma(s.aim, gg, out.c[3][q]);
-  }
-}
-
-// Waveform tap of the INPUT state (sample n): w = sum_j W_j [(1-f) Phi_{i0,j} + f Phi_{i0+1,j}].
-template <int V, int MAP = 0>
-__device__ __forceinline__ void tap(const Row<V>& lo, const Row<V>& hi, const StepParams& p, int i, int mode,
-                                    long long n, int lane) {
-  for (int q = 0; q < p.n_obs; ++q) {
-    if (p.obs[q].i0 != i) continue;
-    const double f = p.obs[q].f;
-    double wr = 0.0, wi = 0.0;
-#pragma unroll
-    for (int v = 0; v < V; ++v) {
-      const int j = col_of<V, MAP>(lane, v);
-      const double wt = (j < p.n_theta) ? __ldg(p.obs[q].weights + j) : 0.0;
-      wr = fma(wt, fma(f, hi.c[0][v], (1.0 - f) * lo.c[0][v]), wr);
-      wi = fma(wt, fma(f, hi.c[1][v], (1.0 - f) * lo.c[1][v]), wi);
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      wr += __shfl_xor_sync(FULL, wr, o);
-      wi += __shfl_xor_sync(FULL, wi, o);
-    }
-    if (lane == 0) {
-      const long long slot = (n - 1) % p.ring_cap;
-      double* dst = p.obs[q].ring + ((size_t)slot * p.n_modes + mode) * 2;
-      dst[0] = wr;
-      dst[1] = wi;
-      if (!isfinite(wr) || !isfinite(wi)) *p.nonfinite = 1;
-    }
-  }
-}
-
-}  // namespace
-
-// ---- TMA bulk-copy row prefetch (cp.async.bulk + mbarrier; SASS: UBLKCP) ------------------------
-// One lane of each warp asks the TMA engine for the whole next r* row (4 components x n_theta
-// doubles, contiguous in HBM) into the warp's shared-memory landing slot; the warp keeps computing
-// and picks the row up from shared memory 1.5 marching iterations later.  No registers are tied
-// up by loads in flight.
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void tma_load_row(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-// same operations on precomputed 32-bit shared addresses (keeps the address conversion out of the hot loop)
-__device__ __forceinline__ void tma_load_row_u32(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
-// Bounded spin: try_wait suspends the warp for a hardware time slice per attempt, so 2^22 failed attempts
-// are seconds, far beyond any HBM latency; a row that never arrives (a faulted TMA copy) then becomes a
-// reported CUDA error (trap -> sticky TEUK_ECUDA) instead of a hung GPU.
-__device__ __forceinline__ void mbar_wait_u32(unsigned bar, unsigned parity) {
-  unsigned ok, tries = 0;
-  do {
-    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-    if (!ok && ++tries > (1u << 22)) asm volatile("trap;");
-  } while (!ok);
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
-  mbar_wait_u32(smem_u32(bar), parity);
-}
-
-// shared-memory row (same [comp][n_theta] layout as HBM) -> registers
-template <int V>
-__device__ __forceinline__ void lds_row(Row<V>& u, const double* srow, int comp_stride, int col, bool valid) {
-#pragma unroll
-  for (int c = 0; c < 4; ++c) {
-    if (valid) {
-      const double* q = srow + c * comp_stride + col;
-      if (V == 1) {
-        u.c[c][0] = q[0];
-      } else {
-#pragma unroll
-        for (int v = 0; v < V; v += 2) {
-          const double2 t = *reinterpret_cast<const double2*>(q + v);
-          u.c[c][v] = t.x;
-          u.c[c][v + 1] = t.y;
-        }
-      }
-    } else {
-#pragma unroll
-      for (int v = 0; v < V; ++v) u.c[c][v] = 0.0;
-    }
-  }
-}
+#include "teuk_stage.cuh"
 
 // r-table staging: the 2*RT_CH records (node + half point) of the next RT_CH marching iterations
 // are copied global -> shared with cp.async while the current chunk is being consumed, so the
@@ -1031,22 +541,6 @@ namespace {
 #endif
 constexpr int TB_RING = TEUK_TB_RING;
 
-template <int V>
-__device__ __forceinline__ void sts_row(const Row<V>& u, double* srow, int nth, int j0) {
-#pragma unroll
-  for (int c = 0; c < 4; ++c) {
-    if (j0 < nth) {
-      double* q = srow + c * nth + j0;
-      if (V == 1) {
-        q[0] = u.c[c][0];
-      } else {
-#pragma unroll
-        for (int v = 0; v < V; v += 2) *reinterpret_cast<double2*>(q + v) = make_double2(u.c[c][v], u.c[c][v + 1]);
-      }
-    }
-  }
-}
-
 __device__ __forceinline__ void mbar_arrive_u32(unsigned bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
@@ -1337,8 +831,6 @@ __global__ void teuk_unpack_kernel(const double* __restrict__ u, Planes dst, siz
   for (int c = 0; c < 4; ++c)
     if (dst.c[c]) dst.c[c][t] = u[(row * 4 + c) * nth + j];
 }
-
-#include "teuk_resident.cuh"
 
 // ---- host-side launchers (called from teuk_api.cu) -------------------------------------------
 template <int V>
