@@ -138,7 +138,10 @@ int teuk_get_state(teuk_solver *s, double *phi_re, double *phi_im, double *pi_re
  *                   shared memory of one block per SM (about n_modes*n_r*n_theta <= 5e5 points), else EINVAL.
  *                   All kernels do the same arithmetic per point: fields are bitwise identical (waveforms too,
  *                   except kernel 1, which sums over theta in another order).  An explicit "slab_rows" makes the
- *                   automatic choice stay with kernel 0. */
+ *                   automatic choice stay with kernel 0.
+ *   "resident_cache" 1 (default) = kernel 2 also keeps the time-independent coefficients b, b^2 and Re beta' of its
+ *                   rows in shared memory when they fit (3 doubles per point and location), 0 = it rebuilds them
+ *                   in every stage like kernel 0.  Same results bit for bit. */
 int teuk_set_option(teuk_solver *s, const char *key, int64_t value);
 
 /* Read-only counters: "steps" (iterations done), "launches" (kernels launched so far),

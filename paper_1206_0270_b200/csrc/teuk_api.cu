@@ -21,7 +21,7 @@ cudaError_t teuk_launch_coef2d(double* c2d, const double* rtab, const double* tt
 cudaError_t teuk_launch_step(const StepParams& p, cudaStream_t st);
 cudaError_t teuk_launch_step_tb2(const StepParams& p, cudaStream_t st);
 cudaError_t teuk_launch_step_resident(const StepParams& p, int ncta, cudaStream_t st);
-size_t teuk_resident_smem_bytes(int n_theta, int res_rows);
+size_t teuk_resident_smem_bytes(int n_theta, int res_rows, int coef_cache);
 size_t teuk_resident_ll_bytes(int n_theta, int n_modes, int ncta);
 cudaError_t teuk_launch_flush_tap(const StepParams& p, cudaStream_t st);
 cudaError_t teuk_launch_bump(long long* d_base, long long inc, cudaStream_t st);
@@ -67,6 +67,7 @@ struct teuk_solver {
   int tuned_rows2;       // autotuned slab length of the temporal-blocking kernel
   // resident kernel ("kernel" = 2): rows per block, blocks per mode, exchange buffer and its running tag
   int kernel_opt;        // "kernel" option: -1 = automatic (resident kernel when the state fits on chip, else kernel 0)
+  int res_cache_opt;     // "resident_cache" option: keep the time-independent coefficients on chip when they fit
   int res_failed;        // automatic choice: a cooperative launch was refused once, stay with kernel 0
   int res_rows, res_ncta, smem_optin;
   void* d_ll;
@@ -189,7 +190,7 @@ bool resident_plan(const teuk_solver* s, int* res_rows, int* ncta) {
   int per_mode = s->n_sms / s->n_modes;
   if (per_mode > interior) per_mode = interior;
   const int rows = (interior + per_mode - 1) / per_mode;
-  if (teuk_resident_smem_bytes(s->n_theta, rows) > (size_t)s->smem_optin) return false;
+  if (teuk_resident_smem_bytes(s->n_theta, rows, 0) > (size_t)s->smem_optin) return false;
   *res_rows = rows;
   *ncta = (interior + rows - 1) / rows;
   return true;
@@ -402,6 +403,7 @@ int teuk_create(teuk_solver** out, double a, double M, const int32_t* m, int32_t
   for (int q = 0; q < n_modes; ++q) s->m[q] = m[q];
   s->outer_bc = 0; s->coef_mode = 0; s->slab_rows_opt = 0; s->use_graph = 1; s->autotune = 1; s->tuned_rows = 0; s->temporal_block = 1; s->tuned_rows2 = 0;
   s->kernel_opt = -1;
+  s->res_cache_opt = 1;
   s->device = dev;
   if (cudaDeviceGetAttribute(&s->n_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) s->n_sms = 148;
   if (cudaDeviceGetAttribute(&s->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) s->smem_optin = 0;
@@ -659,6 +661,7 @@ int run_chunk(teuk_solver* s, long long c) {
       fill_params(s, &p, s->cur, (int)(s->step - s->base_on_device), 0);   // level s->step was tapped by the last flush
       p.n_iter = (int)m;
       p.res_rows = s->res_rows;
+      p.res_cache = s->res_cache_opt && teuk_resident_smem_bytes(s->n_theta, s->res_rows, 1) <= (size_t)s->smem_optin;
       p.tag0 = s->ll_tag;
       p.ll = s->d_ll;
       const cudaError_t el = teuk_launch_step_resident(p, s->res_ncta, s->stream);
@@ -902,6 +905,8 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
     s->slab_rows_opt = (int)value;
   } else if (!strcmp(key, "graph")) {
     s->use_graph = value ? 1 : 0;
+  } else if (!strcmp(key, "resident_cache")) {
+    s->res_cache_opt = value ? 1 : 0;
   } else if (!strcmp(key, "autotune")) {
     s->autotune = value ? 1 : 0;
   } else if (!strcmp(key, "temporal_block")) {

@@ -79,7 +79,7 @@ struct StepParams {
   // resident kernel ("kernel" = 2, teuk_resident.cu): iterations per launch, rows of r* per block, tag of the
   // input level in the block-to-block exchange buffer `ll` ([n_modes][blocks][2 sides][2 parities] rows of
   // 16-byte {value.lo, tag, value.hi, tag} elements)
-  int n_iter, res_rows;
+  int n_iter, res_rows, res_cache;   // res_cache: time-independent coefficients kept in shared memory
   unsigned tag0;
   void* ll;
   ObsDev obs[TEUK_MAX_OBS];

@@ -21,6 +21,8 @@
 //     as in teuk_step_kernel.
 // All blocks must be co-resident (they wait on each other): the launch is cooperative and sized to at most
 // one block per SM; waits are bounded (trap -> sticky TEUK_ECUDA instead of a hung GPU).
+#include <type_traits>
+
 #include "teuk_stage.cuh"
 
 #ifndef TEUK_RES_FLAG_SLEEP
@@ -94,7 +96,9 @@ __device__ __forceinline__ uint4* ll_slot(const StepParams& p, int mode, int nct
 
 // NW = warps per block the register budget allows (65536 / (32 NW) registers per thread); the launch may use
 // fewer (blockDim.x / 32 = min(NW, rows + 1)).
-template <int V, int NW>
+// CC: the time-independent coefficients b2d, Q, Re beta^' of every location of the block are kept in shared memory
+// (3 doubles per point and location) when there is room; else they are rebuilt in every stage as in kernel 0.
+template <int V, int NW, bool CC>
 __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __grid_constant__ StepParams p) {
   constexpr int NP = 32 * V;        // padded row width in shared memory (columns >= n_theta stay zero)
   constexpr int ROWD = 4 * NP;      // doubles per row
@@ -119,6 +123,8 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
   double* const sE = sH + (size_t)(p.res_rows + 1) * ROWD;      // new outer-edge row (last block)
   double* const sR = sE + ROWD;                                 // r-table records of locations 2 lo - 1 + q
   int* const sV = reinterpret_cast<int*>(sR + (size_t)(2 * p.res_rows + 2) * RT_N);   // version counters
+  // coefficient cache: location 2 lo - 1 + q at sC + q * 3 NP, planes b2d, Q, bre (16-byte aligned)
+  double* const sC = reinterpret_cast<double*>(sV + ((2 * p.res_rows + 3 + 3) & ~3));
   const unsigned verU = smem_u32(sV);                           // [res_rows + 2]: level of row slot r, relative to entry
   const unsigned verH = verU + 4u * (unsigned)(p.res_rows + 2); // [res_rows + 1]: iterations that wrote half row h
 
@@ -149,6 +155,37 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
   __syncthreads();
 
   const double tau_h = 0.5 * p.dt, tau_f = 0.25 * p.dt, tdx = 2.0 / p.dx;
+  if (CC) {
+    for (int q = w; q < 2 * rows + 1; q += nw) {
+      double b2d[V], Q[V], bre[V];
+      lw_stage_coefficients<V>(sR + q * RT_N, th.vals, tdx, b2d, Q, bre);
+#pragma unroll
+      for (int v = 0; v < V; ++v) {
+        sC[(size_t)q * 3 * NP + j0 + v] = b2d[v];
+        sC[(size_t)q * 3 * NP + NP + j0 + v] = Q[v];
+        sC[(size_t)q * 3 * NP + 2 * NP + j0 + v] = bre[v];
+      }
+    }
+    __syncthreads();
+  }
+  // one stage at the location with record index q (2 h: half point h + 1/2; 2 r - 1: node r)
+  auto stage = [&](auto half_tag, const Row<V>& A, const Row<V>& B, const Row<V>& base, const int q, const double tau,
+                   Row<V>& out) {
+    constexpr bool HALF = decltype(half_tag)::value;
+    if (CC) {
+      double b2d[V], Q[V], bre[V];
+      const double* cq = sC + (size_t)q * 3 * NP + j0;
+#pragma unroll
+      for (int v = 0; v < V; ++v) {
+        b2d[v] = cq[v];
+        Q[v] = cq[NP + v];
+        bre[v] = cq[2 * NP + v];
+      }
+      lw_stage_cached<V, HALF>(A, B, base, sR + q * RT_N, th, b2d, Q, bre, tau, out);
+    } else {
+      lw_stage<V, HALF>(A, B, base, sR + q * RT_N, th, tau, tdx, out);
+    }
+  };
   const long long n0 = *p.d_base + p.k;                  // index of the input level of iteration 0
   bool cta_taps = false;                                 // does an observer's cell [i0, i0+1] start in this block?
   for (int q = 0; q < p.n_obs; ++q) cta_taps = cta_taps || (p.obs[q].i0 >= lo - 1 && p.obs[q].i0 <= hi - 1);
@@ -183,7 +220,7 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
       if (h == rows && !last && it > 0) ll_receive<V>(ll_slot<V>(p, mode, ncta, cta + 1, 0, tag_in), B, tag_in, lane);
       else lds_row<V>(B, sU + (size_t)(h + 1) * ROWD, NP, j0, true);
       if (cta_taps && n >= 1 && (it > 0 || p.tap_enable)) tap<V>(A, B, p, i, mode, n, lane);
-      lw_stage<V, true>(A, B, A, sR + (2 * h) * RT_N, th, tau_h, tdx, Hn);
+      stage(std::true_type(), A, B, A, 2 * h, tau_h, Hn);
       if (has_source) {
         const double x = p.rs_min + ((double)i + 0.5) * p.dx;
         if (fabs(x - __ldg(p.xp + 2 * n)) <= src_reach) {
@@ -227,7 +264,7 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
       lds_row<V>(Hp, sH + (size_t)(r - 1) * ROWD, NP, j0, true);
       lds_row<V>(Hn, sH + (size_t)r * ROWD, NP, j0, true);
       lds_row<V>(U0, sU + (size_t)r * ROWD, NP, j0, true);
-      lw_stage<V, false>(Hp, Hn, U0, sR + (2 * r - 1) * RT_N, th, tau_f, tdx, out);
+      stage(std::false_type(), Hp, Hn, U0, 2 * r - 1, tau_f, out);
       if (has_source) {
         const double x = p.rs_min + (double)i * p.dx;
         if (fabs(x - __ldg(p.xp + 2 * n + 1)) <= src_reach) {
@@ -275,12 +312,14 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
 template <int V>
 constexpr int resident_max_warps() { return TEUK_RES_NW(V); }
 
-size_t teuk_resident_smem_bytes(int n_theta, int res_rows) {
+size_t teuk_resident_smem_bytes(int n_theta, int res_rows, int coef_cache) {
   const int v = (n_theta + 31) / 32;
   const int V = v <= 1 ? 1 : (v <= 2 ? 2 : 4);
   const size_t rowd = (size_t)4 * 32 * V;
-  return ((size_t)(2 * res_rows + 4) * rowd + (size_t)(2 * res_rows + 2) * RT_N) * sizeof(double) +
-         (size_t)(2 * res_rows + 4) * sizeof(int);
+  size_t bytes = ((size_t)(2 * res_rows + 4) * rowd + (size_t)(2 * res_rows + 2) * RT_N) * sizeof(double) +
+                 (size_t)((2 * res_rows + 3 + 3) & ~3) * sizeof(int);
+  if (coef_cache) bytes += (size_t)(2 * res_rows + 1) * 3 * 32 * V * sizeof(double);
+  return bytes;
 }
 
 // bytes of the exchange buffer: [n_modes][ncta][2 sides][2 parities] rows of 16-byte elements
@@ -290,10 +329,10 @@ size_t teuk_resident_ll_bytes(int n_theta, int n_modes, int ncta) {
   return (size_t)n_modes * ncta * 4 * (4 * 32 * V) * 16;
 }
 
-template <int V>
+template <int V, bool CC>
 static cudaError_t launch_resident_v(const StepParams& p, int ncta, cudaStream_t st) {
   constexpr int NW = resident_max_warps<V>();
-  const size_t dyn = teuk_resident_smem_bytes(p.n_theta, p.res_rows);
+  const size_t dyn = teuk_resident_smem_bytes(p.n_theta, p.res_rows, CC ? 1 : 0);
   static bool attr_set[64] = {false};   // per device
   int dev_ = 0;
   cudaGetDevice(&dev_);
@@ -301,7 +340,7 @@ static cudaError_t launch_resident_v(const StepParams& p, int ncta, cudaStream_t
     int optin = 0;
     cudaError_t e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev_);
     if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(teuk_step_resident_kernel<V, NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+      e = cudaFuncSetAttribute(teuk_step_resident_kernel<V, NW, CC>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
     if (e != cudaSuccess) return e;
     attr_set[dev_ & 63] = true;
   }
@@ -309,14 +348,19 @@ static cudaError_t launch_resident_v(const StepParams& p, int ncta, cudaStream_t
   dim3 grid(ncta, p.n_modes), block(32 * nwarps);
   StepParams pc = p;
   void* args[] = {&pc};
-  return cudaLaunchCooperativeKernel((const void*)teuk_step_resident_kernel<V, NW>, grid, block, args, dyn, st);
+  return cudaLaunchCooperativeKernel((const void*)teuk_step_resident_kernel<V, NW, CC>, grid, block, args, dyn, st);
 }
 
 // n_iter iterations in one cooperative launch; the caller sized res_rows / ncta so that the state fits.
 cudaError_t teuk_launch_step_resident(const StepParams& p, int ncta, cudaStream_t st) {
   const int v = (p.n_theta + 31) / 32;
-  if (v <= 1) return launch_resident_v<1>(p, ncta, st);
-  if (v <= 2) return launch_resident_v<2>(p, ncta, st);
-  return launch_resident_v<4>(p, ncta, st);
+  if (p.res_cache) {
+    if (v <= 1) return launch_resident_v<1, true>(p, ncta, st);
+    if (v <= 2) return launch_resident_v<2, true>(p, ncta, st);
+    return launch_resident_v<4, true>(p, ncta, st);
+  }
+  if (v <= 1) return launch_resident_v<1, false>(p, ncta, st);
+  if (v <= 2) return launch_resident_v<2, false>(p, ncta, st);
+  return launch_resident_v<4, false>(p, ncta, st);
 }
 

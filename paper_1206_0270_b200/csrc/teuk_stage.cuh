@@ -266,6 +266,81 @@ __device__ __forceinline__ void lw_stage(const Row<V>& A, const Row<V>& B, const
   }
 }
 
+// The time-independent part of lw_stage for one location and this lane's V columns: b2d = (2/dx) b, Q = b^2 and
+// Re beta^' = Re beta^ - Q s^2 X3, by the SAME operations in the same order as lw_stage, so that a kernel which
+// keeps them (the resident kernel caches them in shared memory) reproduces lw_stage bit for bit.
+template <int V>
+__device__ __forceinline__ void lw_stage_coefficients(const double* __restrict__ rec, const ThetaVals<V>& th,
+                                                      double two_over_dx, double (&b2d)[V], double (&Q)[V],
+                                                      double (&bre)[V]) {
+  const double eps = rec[RT_EPS], x32 = rec[RT_X32], bre2 = rec[RT_BRE];
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    double b = fma(-eps, th.s2[v], 1.0);
+    b = rsqrt_near_one_arg(b);
+    Q[v] = b * b;
+    b2d[v] = b * two_over_dx;
+    bre[v] = fma(-Q[v], th.s2[v] * x32, bre2);
+  }
+}
+
+// lw_stage with b2d, Q, Re beta^' given (see lw_stage_coefficients): 12 of the 49 FP64 instructions per point
+// and the rsqrt chain at the head of the stage are gone; everything else is lw_stage, operation for operation.
+template <int V, bool HALF>
+__device__ __forceinline__ void lw_stage_cached(const Row<V>& A, const Row<V>& B, const Row<V>& base,
+                                                const double* __restrict__ rec, const ThetaTab<V>& tht,
+                                                const double (&b2d)[V], const double (&Q)[V], const double (&bre)[V],
+                                                double tau, Row<V>& out) {
+  ThetaVals<V> th;
+  tht.get(th);
+  const double2 r23 = *reinterpret_cast<const double2*>(rec + 2);
+  const double2 r45 = *reinterpret_cast<const double2*>(rec + 4);
+  const double2 r67 = *reinterpret_cast<const double2*>(rec + 6);
+  const double2 r89 = *reinterpret_cast<const double2*>(rec + 8);
+  const double bim2 = r23.y;
+  const double a0 = r45.x, a1 = r45.y, a2 = r67.x, g1 = r67.y, gr = r89.x, cl = r89.y;
+  double sfr[V], sfi[V];
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    sfr[v] = A.c[0][v] + B.c[0][v];
+    sfi[v] = A.c[1][v] + B.c[1][v];
+  }
+  double nlr[V], nrr[V], nli[V], nri[V];
+  theta_neighbours<V, 0>(sfr, nlr, nrr, 0);
+  theta_neighbours<V, 0>(sfi, nli, nri, 0);
+  constexpr int G = (TEUK_GROUP < V) ? TEUK_GROUP : V;
+#pragma unroll
+  for (int v0 = 0; v0 < V; v0 += G) {
+    double dfr[G], dfi[G], spr[G], spi[G], dpr[G], dpi[G], aim[G], diag[G];
+    double e2r[G], e2i[G], ltr[G], lti[G], br[G], bi[G];
+#define FORG _Pragma("unroll") for (int g = 0; g < G; ++g)
+    FORG { dfr[g] = B.c[0][v0 + g] - A.c[0][v0 + g]; dfi[g] = B.c[1][v0 + g] - A.c[1][v0 + g]; }
+    FORG { spr[g] = A.c[2][v0 + g] + B.c[2][v0 + g]; spi[g] = A.c[3][v0 + g] + B.c[3][v0 + g]; }
+    FORG { dpr[g] = B.c[2][v0 + g] - A.c[2][v0 + g]; dpi[g] = B.c[3][v0 + g] - A.c[3][v0 + g]; }
+    FORG { aim[g] = fma(a2, th.cs[v0 + g], a1); diag[g] = th.d0[v0 + g] - gr; }
+    FORG { e2r[g] = fma(-b2d[v0 + g], dfr[g], spr[g]); e2i[g] = fma(-b2d[v0 + g], dfi[g], spi[g]); }
+    FORG {
+      out.c[0][v0 + g] = fma(tau, e2r[g], HALF ? sfr[v0 + g] : base.c[0][v0 + g]);
+      out.c[1][v0 + g] = fma(tau, e2i[g], HALF ? sfi[v0 + g] : base.c[1][v0 + g]);
+    }
+    FORG { ltr[g] = diag[g] * sfr[v0 + g]; lti[g] = diag[g] * sfi[v0 + g]; }
+    FORG { ltr[g] = fma(th.am[v0 + g], nlr[v0 + g], ltr[g]); lti[g] = fma(th.am[v0 + g], nli[v0 + g], lti[g]); }
+    FORG { ltr[g] = fma(th.ap[v0 + g], nrr[v0 + g], ltr[g]); lti[g] = fma(th.ap[v0 + g], nri[v0 + g], lti[g]); }
+    FORG { br[g] = bre[v0 + g] * dfr[g]; bi[g] = bre[v0 + g] * dfi[g]; }
+    FORG { br[g] = fma(-bim2, dfi[g], br[g]); bi[g] = fma(bim2, dfr[g], bi[g]); }
+    FORG { br[g] = fma(a0, e2r[g], br[g]); bi[g] = fma(a0, e2i[g], bi[g]); }
+    FORG { br[g] = fma(-aim[g], e2i[g], br[g]); bi[g] = fma(aim[g], e2r[g], bi[g]); }
+    FORG { br[g] = fma(cl, ltr[g], br[g]); bi[g] = fma(cl, lti[g], bi[g]); }
+    FORG { br[g] = fma(-g1, sfi[v0 + g], br[g]); bi[g] = fma(g1, sfr[v0 + g], bi[g]); }
+    FORG { br[g] = fma(b2d[v0 + g], dpr[g], Q[v0 + g] * br[g]); bi[g] = fma(b2d[v0 + g], dpi[g], Q[v0 + g] * bi[g]); }
+    FORG {
+      out.c[2][v0 + g] = fma(tau, br[g], HALF ? spr[g] : base.c[2][v0 + g]);
+      out.c[3][v0 + g] = fma(tau, bi[g], HALF ? spi[g] : base.c[3][v0 + g]);
+    }
+#undef FORG
+  }
+}
+
 // ---- coef_mode 1: the same stage with the eight 2D coefficient planes STREAMED from HBM ----------
 // (comparison arm for the bytes-vs-flops choice: +128 B per point per iteration, -26 FP64 instructions).
 // `loc` points at this location's [8][n_theta] planes (see teuk_coef2d_kernel); textbook form

@@ -287,9 +287,10 @@ def test_resident_kernel_is_bitwise_identical(orc, teuk, n_r, n_theta, modes):
                           dt_over_dx=0.004, steps=80, modes=modes, observers=(-5.0, -5.0 + L - 0.01, -5.0 + 0.37 * L))
     W = wl.observer_weights(cfg)
     out = []
-    for kernel, chunks in ((0, [77]), (2, [77]), (2, [1, 2, 3, 40, 31]), (-1, [5, 72])):
+    for kernel, chunks, cache in ((0, [77], 1), (2, [77], 1), (2, [1, 2, 3, 40, 31], 0), (-1, [5, 72], 1)):
         g = teuk.Solver.from_config(cfg)
         g.set_option("kernel", kernel)
+        g.set_option("resident_cache", cache)     # time-independent coefficients kept in shared memory, or rebuilt
         assert g.stat("kernel") == (0 if kernel == 0 else 2)
         g.set_initial(*wl.random_state(cfg, 23))
         g.set_source(wl.orbit_table(cfg, n_steps=80))
