@@ -200,6 +200,7 @@ def main():
     ap.add_argument("--coef-mode", type=int, default=0, help="0 rebuild coefficients (default), 1 stream 2D planes")
     ap.add_argument("--source-kind", type=int, default=0, help="0 Gaussian deposit (the configs'), 1 / 2 discrete delta")
     ap.add_argument("--temporal-block", type=int, default=0, help="0 library default, 1 or 2 iterations per HBM round trip")
+    ap.add_argument("--pdl", type=int, default=-1, help="-1 library default, 0/1 programmatic dependent launch inside graph batches")
     ap.add_argument("--kernel", type=int, default=-1, help="-1 library default (automatic), 0 marching kernel, 1 smem-resident marching kernel, 2 resident (state on chip)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -240,6 +241,8 @@ def main():
             g.set_option("slab_rows", args.slab_rows)
         if args.kernel >= 0:
             g.set_option("kernel", args.kernel)
+        if args.pdl >= 0:
+            g.set_option("pdl", args.pdl)
         if args.coef_mode:
             g.set_option("coef_mode", args.coef_mode)
         if args.temporal_block:

@@ -67,6 +67,7 @@ struct teuk_solver {
   int tuned_rows2;       // autotuned slab length of the temporal-blocking kernel
   // resident kernel ("kernel" = 2): rows per block, blocks per mode, exchange buffer and its running tag
   int kernel_opt;        // "kernel" option: -1 = automatic (resident kernel when the state fits on chip, else kernel 0)
+  int use_pdl;           // "pdl" option: programmatic dependent launch inside CUDA-graph batches
   int res_cache_opt;     // "resident_cache" option: keep the time-independent coefficients on chip when they fit
   int res_failed;        // automatic choice: a cooperative launch was refused once, stay with kernel 0
   int res_rows, res_ncta, smem_optin;
@@ -404,6 +405,7 @@ int teuk_create(teuk_solver** out, double a, double M, const int32_t* m, int32_t
   s->outer_bc = 0; s->coef_mode = 0; s->slab_rows_opt = 0; s->use_graph = 1; s->autotune = 1; s->tuned_rows = 0; s->temporal_block = 1; s->tuned_rows2 = 0;
   s->kernel_opt = -1;
   s->res_cache_opt = 1;
+  s->use_pdl = 1;
   s->device = dev;
   if (cudaDeviceGetAttribute(&s->n_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) s->n_sms = 148;
   if (cudaDeviceGetAttribute(&s->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) s->smem_optin = 0;
@@ -545,6 +547,8 @@ int build_graph(teuk_solver* s, int tb) {
     for (int k = 0; k < kGraphBatch && e == cudaSuccess; ++k) {
       StepParams p;
       fill_params(s, &p, s->cur ^ (k & 1), k, sep_tap ? 0 : 1);
+      // iterations 2..32 of the batch follow another step kernel directly: their prologue may overlap its tail
+      p.pdl = (s->use_pdl && k > 0 && !sep_tap && s->variant == 0) ? 1 : 0;
       e = teuk_launch_step(p, s->own_stream);
       if (sep_tap && e == cudaSuccess) {
         fill_params(s, &p, s->cur ^ ((k + 1) & 1), k + 1, 1);
@@ -905,6 +909,8 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
     s->slab_rows_opt = (int)value;
   } else if (!strcmp(key, "graph")) {
     s->use_graph = value ? 1 : 0;
+  } else if (!strcmp(key, "pdl")) {
+    s->use_pdl = value ? 1 : 0;
   } else if (!strcmp(key, "resident_cache")) {
     s->res_cache_opt = value ? 1 : 0;
   } else if (!strcmp(key, "autotune")) {

@@ -60,6 +60,7 @@ struct StepParams {
   int n_r, n_theta, n_modes;
   int slab_rows, n_slabs;
   int n_seg, seg_payload; // theta segments (register kernel, n_theta > 128): count and payload columns each
+  int pdl;                // host side only: launch teuk_step_kernel as a programmatic dependent of the previous launch
   int variant;            // 0 = register-resident kernel, 1 = shared-memory-resident kernel, 2 = resident (on-chip) kernel
   int outer_bc;
   double dt, dx, rs_min, dth;

@@ -87,7 +87,6 @@ __global__ void __launch_bounds__(128, (V == 2 ? 3 : TEUK_MIN_BLOCKS)) teuk_step
   const double* __restrict__ uin = p.uin + (size_t)mode * nr * row_stride;
   double* __restrict__ uout = p.uout + (size_t)mode * nr * row_stride;
   const double* __restrict__ rtab = p.rtab + (size_t)mode * (2 * nr - 1) * RT_N;
-  const long long n = *p.d_base + p.k;               // index of the input time level
   __shared__ __align__(16) double s_rt[4][2][RT_CHUNK_DOUBLES];
   constexpr int NS = TEUK_SLOTS;
   __shared__ __align__(8) unsigned long long s_bar[4][NS];
@@ -118,6 +117,15 @@ __global__ void __launch_bounds__(128, (V == 2 ? 3 : TEUK_MIN_BLOCKS)) teuk_step
                      "r"(smem_u32(&bars[q % NS])) : "memory");
     }
   };
+  // Programmatic dependent launch: when the host launched this grid with the stream-serialisation attribute
+  // (iterations 2..32 of a CUDA-graph batch), everything above -- index arithmetic and the first r-table chunk,
+  // which no kernel of the loop writes -- ran while the previous iteration was still finishing.  From here on the
+  // previous iteration's output (our input) is read and its input (our output) overwritten: wait for it, and let
+  // the next iteration's grid start its own prologue as soon as SM slots free up.  (Without the attribute both
+  // instructions do nothing.)
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const long long n = *p.d_base + p.k;               // index of the input time level
   if (VEC) {
     if (lane == 0) {
 #pragma unroll
@@ -851,6 +859,16 @@ static cudaError_t launch_v(const StepParams& p, cudaStream_t st) {
       if (e != cudaSuccess) return e;                                                                        \
       attr_set[dev_ & 63] = true;                                                                            \
     }                                                                                                        \
+    if (p.pdl) {                                                                                             \
+      cudaLaunchAttribute at_[1];                                                                            \
+      at_[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;                                        \
+      at_[0].val.programmaticStreamSerializationAllowed = 1;                                                 \
+      cudaLaunchConfig_t lc_ = {};                                                                           \
+      lc_.gridDim = grid; lc_.blockDim = block; lc_.dynamicSmemBytes = dyn; lc_.stream = st;                 \
+      lc_.attrs = at_; lc_.numAttrs = 1;                                                                     \
+      cudaError_t e = cudaLaunchKernelEx(&lc_, teuk_step_kernel<V, VECF, CMF, SEGF, FWF>, p);                \
+      if (e != cudaSuccess) return e;                                                                        \
+    } else                                                                                                   \
     teuk_step_kernel<V, VECF, CMF, SEGF, FWF><<<grid, block, dyn, st>>>(p);                                  \
   } while (0)
   const bool fullw = p.n_theta == 32 * V;
