@@ -62,9 +62,10 @@ struct teuk_solver {
   int m[TEUK_MAX_MODES];
   // options
   int outer_bc, coef_mode, slab_rows_opt, use_graph, variant, autotune;
-  int tuned_rows;        // slab length chosen by the one-time autotune (0 = not tuned yet)
+  int tuned_rows;        // slabs per mode chosen by the one-time autotune (0 = not tuned yet)
   int temporal_block;    // 1 = one iteration per launch, 2 = two (warp pairs, level n+1 stays on chip)
-  int tuned_rows2;       // autotuned slab length of the temporal-blocking kernel
+  int tuned_rows2;       // autotuned slabs per mode of the temporal-blocking kernel
+  int force_slabs;       // autotune in progress: slabs per mode of the candidate being timed
   // resident kernel ("kernel" = 2): rows per block, blocks per mode, exchange buffer and its running tag
   int kernel_opt;        // "kernel" option: -1 = automatic (resident kernel when the state fits on chip, else kernel 0)
   int use_pdl;           // "pdl" option: programmatic dependent launch inside CUDA-graph batches
@@ -217,6 +218,22 @@ int rows_for_waves(const teuk_solver* s, double waves, int tb = 1) {
 
 int auto_slab_rows(const teuk_solver* s, int tb = 1) { return rows_for_waves(s, 2.0, tb); }
 
+int slabs_for_rows(const teuk_solver* s, long long rows) {
+  const long long interior = s->n_r - 2;
+  if (rows < 1) rows = 1;
+  if (rows > interior) rows = interior;
+  return (int)((interior + rows - 1) / rows);
+}
+
+// Slabs per mode of the marching kernels: the candidate under measurement, an explicit "slab_rows", the measured
+// optimum, or the two-wave heuristic.  The rows are then dealt evenly to that many slabs.
+int slabs_in_use(const teuk_solver* s, int tb = 1) {
+  if (s->force_slabs > 0) return s->force_slabs;
+  if (s->slab_rows_opt > 0) return slabs_for_rows(s, s->slab_rows_opt);
+  const int tuned = tb == 2 ? s->tuned_rows2 : s->tuned_rows;
+  return tuned > 0 ? tuned : slabs_for_rows(s, auto_slab_rows(s, tb));
+}
+
 void fill_params(const teuk_solver* s, StepParams* p, int in_buf, int k, int tap_enable, int tb = 1) {
   memset(p, 0, sizeof(*p));
   p->uin = s->d_u[in_buf];
@@ -228,10 +245,9 @@ void fill_params(const teuk_solver* s, StepParams* p, int in_buf, int k, int tap
   p->n_r = s->n_r;
   p->n_theta = s->n_theta;
   p->n_modes = s->n_modes;
-  const int tuned = tb == 2 ? s->tuned_rows2 : s->tuned_rows;
-  p->slab_rows = s->slab_rows_opt > 0 ? s->slab_rows_opt : (tuned > 0 ? tuned : auto_slab_rows(s, tb));
-  if (p->slab_rows > s->n_r - 2) p->slab_rows = s->n_r - 2;
-  p->n_slabs = (s->n_r - 2 + p->slab_rows - 1) / p->slab_rows;
+  p->n_slabs = slabs_in_use(s, tb);
+  p->slab_q = (s->n_r - 2) / p->n_slabs;
+  p->slab_rem = (s->n_r - 2) % p->n_slabs;
   p->n_seg = n_segments(s);
   p->seg_payload = p->n_seg > 1 ? ((s->n_theta + p->n_seg - 1) / p->n_seg + 3) / 4 * 4 : s->n_theta;
   p->outer_bc = s->outer_bc;
@@ -572,35 +588,38 @@ int build_graph(teuk_solver* s, int tb) {
 // iteration counter and the recorded series are untouched, and results do not depend on the slab length.
 int tune_slab_rows(teuk_solver* s, int tb) {
   const double waves[] = {0.95, 1.9, 2.0, 2.9, 3.9, 5.8};
-  int cand[48];
+  int cand[64];
   int nc = 0;
-  auto add = [&](int r) {
-    if (r < 1) r = 1;
-    if (r > s->n_r - 2) r = s->n_r - 2;
+  const int interior = s->n_r - 2;
+  auto add = [&](long long n) {                        // candidate: n slabs per mode
+    if (n < 1) n = 1;
+    if (n > interior) n = interior;
     for (int q = 0; q < nc; ++q)
-      if (cand[q] == r) return;
-    if (nc < 48) cand[nc++] = r;
+      if (cand[q] == (int)n) return;
+    if (nc < 64) cand[nc++] = (int)n;
   };
   const int base = auto_slab_rows(s, tb);
   if (base <= 24) {
     const int small[] = {1, 2, 3, 4, 5, 6, 7, 8, 10, 12, 14, 16, 20, 24};   // small grids: wave quantisation is coarse
-    for (int r : small) add(r);
+    for (int r : small) add(slabs_for_rows(s, r));
   } else {
     for (double w : waves) {
       const int r = rows_for_waves(s, w, tb);
-      add(r);
-      add(r + (r + 9) / 10);                       // and its +-10 % neighbours
-      add(r - (r + 9) / 10);
+      add(slabs_for_rows(s, r));
+      add(slabs_for_rows(s, r + (r + 9) / 10));        // and its +-10 % neighbours
+      add(slabs_for_rows(s, r - (r + 9) / 10));
     }
   }
+  // whole numbers of waves: k times the warps that are resident at once, shared by the modes and theta segments
+  const long long per_wave = (long long)resident_warps(s) / tb / ((long long)s->n_modes * n_segments(s));
+  for (int k = 1; k <= 6; ++k) add(k * per_wave);
   cudaEvent_t e0, e1;
   CK(cudaEventCreate(&e0), "autotune: event");
   CK(cudaEventCreate(&e1), "autotune: event");
   float best = 1e30f;
-  int best_rows = base;
-  const int saved = s->slab_rows_opt;
+  int best_slabs = slabs_for_rows(s, base);
   for (int q = 0; q < nc; ++q) {
-    s->slab_rows_opt = cand[q];
+    s->force_slabs = cand[q];
     StepParams p;
     fill_params(s, &p, s->cur, (int)(s->step - s->base_on_device), 0, tb);
     p.tap_enable2 = 0;
@@ -622,15 +641,15 @@ int tune_slab_rows(teuk_solver* s, int tb) {
     }
     s->launches += 1;
     if (e != cudaSuccess) {
-      s->slab_rows_opt = saved;
+      s->force_slabs = 0;
       cudaEventDestroy(e0);
       cudaEventDestroy(e1);
       return cuda_fail(s, e, "autotune");
     }
-    if (ms < best) { best = ms; best_rows = cand[q]; }
+    if (ms < best) { best = ms; best_slabs = cand[q]; }
   }
-  s->slab_rows_opt = saved;
-  if (tb == 2) s->tuned_rows2 = best_rows; else s->tuned_rows = best_rows;
+  s->force_slabs = 0;
+  if (tb == 2) s->tuned_rows2 = best_slabs; else s->tuned_rows = best_slabs;
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
   return TEUK_OK;
@@ -956,10 +975,10 @@ int teuk_get_stat(const teuk_solver* s, const char* key, int64_t* value) {
     else if (!strcmp(key, "resident_rows")) *value = res ? rr : 0;
     else *value = res ? (int64_t)nc * s->n_modes : 0;
   }
-  else if (!strcmp(key, "slab_rows")) {
-    const int tb = tb2_active(s) ? 2 : 1;
-    const int tuned = tb == 2 ? s->tuned_rows2 : s->tuned_rows;
-    *value = s->slab_rows_opt > 0 ? s->slab_rows_opt : (tuned > 0 ? tuned : auto_slab_rows(s, tb));
+  else if (!strcmp(key, "slabs")) *value = slabs_in_use(s, tb2_active(s) ? 2 : 1);
+  else if (!strcmp(key, "slab_rows")) {                 // longest slab in use
+    const int n = slabs_in_use(s, tb2_active(s) ? 2 : 1);
+    *value = (s->n_r - 2 + n - 1) / n;
   }
   else return TEUK_EINVAL;
   return TEUK_OK;

@@ -58,7 +58,7 @@ struct StepParams {
   const double* coef2d;   // coef_mode 1: [n_modes][2 n_r - 1][8][n_theta] streamed coefficient planes
   int coef_mode;
   int n_r, n_theta, n_modes;
-  int slab_rows, n_slabs;
+  int n_slabs, slab_q, slab_rem;   // marching kernels: slabs per mode; rows per slab = slab_q (+ 1 for the first slab_rem)
   int n_seg, seg_payload; // theta segments (register kernel, n_theta > 128): count and payload columns each
   int pdl;                // host side only: launch teuk_step_kernel as a programmatic dependent of the previous launch
   int variant;            // 0 = register-resident kernel, 1 = shared-memory-resident kernel, 2 = resident (on-chip) kernel

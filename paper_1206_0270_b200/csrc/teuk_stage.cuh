@@ -16,6 +16,12 @@ namespace {
 
 constexpr unsigned FULL = 0xffffffffu;
 
+// The n_r - 2 interior rows are dealt to the n_slabs slabs as evenly as possible: the first slab_rem slabs get
+// slab_q + 1 rows, the others slab_q (so that n_slabs = a whole number of waves of warps leaves no ragged tail).
+__device__ __forceinline__ int slab_first_row(const StepParams& p, int slab) {
+  return 1 + slab * p.slab_q + min(slab, p.slab_rem);
+}
+
 template <int V>
 struct Row {
   double c[4][V];  // Phi_R, Phi_I, Pi_R, Pi_I for this lane's V columns

@@ -76,8 +76,8 @@ __global__ void __launch_bounds__(128, (V == 2 ? 3 : TEUK_MIN_BLOCKS)) teuk_step
   const int mode = blockIdx.y;
   const int nth = FULLW ? 32 * V : p.n_theta, nr = p.n_r;
   if (slab >= p.n_slabs) return;
-  const int r0 = 1 + slab * p.slab_rows;             // first interior node of this slab
-  const int r1 = min(r0 + p.slab_rows, nr - 1);      // one past the last
+  const int r0 = slab_first_row(p, slab);            // first interior node of this slab
+  const int r1 = slab_first_row(p, slab + 1);        // one past the last
   const int c_lo = SEG ? (int)blockIdx.z * p.seg_payload - 4 : 0;            // first column of the window
   const int pay_lo = SEG ? (int)blockIdx.z * p.seg_payload : 0;
   const int pay_hi = SEG ? min(pay_lo + p.seg_payload, nth) : nth;
@@ -388,8 +388,8 @@ __global__ void __launch_bounds__(128, TEUK_SMEM_MIN_BLOCKS) teuk_step_smem_kern
   __syncthreads();
 #endif
   if (slab >= p.n_slabs) return;
-  const int r0 = 1 + slab * p.slab_rows;
-  const int r1 = min(r0 + p.slab_rows, nr - 1);
+  const int r0 = slab_first_row(p, slab);
+  const int r1 = slab_first_row(p, slab + 1);
   const size_t row_stride = (size_t)4 * nth;
   const double* __restrict__ uin = p.uin + (size_t)mode * nr * row_stride;
   double* __restrict__ uout = p.uout + (size_t)mode * nr * row_stride;
@@ -761,8 +761,8 @@ __global__ void __launch_bounds__(128, (V == 2 ? 3 : TEUK_MIN_BLOCKS)) teuk_step
   }
   __syncthreads();                                          // barriers are initialised for both warps of a pair
   if (slab >= p.n_slabs) return;                            // both warps of the pair leave together
-  const int r0 = 1 + slab * p.slab_rows;
-  const int r1 = min(r0 + p.slab_rows, p.n_r - 1);
+  const int r0 = slab_first_row(p, slab);
+  const int r1 = slab_first_row(p, slab + 1);
   const size_t row_doubles = (size_t)4 * nth;
   Tb2Shared sh;
   sh.rt_buf = &s_rt[wib][0][0];
