@@ -123,7 +123,8 @@ int teuk_get_state(teuk_solver *s, double *phi_re, double *phi_im, double *pi_re
  *   "coef_mode"     0 = coefficients recomputed on the fly from 1D tables (default),
  *                   1 = coefficients streamed from precomputed 2D FP64 planes (n_theta <= 128 only)
  *   "slab_rows"     rows of r* marched by one warp (0 = automatic: measured once at the first teuk_step,
- *                   which then waits for a few untimed-by-the-caller trial launches into scratch memory)
+ *                   which then waits for a few untimed-by-the-caller trial launches into scratch memory); the
+ *                   interior rows are dealt evenly to ceil((n_r - 2) / slab_rows) slabs
  *   "autotune"      1 = measure the slab length (default), 0 = use the two-wave heuristic
  *   "temporal_block" 1 = one iteration per kernel launch (default), 2 = two iterations per HBM round trip
  *                   (warp pairs; level n+1 stays in shared memory; same results bit for bit; needs kernel 0,
@@ -139,13 +140,15 @@ int teuk_get_state(teuk_solver *s, double *phi_re, double *phi_im, double *pi_re
  *                   All kernels do the same arithmetic per point: fields are bitwise identical (waveforms too,
  *                   except kernel 1, which sums over theta in another order).  An explicit "slab_rows" makes the
  *                   automatic choice stay with kernel 0.
+ *   "pdl"           1 (default) = inside a CUDA-graph batch, iteration k + 1 of kernel 0 is launched as a programmatic
+ *                   dependent of iteration k (its prologue overlaps k's tail); 0 = fully serialised launches
  *   "resident_cache" 1 (default) = kernel 2 also keeps the time-independent coefficients b, b^2 and Re beta' of its
  *                   rows in shared memory when they fit (3 doubles per point and location), 0 = it rebuilds them
  *                   in every stage like kernel 0.  Same results bit for bit. */
 int teuk_set_option(teuk_solver *s, const char *key, int64_t value);
 
 /* Read-only counters: "steps" (iterations done), "launches" (kernels launched so far),
- * "n_pts" (n_modes*n_r*n_theta), "state_bytes" (one copy of the fields), "slab_rows" (in use),
+ * "n_pts" (n_modes*n_r*n_theta), "state_bytes" (one copy of the fields), "slab_rows" (longest slab in use), "slabs" (slabs per mode),
  * "kernel" (the kernel the next teuk_step would run), "resident_rows" / "resident_blocks" (rows of r* per
  * block and blocks of kernel 2, 0 if it is not in use). */
 int teuk_get_stat(const teuk_solver *s, const char *key, int64_t *value);

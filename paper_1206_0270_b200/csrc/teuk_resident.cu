@@ -87,6 +87,44 @@ __device__ __forceinline__ void flag_wait(unsigned addr, int need) {
   }
 }
 
+// Shared-memory rows through explicit 32-bit shared addresses (worked out once per warp): ptxas otherwise rebuilds
+// the generic -> shared window base at every access site inside the time loop.  `addr` is this lane's first
+// column of component 0; the four components of a row are 32 V doubles apart.
+template <int V>
+__device__ __forceinline__ void lds_row_s(Row<V>& u, unsigned addr) {
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const unsigned q = addr + (unsigned)(c * 32 * V * 8);
+    if (V == 1) {
+      asm volatile("ld.shared.f64 %0, [%1];" : "=d"(u.c[c][0]) : "r"(q) : "memory");
+    } else {
+#pragma unroll
+      for (int v = 0; v < V; v += 2)
+        asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(u.c[c][v]), "=d"(u.c[c][v + 1]) : "r"(q + 8u * v) : "memory");
+    }
+  }
+}
+template <int V>
+__device__ __forceinline__ void sts_row_s(const Row<V>& u, unsigned addr) {
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const unsigned q = addr + (unsigned)(c * 32 * V * 8);
+    if (V == 1) {
+      asm volatile("st.shared.f64 [%0], %1;" ::"r"(q), "d"(u.c[c][0]) : "memory");
+    } else {
+#pragma unroll
+      for (int v = 0; v < V; v += 2)
+        asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(q + 8u * v), "d"(u.c[c][v]), "d"(u.c[c][v + 1]) : "memory");
+    }
+  }
+}
+// one r-table record (RT_N = 10 doubles, warp-uniform address: broadcast loads) into registers
+__device__ __forceinline__ void lds_record_s(double (&rc)[RT_N], unsigned addr) {
+#pragma unroll
+  for (int k = 0; k < RT_N; k += 2)
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(rc[k]), "=d"(rc[k + 1]) : "r"(addr + 8u * k) : "memory");
+}
+
 template <int V>
 __device__ __forceinline__ uint4* ll_slot(const StepParams& p, int mode, int ncta, int cta, int side, unsigned tag) {
   return reinterpret_cast<uint4*>(p.ll) + ((((size_t)mode * ncta + cta) * 2 + side) * 2 + (tag & 1u)) * (size_t)(4 * 32 * V);
@@ -125,6 +163,12 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
   int* const sV = reinterpret_cast<int*>(sR + (size_t)(2 * p.res_rows + 2) * RT_N);   // version counters
   // coefficient cache: location 2 lo - 1 + q at sC + q * 3 NP, planes b2d, Q, bre (16-byte aligned)
   double* const sC = reinterpret_cast<double*>(sV + ((2 * p.res_rows + 3 + 3) & ~3));
+  constexpr unsigned ROWB = ROWD * 8;                           // bytes per row
+  const unsigned uU = smem_u32(sU) + 8u * (unsigned)(lane * V); // this lane's columns of row slot 0, component 0
+  const unsigned uH = smem_u32(sH) + 8u * (unsigned)(lane * V);
+  const unsigned uE = smem_u32(sE) + 8u * (unsigned)(lane * V);
+  const unsigned uC = smem_u32(sC) + 8u * (unsigned)(lane * V);
+  const unsigned uR = smem_u32(sR);
   const unsigned verU = smem_u32(sV);                           // [res_rows + 2]: level of row slot r, relative to entry
   const unsigned verH = verU + 4u * (unsigned)(p.res_rows + 2); // [res_rows + 1]: iterations that wrote half row h
 
@@ -172,18 +216,26 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
   auto stage = [&](auto half_tag, const Row<V>& A, const Row<V>& B, const Row<V>& base, const int q, const double tau,
                    Row<V>& out) {
     constexpr bool HALF = decltype(half_tag)::value;
+    __align__(16) double rc[RT_N];
+    lds_record_s(rc, uR + (unsigned)(q * RT_N * 8));
     if (CC) {
       double b2d[V], Q[V], bre[V];
-      const double* cq = sC + (size_t)q * 3 * NP + j0;
+      const unsigned cq = uC + (unsigned)q * (unsigned)(3 * NP * 8);
 #pragma unroll
-      for (int v = 0; v < V; ++v) {
-        b2d[v] = cq[v];
-        Q[v] = cq[NP + v];
-        bre[v] = cq[2 * NP + v];
+      for (int v = 0; v < V; v += (V == 1 ? 1 : 2)) {
+        if (V == 1) {
+          asm volatile("ld.shared.f64 %0, [%1];" : "=d"(b2d[0]) : "r"(cq) : "memory");
+          asm volatile("ld.shared.f64 %0, [%1];" : "=d"(Q[0]) : "r"(cq + (unsigned)(NP * 8)) : "memory");
+          asm volatile("ld.shared.f64 %0, [%1];" : "=d"(bre[0]) : "r"(cq + (unsigned)(2 * NP * 8)) : "memory");
+        } else {
+          asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(b2d[v]), "=d"(b2d[v + (V > 1 ? 1 : 0)]) : "r"(cq + 8u * v) : "memory");
+          asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(Q[v]), "=d"(Q[v + (V > 1 ? 1 : 0)]) : "r"(cq + (unsigned)(NP * 8) + 8u * v) : "memory");
+          asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(bre[v]), "=d"(bre[v + (V > 1 ? 1 : 0)]) : "r"(cq + (unsigned)(2 * NP * 8) + 8u * v) : "memory");
+        }
       }
-      lw_stage_cached<V, HALF>(A, B, base, sR + q * RT_N, th, b2d, Q, bre, tau, out);
+      lw_stage_cached<V, HALF>(A, B, base, rc, th, b2d, Q, bre, tau, out);
     } else {
-      lw_stage<V, HALF>(A, B, base, sR + q * RT_N, th, tau, tdx, out);
+      lw_stage<V, HALF>(A, B, base, rc, th, tau, tdx, out);
     }
   };
   const long long n0 = *p.d_base + p.k;                  // index of the input level of iteration 0
@@ -216,9 +268,9 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
       if (h >= 1) flag_wait(verU + 4u * (unsigned)h, it);
       if (h + 1 <= rows) flag_wait(verU + 4u * (unsigned)(h + 1), it);
       if (h == 0 && !first && it > 0) ll_receive<V>(ll_slot<V>(p, mode, ncta, cta - 1, 1, tag_in), A, tag_in, lane);
-      else lds_row<V>(A, sU + (size_t)h * ROWD, NP, j0, true);
+      else lds_row_s<V>(A, uU + (unsigned)h * ROWB);
       if (h == rows && !last && it > 0) ll_receive<V>(ll_slot<V>(p, mode, ncta, cta + 1, 0, tag_in), B, tag_in, lane);
-      else lds_row<V>(B, sU + (size_t)(h + 1) * ROWD, NP, j0, true);
+      else lds_row_s<V>(B, uU + (unsigned)(h + 1) * ROWB);
       if (cta_taps && n >= 1 && (it > 0 || p.tap_enable)) tap<V>(A, B, p, i, mode, n, lane);
       stage(std::true_type(), A, B, A, 2 * h, tau_h, Hn);
       if (has_source) {
@@ -229,9 +281,10 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
           add_source<V>(Hn, s, p, i, true);
         }
       }
-      sts_row<V>(Hn, sH + (size_t)h * ROWD, NP, j0);
+      sts_row_s<V>(Hn, uH + (unsigned)h * ROWB);
       if (last && h == rows) {   // outer radial edge (reading A6): A = row n_r-2, B = row n_r-1
-        const double eps = sR[(2 * rows + 1) * RT_N + RT_EPS];   // location 2 (n_r - 1)
+        double eps;                                               // of location 2 (n_r - 1)
+        asm volatile("ld.shared.f64 %0, [%1];" : "=d"(eps) : "r"(uR + (unsigned)(((2 * rows + 1) * RT_N + RT_EPS) * 8)) : "memory");
         ThetaVals<V> tv;
         th.get(tv);
         Row<V> e;
@@ -248,7 +301,7 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
           e.c[2][v] = 0.0;
           e.c[3][v] = 0.0;
         }
-        sts_row<V>(e, sE, NP, j0);
+        sts_row_s<V>(e, uE);
       }
       __syncwarp();
       if (lane == 0) flag_set(verH + 4u * (unsigned)h, it + 1);
@@ -261,9 +314,9 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
       // both half-step rows of this iteration exist; their producers were the last readers of the old U[r]
       flag_wait(verH + 4u * (unsigned)(r - 1), it + 1);
       flag_wait(verH + 4u * (unsigned)r, it + 1);
-      lds_row<V>(Hp, sH + (size_t)(r - 1) * ROWD, NP, j0, true);
-      lds_row<V>(Hn, sH + (size_t)r * ROWD, NP, j0, true);
-      lds_row<V>(U0, sU + (size_t)r * ROWD, NP, j0, true);
+      lds_row_s<V>(Hp, uH + (unsigned)(r - 1) * ROWB);
+      lds_row_s<V>(Hn, uH + (unsigned)r * ROWB);
+      lds_row_s<V>(U0, uU + (unsigned)r * ROWB);
       stage(std::false_type(), Hp, Hn, U0, 2 * r - 1, tau_f, out);
       if (has_source) {
         const double x = p.rs_min + (double)i * p.dx;
@@ -277,19 +330,19 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
         if (r == 1 && !first) ll_publish<V>(ll_slot<V>(p, mode, ncta, cta, 0, tag_in + 1u), out, tag_in + 1u, lane);
         if (r == rows && !last) ll_publish<V>(ll_slot<V>(p, mode, ncta, cta, 1, tag_in + 1u), out, tag_in + 1u, lane);
       }
-      sts_row<V>(out, sU + (size_t)r * ROWD, NP, j0);
+      sts_row_s<V>(out, uU + (unsigned)r * ROWB);
       if (first && r == 1) {     // inner radial edge: Phi = Pi = 0
         Row<V> z;
 #pragma unroll
         for (int cc = 0; cc < 4; ++cc)
 #pragma unroll
           for (int v = 0; v < V; ++v) z.c[cc][v] = 0.0;
-        sts_row<V>(z, sU, NP, j0);
+        sts_row_s<V>(z, uU);
       }
       if (last && r == rows) {   // new outer-edge row, computed from level n with the half-step row h = rows
         Row<V> e;
-        lds_row<V>(e, sE, NP, j0, true);
-        sts_row<V>(e, sU + (size_t)(rows + 1) * ROWD, NP, j0);
+        lds_row_s<V>(e, uE);
+        sts_row_s<V>(e, uU + (unsigned)(rows + 1) * ROWB);
       }
       __syncwarp();
       if (lane == 0) flag_set(verU + 4u * (unsigned)r, it + 1);

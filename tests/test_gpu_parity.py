@@ -166,6 +166,32 @@ def test_graph_and_plain_launches_agree_bitwise(orc, teuk):
         assert np.array_equal(out[0][1][1], out[k][1][1]) and len(out[k][1][0]) == 150
 
 
+def test_programmatic_dependent_launch_is_bitwise_identical(orc, teuk):
+    """"pdl" = 1 (default) launches iterations 2..32 of a CUDA-graph batch as programmatic dependents of the previous
+    one (their prologue overlaps its tail): same fields and waveforms as fully serialised launches; and the number of
+    slabs the rows are dealt to does not change anything either."""
+    cfg = SMALL[3]
+    out = []
+    for pdl, slab_rows in ((1, 0), (0, 0), (1, 7), (0, 1)):
+        g = teuk.Solver.from_config(cfg)
+        g.set_option("kernel", 0)
+        g.set_option("pdl", pdl)
+        g.set_option("slab_rows", slab_rows)
+        g.set_initial(*wl.random_state(cfg, 4))
+        g.set_source(wl.orbit_table(cfg, n_steps=200))
+        g.add_observer(30.0, wl.observer_weights(cfg))
+        g.step(133)                     # one plain launch, four graph batches, remainder
+        g.step(67)
+        n = g.stat("slabs")
+        assert 1 <= n <= cfg.n_r - 2 and g.stat("slab_rows") == -(-(cfg.n_r - 2) // n)
+        out.append((g.get_state(), g.extract(30.0)))
+        g.close()
+    for k in (1, 2, 3):
+        for a, b in zip(out[0][0], out[k][0]):
+            assert np.array_equal(a, b)
+        assert np.array_equal(out[0][1][1], out[k][1][1]) and len(out[k][1][0]) == 200
+
+
 def test_ring_buffer_wraps_and_drains(orc, teuk):
     """More iterations than the device ring holds (32768): samples are drained by async copies."""
     cfg = wl.CONFIGS[1].scaled(name="ring", n_r=24, n_theta=8, rs_min=10.0, rs_max=19.2, steps=40000,
