@@ -117,27 +117,12 @@ __global__ void __launch_bounds__(128, (V == 2 ? 3 : TEUK_MIN_BLOCKS)) teuk_step
                      "r"(smem_u32(&bars[q % NS])) : "memory");
     }
   };
-  // Programmatic dependent launch: when the host launched this grid with the stream-serialisation attribute
-  // (iterations 2..32 of a CUDA-graph batch), everything above -- index arithmetic and the first r-table chunk,
-  // which no kernel of the loop writes -- ran while the previous iteration was still finishing.  From here on the
-  // previous iteration's output (our input) is read and its input (our output) overwritten: wait for it, and let
-  // the next iteration's grid start its own prologue as soon as SM slots free up.  (Without the attribute both
-  // instructions do nothing.)
-  asm volatile("griddepcontrol.wait;" ::: "memory");
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  const long long n = *p.d_base + p.k;               // index of the input time level
-  if (VEC) {
-    if (lane == 0) {
+  const long long n = *p.d_base + p.k;               // index of the input time level (step kernels never write it)
+  if (VEC && lane == 0) {
 #pragma unroll
-      for (int q = 0; q < NS; ++q) mbar_init(&bars[q], 1);
-      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      // row q lands in slot q % NS; rows r0+2 .. r0+NS go out now, row i+NS+1 in the middle of iteration i
-#pragma unroll
-      for (int q = 2; q <= NS; ++q)
-        if (r0 + q <= r1) issue_row(r0 + q);
-    }
-    __syncwarp();
+    for (int q = 0; q < NS; ++q) mbar_init(&bars[q], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
 
   ThetaTab<V> th;
@@ -164,6 +149,24 @@ __global__ void __launch_bounds__(128, (V == 2 ? 3 : TEUK_MIN_BLOCKS)) teuk_step
   }
   const bool any_src = __any_sync(FULL, src_h.on || src_f.on);   // vote result: provably warp-uniform
   const double tau_h = 0.5 * p.dt, tau_f = 0.25 * p.dt, tdx = 2.0 / p.dx;
+
+  // Programmatic dependent launch: when the host launched this grid with the stream-serialisation attribute
+  // (iterations 2..32 of a CUDA-graph batch), everything above -- index arithmetic, the first r-table chunk, the
+  // theta tables, the source window and deposit profile, none of which a step kernel writes -- ran while the
+  // previous iteration was still finishing.  From here on the previous iteration's output (our input) is read and
+  // its input (our output) overwritten: wait for it, and let the next iteration's grid start its own prologue as
+  // soon as SM slots free up.  (Without the attribute both instructions do nothing.)
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  if (VEC) {
+    if (lane == 0) {
+      // row q lands in slot q % NS; rows r0+2 .. r0+NS go out now, row i+NS+1 in the middle of iteration i
+#pragma unroll
+      for (int q = 2; q <= NS; ++q)
+        if (r0 + q <= r1) issue_row(r0 + q);
+    }
+    __syncwarp();
+  }
 
   Row<V> ua, ub, uc, hp, hn, out;
   load_row<V, VEC>(ua, uin + (size_t)(r0 - 1) * row_stride, nth, j0);
