@@ -30,6 +30,10 @@ struct Row {
 #ifndef TEUK_MIN_BLOCKS
 #define TEUK_MIN_BLOCKS 2   // resident blocks for V = 1, 4 (V = 2 always asks for 3); 3 with V = 4 spills: 29 GPts/s
 #endif
+#ifndef TEUK_V2_BLOCKS
+#define TEUK_V2_BLOCKS 3     // resident blocks of the marching kernel for V = 2 (160 registers, no spills); 4 (128 registers,
+                             // 228 B of spill stores): configs 3 / 4 at 62 / 74 instead of 67 / 78 GPts/s
+#endif
 #ifndef TEUK_FAST_RSQRT
 #define TEUK_FAST_RSQRT 1   // own MUFU.RSQ64H + one third-order step instead of CUDA's rsqrt(): +6 GPts/s
 #endif

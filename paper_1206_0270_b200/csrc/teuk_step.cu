@@ -66,7 +66,7 @@ __device__ __forceinline__ void stage_rtab_chunk(double* sbuf, const double* __r
 // blocks, __maxnreg__(224): 388 B of spill stores) 69.6; bracket B accumulated in two partial sums
 // (shorter dependent chains, more spills) 89.1.
 template <int V, bool VEC, int CM, bool SEG, bool FULLW>
-__global__ void __launch_bounds__(128, (V == 2 ? 3 : TEUK_MIN_BLOCKS)) teuk_step_kernel(const __grid_constant__ StepParams p) {
+__global__ void __launch_bounds__(128, (V == 2 ? TEUK_V2_BLOCKS : TEUK_MIN_BLOCKS)) teuk_step_kernel(const __grid_constant__ StepParams p) {
   const int lane = threadIdx.x & 31;
   // warp index broadcast from lane 0: tells the compiler that everything derived from it (slab bounds, loop
   // trip count, the early exit) is warp-uniform, so the warp stays provably converged: no BRA.DIV guards
