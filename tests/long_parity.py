@@ -45,6 +45,7 @@ def main():
     for x in cfg.observers:
         g.add_observer(x, W)
     g.sync()
+    kernel = g.stat("kernel")     # 2 = resident kernel (state on chip), 0 = marching kernel
     t0 = time.perf_counter()
     g.step(steps)
     g.sync()
@@ -83,7 +84,7 @@ def main():
     phi_g, phi_o = sg[0] + 1j * sg[1], so[0] + 1j * so[1]
     pi_g, pi_o = sg[2] + 1j * sg[3], so[2] + 1j * so[3]
     res = {
-        "config": cfg.cid, "workload": cfg.name, "steps": steps, "full_length": steps == cfg.steps,
+        "config": cfg.cid, "workload": cfg.name, "steps": steps, "full_length": steps == cfg.steps, "kernel": int(kernel),
         "rel_l2_phi": rel(phi_g, phi_o), "rel_l2_pi": rel(pi_g, pi_o),
         "norm_phi": float(np.linalg.norm(phi_o)), "norm_pi": float(np.linalg.norm(pi_o)),
         "waveforms": [{"x_obs": x, "rel_l2": (rel(g_[1], o_[1]) if np.linalg.norm(o_[1]) >= 1e-200 else "silent"),
