@@ -244,7 +244,7 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
 
   // Task list of one iteration: T = 2 rows + 1 tasks, first the rows + 1 half-step rows (those that need a
   // neighbour block's row LAST), then the rows full-step rows (the two edge rows of the block, which are
-  // published, FIRST).  Task g = it * T + t runs on warp g mod nw, so the load rotates over the warps, and
+  // published, EARLY).  Task g = it * T + t runs on warp g mod nw, so the load rotates over the warps, and
   // every warp works through its tasks in increasing g.  A task waits for the rows it reads (version counters
   // in shared memory, release/acquire), never for a block-wide barrier; every dependence points to a smaller g,
   // so the smallest unfinished task can always run.
@@ -308,7 +308,11 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
     } else {
       // ---- full-step row in place (Eq. 4) ----
       const int tt = t - (rows + 1);
-      const int r = (tt == 0) ? 1 : (tt == 1 ? rows : tt);
+      // order: the two edge rows of the block (whose results are published) early, but behind `defer` interior rows:
+      // their half-step inputs H[0], H[rows] were the LAST half-step tasks, so starting with them left two warps
+      // idle for a task's time (config 2, us per iteration: defer 0 / 2 / 3 / 4 / 5 / 8 = 3.54 / 3.39 / 3.34 / 3.33 / 3.40 / 3.42)
+      const int defer = rows >= 12 ? 4 : 0;
+      const int r = (tt < defer) ? tt + 2 : (tt == defer ? 1 : (tt == defer + 1 ? rows : tt));
       const int i = lo - 1 + r;
       Row<V> Hp, Hn, U0, out;
       // both half-step rows of this iteration exist; their producers were the last readers of the old U[r]
