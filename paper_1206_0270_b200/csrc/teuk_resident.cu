@@ -25,9 +25,6 @@
 
 #include "teuk_stage.cuh"
 
-#ifndef TEUK_RES_FLAG_SLEEP
-#define TEUK_RES_FLAG_SLEEP 0   // ns between two polls of a version counter
-#endif
 #ifndef TEUK_RES_NW
 #define TEUK_RES_NW(V) ((V) == 4 ? 8 : 16)   // warps per block the register budget is cut for
 #endif
@@ -74,16 +71,15 @@ __device__ __forceinline__ void ll_receive(const uint4* slot, Row<V>& u, unsigne
 __device__ __forceinline__ void flag_set(unsigned addr, int v) {
   asm volatile("st.release.cta.shared.s32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
-__device__ __forceinline__ void flag_wait(unsigned addr, int need) {
+// both counters of a task are polled together (one round trip to shared memory, one vote)
+__device__ __forceinline__ void flag_wait2(unsigned addr_a, unsigned addr_b, int need) {
   unsigned tries = 0;
   for (;;) {
-    int v;
-    asm volatile("ld.acquire.cta.shared.s32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
-    if (__all_sync(FULL, v >= need)) break;
+    int va, vb;
+    asm volatile("ld.acquire.cta.shared.s32 %0, [%1];" : "=r"(va) : "r"(addr_a) : "memory");
+    asm volatile("ld.acquire.cta.shared.s32 %0, [%1];" : "=r"(vb) : "r"(addr_b) : "memory");
+    if (__all_sync(FULL, va >= need && vb >= need)) break;
     if (++tries > (1u << 26)) asm volatile("trap;");
-#if TEUK_RES_FLAG_SLEEP > 0
-    __nanosleep(TEUK_RES_FLAG_SLEEP);
-#endif
   }
 }
 
@@ -265,8 +261,7 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
       const int i = lo - 1 + h;
       Row<V> A, B, Hn;
       // own rows must be at level `it`; that also says the readers of the old H[h] are done (they wrote them)
-      if (h >= 1) flag_wait(verU + 4u * (unsigned)h, it);
-      if (h + 1 <= rows) flag_wait(verU + 4u * (unsigned)(h + 1), it);
+      flag_wait2(verU + 4u * (unsigned)(h >= 1 ? h : 1), verU + 4u * (unsigned)(h + 1 <= rows ? h + 1 : rows), it);
       if (h == 0 && !first && it > 0) ll_receive<V>(ll_slot<V>(p, mode, ncta, cta - 1, 1, tag_in), A, tag_in, lane);
       else lds_row_s<V>(A, uU + (unsigned)h * ROWB);
       if (h == rows && !last && it > 0) ll_receive<V>(ll_slot<V>(p, mode, ncta, cta + 1, 0, tag_in), B, tag_in, lane);
@@ -316,8 +311,7 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
       const int i = lo - 1 + r;
       Row<V> Hp, Hn, U0, out;
       // both half-step rows of this iteration exist; their producers were the last readers of the old U[r]
-      flag_wait(verH + 4u * (unsigned)(r - 1), it + 1);
-      flag_wait(verH + 4u * (unsigned)r, it + 1);
+      flag_wait2(verH + 4u * (unsigned)(r - 1), verH + 4u * (unsigned)r, it + 1);
       lds_row_s<V>(Hp, uH + (unsigned)(r - 1) * ROWB);
       lds_row_s<V>(Hn, uH + (unsigned)r * ROWB);
       lds_row_s<V>(U0, uU + (unsigned)r * ROWB);
