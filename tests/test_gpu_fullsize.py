@@ -53,6 +53,41 @@ def test_full_grid_short_run(orc, teuk, cid, steps):
     o.close()
 
 
+@pytest.mark.parametrize("cid,steps", [(1, 300), (2, 150)])
+def test_full_grid_resident_kernel(orc, teuk, cid, steps):
+    """Configs 1 and 2 at full size in the launch configuration bench.py times for them: the resident kernel (the
+    library's default there: 128 blocks x 4 rows, 147 blocks x 28 rows), every point against the oracle from seeded
+    random data, and bit for bit against the marching kernel."""
+    cfg = wl.CONFIGS[cid]
+    ini = wl.random_state(cfg, 600 + cid)
+    W = wl.observer_weights(cfg)
+    x_obs = cfg.observers[-1]
+    o = orc.OracleSolver.from_config(cfg)
+    o.set_initial(*ini)
+    o.add_observer(x_obs, W)
+    o.step(steps)
+    so = o.get_state()
+    to, wo = o.waveform(0)
+    o.close()
+    out = []
+    for kernel in (-1, 0):
+        g = teuk.Solver.from_config(cfg)
+        g.set_option("kernel", kernel)
+        assert g.stat("kernel") == (2 if kernel < 0 else 0)
+        g.set_initial(*ini)
+        g.add_observer(x_obs, W)
+        g.step(steps)
+        out.append((g.get_state(), g.extract(x_obs)))
+        g.close()
+    for a, b in zip(out[0][0], so):
+        assert np.all(np.isfinite(a)) and _rel(a, b) <= TOL
+        assert np.max(np.abs(a - b)) <= 1e-9 * np.max(np.abs(b))
+    assert len(out[0][1][0]) == steps and _rel(out[0][1][1], wo) <= TOL
+    for a, b in zip(out[0][0], out[1][0]):
+        assert np.array_equal(a, b)
+    assert np.array_equal(out[0][1][1], out[1][1][1])
+
+
 def test_config5_sampled_windows_after_long_run(orc, teuk):
     cfg = wl.CONFIGS[5]
     n_long, n_check, half = 600, 3, 40
