@@ -51,10 +51,22 @@ def test_create_fails_loudly_without_gpu(lib_path):
     assert e.value.code == teuk.TEUK_ECUDA and "no CPU fallback" in str(e.value)
 
 
+def test_every_option_and_stat_key_is_documented_in_the_header():
+    """include/teuk.h is the contract: each key teuk_set_option / teuk_get_stat accepts must be described there."""
+    src = open(os.path.join(PKG, "csrc", "teuk_api.cu")).read()
+    header = open(os.path.join(ROOT, "include", "teuk.h")).read()
+    opt = src[src.index("int teuk_set_option("):src.index("int teuk_get_stat(")]
+    stat = src[src.index("int teuk_get_stat("):]
+    keys = set(re.findall(r'strcmp\(key, "([a-z_0-9]+)"\)', opt)) | set(re.findall(r'strcmp\(key, "([a-z_0-9]+)"\)', stat))
+    assert {"outer_bc", "kernel", "slab_rows", "pdl", "resident_cache", "steps", "launches"} <= keys
+    for k in sorted(keys):
+        assert '"%s"' % k in header, "option / counter %r is not documented in include/teuk.h" % k
+
+
 def test_product_never_references_the_oracle():
     for dirpath, _, files in os.walk(PKG):
         for f in files:
-            if f.endswith((".py", ".cu", ".h", ".cpp")):
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
                 text = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle", text, flags=re.M), f
                 assert "liboracle" not in text and "orc_" not in text, f
