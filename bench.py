@@ -42,17 +42,63 @@ def measured_peak_gbs():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "traffic.json")
+
+
 def ncu_traffic_bytes(cfg):
-    """DRAM bytes per launch of the step kernel from the committed ncu capture, if one matches."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(p):
+    """(DRAM bytes per launch of the step kernel, where the figure comes from) from the committed ncu capture,
+    if one matches this workload.  It is NOT measured in this run (ncu cannot run inside a timed region):
+    `bench.py --ncu-traffic RAW.csv` refreshes the file from an `ncu --page raw --csv` export."""
+    if os.path.exists(TRAFFIC_JSON):
         try:
-            d = json.load(open(p))
+            d = json.load(open(TRAFFIC_JSON))
             if d.get("workload") == cfg.name:
-                return float(d["dram_bytes_per_launch"])
+                return float(d["dram_bytes_per_launch"]), d.get("source", "profiles/traffic.json")
         except Exception:
             pass
-    return None
+    return None, None
+
+
+def refresh_traffic(csv_path, cfg):
+    """profiles/traffic.json from the raw page of one `ncu --set full` capture (`ncu -i X.ncu-rep --page raw --csv`):
+    mean over the captured launches of teuk_step_kernel of dram__bytes_read.sum + dram__bytes_write.sum."""
+    import csv
+    rows = list(csv.reader(open(csv_path)))
+    hdr = rows[0]
+    units = rows[1]
+    kn, rd, wr = hdr.index("Kernel Name"), hdr.index("dram__bytes_read.sum"), hdr.index("dram__bytes_write.sum")
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    tot_r, tot_w, n, name = 0.0, 0.0, 0, None
+    for r in rows[2:]:
+        if len(r) <= max(rd, wr) or "teuk_step" not in r[kn]:
+            continue
+        tot_r += float(r[rd].replace(",", "")) * scale[units[rd]]
+        tot_w += float(r[wr].replace(",", "")) * scale[units[wr]]
+        n += 1
+        name = r[kn]
+    if n == 0:
+        raise SystemExit("no teuk_step kernel launch in " + csv_path)
+    d = {"workload": cfg.name, "kernel": name, "dram_bytes_per_launch": (tot_r + tot_w) / n,
+         "dram_bytes_read": tot_r / n, "dram_bytes_write": tot_w / n, "launches_averaged": n,
+         "source": "ncu --set full capture, raw page %s (python bench.py --ncu-traffic)" % os.path.basename(csv_path)}
+    json.dump(d, open(TRAFFIC_JSON, "w"), indent=1)
+    print(json.dumps(d))
+
+
+# FP64 instructions per point per iteration of the stage code (teuk_stage.cuh lw_stage, both stages), counted from
+# the executed-instruction column of the ncu source page of teuk_step_kernel<4,...> on config 5
+# (profiles/r2_sass_histogram.md): DFMA with three distinct register operands, other DFMA, DADD, DMUL.
+FP64_MIX = {"dfma3": 46.4, "dfma2": 10.3, "dadd": 18.2, "dmul": 22.6}
+
+
+def alu_peak(cfg, clocks):
+    """ "alu" ceiling of the step kernel in GPts/s from the library's FP64 microbenchmark (teuk_measure_fp64,
+    DESIGN.md 5.1): the instruction mix above issued back to back at the measured rate of each kind."""
+    from paper_1206_0270_b200 import measure_fp64
+    r = {k: measure_fp64(i) for i, k in enumerate(("dfma2", "dfma3", "dadd", "dmul"))}
+    sec_per_pt = sum(FP64_MIX[k] / r[k] for k in FP64_MIX)
+    return {"gpts": 1.0 / sec_per_pt / 1e9, "lane_ops_per_s": r, "fp64_per_pt_step": sum(FP64_MIX.values()),
+            "mix": FP64_MIX}
 
 
 class ClockSampler:
@@ -110,8 +156,9 @@ class ClockSampler:
 
 
 def oracle_sample_config(cfg, rows):
-    """Bounded sample of the workload for the CPU oracle: a radial crop around the particle."""
-    if cfg.n_r <= rows:
+    """The workload itself (rows = 0, the default), or, for development runs, a radial crop of `rows` rows
+    around the particle."""
+    if rows <= 0 or cfg.n_r <= rows:
         return cfg
     dx = cfg.dx
     lo = -rows // 8
@@ -141,8 +188,12 @@ def time_oracle(cfg, steps, warmup, rows, source_kind=0):
     dt = time.perf_counter() - t0
     o.close()
     threads = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
-    sample = "%d iterations of a %d x %d radial crop (of %d x %d) incl. source window and observer" % (
-        steps, c.n_r, c.n_theta, cfg.n_r, cfg.n_theta)
+    if c is cfg:
+        sample = "%d iterations (after %d untimed) of the whole %d x %d x %d-mode grid of the workload incl. source and observer" % (
+            steps, warmup, cfg.n_r, cfg.n_theta, cfg.n_modes)
+    else:
+        sample = "%d iterations of a %d x %d radial crop (of %d x %d) incl. source window and observer" % (
+            steps, c.n_r, c.n_theta, cfg.n_r, cfg.n_theta)
     return c.n_pts * steps / dt / 1e9, dt, threads, sample
 
 
@@ -192,7 +243,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=5)
-    ap.add_argument("--oracle-rows", type=int, default=16384)
+    ap.add_argument("--oracle-rows", type=int, default=0,
+                    help="0 (default): the oracle runs the whole grid of the workload; > 0: a radial crop of that many rows")
+    ap.add_argument("--ncu-traffic", default=None, metavar="RAW.csv",
+                    help="refresh profiles/traffic.json from an `ncu --page raw --csv` export and exit")
+    ap.add_argument("--fp64-peak", action="store_true", help="print the FP64 issue-rate microbenchmark (teuk_measure_fp64) and exit")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--quick", action="store_true", help="development: device-resident timing only")
     ap.add_argument("--slab-rows", type=int, default=0)
@@ -209,8 +264,14 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
 
+    if args.ncu_traffic:
+        refresh_traffic(args.ncu_traffic, cfg)
+        return
     if args.impl == "reference":
         run_reference(args, cfg, rank, world)
+        return
+    if args.fp64_peak:
+        print(json.dumps(alu_peak(cfg, None)))
         return
 
     import torch
@@ -229,8 +290,12 @@ def main():
         torch.cuda.synchronize()
 
     K, W = args.steps, args.warmup
-    # replica r evolves trajectory segment r: its table starts K+W iterations later
-    orbit = replica_orbit(cfg, rank, K + W)
+    # Untimed iterations on top of the W warm-up steps, so that everything a long teuk_step(K) call uses exists
+    # before the timed region starts: the first call runs one plain launch, then builds and replays the CUDA
+    # graph of one ping-pong parity (32 iterations), the second call that of the other parity.
+    XW = 2 * 33
+    # replica r evolves trajectory segment r: its table starts K+W+XW iterations later
+    orbit = replica_orbit(cfg, rank, K + W + XW)
     weights = wl.observer_weights(cfg)
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
@@ -260,6 +325,8 @@ def main():
             g.add_observer(x, weights)
         # ---- device-resident timing -----------------------------------------------------------
         g.step(W)
+        g.step(33)
+        g.step(33)
         barrier()
         sampler = ClockSampler(local_rank)
         if rank == 0:
@@ -291,11 +358,12 @@ def main():
             host_out = [torch.empty_like(h).pin_memory() for h in host_in]
         e2e_ms = []
         series = []
+        orbit_e2e = replica_orbit(cfg, rank, K)
         for rep in range(0 if args.quick else 2):   # first repetition warms the pinned paths
             barrier()
             t0 = time.perf_counter()
             g.set_initial(*host_in)                 # H2D: 4 planes
-            g.set_source(orbit)                     # H2D: trajectory table
+            g.set_source(orbit_e2e)                 # H2D: trajectory table
             g.step(K)
             series = [g.extract(x, allow_nonfinite=True) for x in cfg.observers]   # D2H: waveforms
             g.get_state(host_out)                   # D2H: 4 planes
@@ -304,13 +372,15 @@ def main():
         e2e_t = max_over_ranks(e2e_ms[-1] if e2e_ms else float("inf"), "cuda", world)
         e2e = world * cfg.n_pts * K / (e2e_t * 1e-3) / 1e9
         state_bytes = 4 * cfg.n_pts * 8
-        orbit_bytes = 0 if orbit is None else 8 * (2 + 2 * cfg.n_modes) * orbit["n_samples"]
+        orbit_bytes = 0 if orbit_e2e is None else 8 * (2 + 2 * cfg.n_modes) * orbit_e2e["n_samples"]
         wave_bytes = sum(len(s[0]) * (8 + 16 * cfg.n_modes) for s in series)
         g.close()
 
     if rank == 0:
         peak, peak_src = measured_peak_gbs()
         achieved = BYTES_PER_PT_STEP * cfg.n_pts * K / (ms * 1e-3) / 1e9   # per GPU: ms is the max over ranks
+        traffic, traffic_src = ncu_traffic_bytes(cfg)
+        hbm_bound = 2 * 4 * cfg.n_pts * 8 > 2.5e8       # both state copies exceed the 126 MB L2
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -318,6 +388,7 @@ def main():
             "config": {"workload": cfg.name, "grid": [cfg.n_r, cfg.n_theta], "modes": list(cfg.modes), "a": cfg.a,
                        "dt": cfg.dt, "source": cfg.source, "source_kind": args.source_kind, "coef_mode": args.coef_mode, "slab_rows": int(slab_rows), "kernel": int(kernel_used), "temporal_block": args.temporal_block or "default", "observers": list(cfg.observers),
                        "state_mb": 4 * cfg.n_pts * 8 / 1e6, "parallelism": "replicas x%d" % world,
+                       "extra_untimed_warmup": XW,
                        "l2": "inputs larger than L2 (two 537 MB state copies stream through a 126 MB L2)"
                        if 4 * cfg.n_pts * 8 > 2.5e8 else
                        ("state resident in shared memory between iterations (resident kernel): not an HBM measurement"
@@ -328,11 +399,23 @@ def main():
                     "note": "set_initial + set_source + step(K) + extract + get_state with pinned host buffers"},
             "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": ncu_traffic_bytes(cfg), "peak_source": peak_src,
+                         "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                          "kernel": "teuk_step_resident_kernel" if kernel_used == 2 else "teuk_step_kernel", "bytes_per_pt_step": BYTES_PER_PT_STEP},
         }
+        if K < 200:
+            line["note"] = "burst (%d steps: the SM clock has not settled under the power cap; sustained figures need >= 1000 steps)" % K
+        if not args.quick or not hbm_bound:
+            # the FP64 side: co-limit of the HBM roofline on config 5, THE limit where the state stays in L2 / on chip
+            alu = alu_peak(cfg, clocks)
+            line["roofline_alu"] = {"bound": "alu", "achieved": value / world, "peak": alu["gpts"], "unit": "GPts/s",
+                                    "frac": value / world / alu["gpts"], "lane_ops_per_s": alu["lane_ops_per_s"],
+                                    "fp64_instructions_per_pt_step": alu["fp64_per_pt_step"],
+                                    "peak_source": "teuk_measure_fp64 x the stage's SASS instruction mix (DESIGN.md 5.1), measured in this run after the timed region"}
+            if not hbm_bound:
+                line["roofline"] = dict(line["roofline_alu"], kernel=line["roofline"]["kernel"], traffic=None,
+                                        note="state fits in L2 / on chip: the FP64 pipe, not HBM, bounds this workload")
         if world == 1 and not args.no_cpu_baseline and not args.quick:
-            val, dt, threads, sample = time_oracle(cfg, 20, 3, args.oracle_rows, args.source_kind)
+            val, dt, threads, sample = time_oracle(cfg, 50, 3, args.oracle_rows, args.source_kind)
             line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample}
         print(json.dumps(line), flush=True)
     if world > 1:

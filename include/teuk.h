@@ -42,7 +42,10 @@ typedef enum {
   TEUK_OK = 0,
   TEUK_EINVAL = -1,     /* bad parameter, NULL where not allowed, trajectory too short for n     */
   TEUK_ENOMEM = -2,     /* host or device allocation failed                                       */
-  TEUK_ECUDA = -3,      /* CUDA error (sticky: the solver is unusable afterwards), or no device   */
+  TEUK_ECUDA = -3,      /* CUDA error (sticky: the solver is unusable afterwards), or no device.
+                           Every wait inside the kernels is bounded; one that times out (a faulted copy,
+                           a lost neighbour block) executes `trap`, which is reported here -- and, like any
+                           device-side fault, poisons the process's CUDA context, not only this solver   */
   TEUK_ENONFINITE = -4  /* a NaN/Inf was seen on a tapped waveform sample                         */
 } teuk_status;
 
@@ -71,6 +74,14 @@ typedef struct {
  * is current in the thread.  The Python binding calls it with torch's current device. */
 int teuk_select_device(int32_t device);
 
+/* FP64 issue-rate microbenchmark on the current device (no solver needed): the plain FP64 arithmetic of the
+ * right-hand sides is what the iteration spends its instructions on, and its ceiling is the
+ * co-limit of the HBM roofline.  kind 0 = DFMA reading two distinct registers, 1 = DFMA reading
+ * three distinct registers, 2 = DADD, 3 = DMUL; *lane_ops_per_s = lane-operations per second over the whole
+ * device with every SM saturated (one DFMA on one lane = 1).  Runs on the default stream and waits for it
+ * (a few milliseconds).  bench.py reports the "alu" roofline of the step kernel from these figures. */
+int teuk_measure_fp64(int32_t kind, double *lane_ops_per_s);
+
 /* Create a solver for Kerr parameters (a, M), |a| < M, M > 0, and n_modes (1..64) azimuthal
  * modes m[k] evolved together as independent fields ("decoupled"; one launch per
  * iteration covers all modes).  dt > 0 is the time step (the caller is responsible for stability:
@@ -81,18 +92,22 @@ int teuk_select_device(int32_t device);
 int teuk_create(teuk_solver **out, double a, double M, const int32_t *m, int32_t n_modes,
                 const teuk_grid *grid, double dt);
 
-/* Set Phi, Pi at t = 0 and reset the iteration counter, the simulated time and every observer's
- * recorded series.  NULL = zeros for that component.  ptr_is_device: 0 host, 1 device pointers. */
+/* Set the solution vector u = {Phi_R, Phi_I, Pi_R, Pi_I} at t = 0 -- Phi is the field of Eq. (2)
+ * (PAPER.md:84-88), Pi its "auxiliary momentum field" -- and reset the iteration counter, the
+ * simulated time and every observer's recorded series.  Each array [n_modes][n_r][n_theta], theta fastest;
+ * NULL = zeros for that component.  ptr_is_device: 0 host pointers (copied before the call returns), 1 device
+ * pointers (the layout change is enqueued on the solver's stream; keep the arrays alive until it has run). */
 int teuk_set_initial(teuk_solver *s, const double *phi_re, const double *phi_im,
                      const double *pi_re, const double *pi_im, int32_t ptr_is_device);
 
 /* Install (copy to the device) the trajectory table; NULL = source-free.  Host pointers. */
 int teuk_set_source(teuk_solver *s, const teuk_orbit *orbit);
 
-/* Enqueue n >= 0 iterations.  No host synchronisation (except the one-time slab-length measurement of
- * the first call, see "autotune"), no full-grid host transfer; observers are
- * tapped on the device after every iteration (sample time t = n_done*dt).  TEUK_EINVAL if a
- * source is installed and its table is too short. */
+/* Enqueue n >= 0 iterations of the two-step Lax-Wendroff scheme ("Each iteration consists of two
+ * steps": the half step Eq. (3), then the full step Eq. (4), with the boundary
+ * conditions of PAPER.md:104 and the source of PAPER.md:114).  No host synchronisation, no full-grid host
+ * transfer (per-step transfers cancel the GPU's gain); observers are tapped on the device after
+ * every iteration (sample time t = n_done*dt).  TEUK_EINVAL if a source is installed and its table is too short. */
 int teuk_step(teuk_solver *s, int64_t n);
 
 /* Observer at r* = rs_obs (x_0 <= rs_obs < x_{n_r-1}): w(t_n) = sum_j weights[j] *
@@ -106,7 +121,9 @@ int teuk_step(teuk_solver *s, int64_t n);
 int teuk_extract(teuk_solver *s, double rs_obs, const double *weights, double *t_out,
                  double *w_re, double *w_im, int64_t capacity, int64_t *n_written);
 
-/* Copy the current fields out (parity checks, checkpoints).  NULL = skip that component.
+/* Copy the current solution vector u^n = {Phi_R, Phi_I, Pi_R, Pi_I} out, same layout as
+ * teuk_set_initial (parity checks, checkpoints; the paper's temporal parallelisation restarts segments from zero
+ * data instead).  NULL = skip that component.
  * Host pointers: waits for the stream.  Device pointers: enqueued on the stream. */
 int teuk_get_state(teuk_solver *s, double *phi_re, double *phi_im, double *pi_re, double *pi_im,
                    int32_t ptr_is_device);
@@ -122,10 +139,13 @@ int teuk_get_state(teuk_solver *s, double *phi_re, double *phi_im, double *pi_re
  *   "stream"        a cudaStream_t cast to int64 (0 = back to the solver's own stream)
  *   "coef_mode"     0 = coefficients recomputed on the fly from 1D tables (default),
  *                   1 = coefficients streamed from precomputed 2D FP64 planes (n_theta <= 128 only)
- *   "slab_rows"     rows of r* marched by one warp (0 = automatic: measured once at the first teuk_step,
- *                   which then waits for a few untimed-by-the-caller trial launches into scratch memory); the
- *                   interior rows are dealt evenly to ceil((n_r - 2) / slab_rows) slabs
- *   "autotune"      1 = measure the slab length (default), 0 = use the two-wave heuristic
+ *   "slab_rows"     rows of r* marched by one warp (0 = automatic, see "autotune"); the interior rows are dealt
+ *                   evenly to ceil((n_r - 2) / slab_rows) slabs
+ *   "autotune"      1 (default) = the number of slabs of the marching kernels is MEASURED: a few dozen trial launches
+ *                   of the real kernel into the idle copy of the state (fields, counters and series untouched),
+ *                   timed inside teuk_create and again inside any teuk_set_option call that changes the launch
+ *                   shape ("kernel", "coef_mode", "temporal_block", "slab_rows", "autotune") -- calls that wait for
+ *                   the device anyway; teuk_step never does.  0 = use the two-wave heuristic
  *   "temporal_block" 1 = one iteration per kernel launch (default), 2 = two iterations per HBM round trip
  *                   (warp pairs; level n+1 stays in shared memory; same results bit for bit; needs kernel 0,
  *                   coef_mode 0, n_theta <= 128)

@@ -28,7 +28,23 @@ def build(force: bool = False) -> str:
     return _LIB
 
 
+# A second build of the SAME source whose only difference is rounding: FMA contraction allowed (the default build
+# forbids it).  tests/long_parity.py runs it next to the oracle to measure how far two correct implementations
+# of the iteration drift apart on long runs (the oracle-vs-oracle' arm); nothing else uses it.
+_LIB_FMA = os.path.join(_HERE, "liboracle_fma.so")
+CXXFLAGS_FMA = [f for f in CXXFLAGS if f != "-ffp-contract=off"] + ["-mfma", "-ffp-contract=fast"]
+
+
+def build_fma(force: bool = False) -> str:
+    if force or not os.path.exists(_LIB_FMA) or os.path.getmtime(_LIB_FMA) < os.path.getmtime(_SRC):
+        tmp = _LIB_FMA + ".tmp%d" % os.getpid()
+        subprocess.check_call(["g++"] + CXXFLAGS_FMA + ["-o", tmp, _SRC])
+        os.replace(tmp, _LIB_FMA)
+    return _LIB_FMA
+
+
 _lib = None
+_lib_fma = None
 _dp = C.POINTER(C.c_double)
 
 
@@ -36,10 +52,23 @@ def _p(a):
     return None if a is None else a.ctypes.data_as(_dp)
 
 
+def lib_fma():
+    """The differently rounded build (see build_fma)."""
+    global _lib_fma
+    if _lib_fma is None:
+        _lib_fma = _declare(C.CDLL(build_fma()))
+    return _lib_fma
+
+
 def lib():
     global _lib
     if _lib is None:
-        L = C.CDLL(build())
+        _lib = _declare(C.CDLL(build()))
+    return _lib
+
+
+def _declare(L):
+    if True:
         L.orc_r_of_rstar.argtypes = [C.c_double, C.c_double, C.c_double, _dp, _dp, _dp]
         L.orc_r_of_rstar.restype = None
         L.orc_coefficients.argtypes = [C.c_double, C.c_double, C.c_int, C.c_double, C.c_double, _dp]
@@ -74,8 +103,7 @@ def lib():
         L.orc_set_source_kind.restype = None
         L.orc_delta.argtypes = [C.c_int32, C.c_double, C.c_double]
         L.orc_delta.restype = C.c_double
-        _lib = L
-    return _lib
+    return L
 
 
 def r_of_rstar(M, a, x):
@@ -105,24 +133,25 @@ def delta(kind, y, h):
 class OracleSolver:
     """Plain CPU solver.  Arrays are [n_modes][n_r][n_theta] float64, theta fastest."""
 
-    def __init__(self, a, M, modes, rs_min, rs_max, n_r, n_theta, dt, outer_bc=0):
+    def __init__(self, a, M, modes, rs_min, rs_max, n_r, n_theta, dt, outer_bc=0, library=None):
+        self._L = library if library is not None else lib()
         self.modes = list(modes)
         self.shape = (len(self.modes), n_r, n_theta)
         m = (C.c_int32 * len(self.modes))(*self.modes)
-        self._h = lib().orc_create(a, M, m, len(self.modes), rs_min, rs_max, n_r, n_theta, dt, outer_bc)
+        self._h = self._L.orc_create(a, M, m, len(self.modes), rs_min, rs_max, n_r, n_theta, dt, outer_bc)
         if not self._h:
             raise ValueError("orc_create: invalid parameters")
         self.dt = dt
         self._keep = []
 
     @classmethod
-    def from_config(cls, cfg):
+    def from_config(cls, cfg, library=None):
         return cls(cfg.a, cfg.M, cfg.modes, cfg.rs_min, cfg.rs_max, cfg.n_r, cfg.n_theta, cfg.dt,
-                   cfg.outer_bc)
+                   cfg.outer_bc, library=library)
 
     def close(self):
         if self._h:
-            lib().orc_destroy(self._h)
+            self._L.orc_destroy(self._h)
             self._h = None
 
     def __del__(self):
@@ -138,64 +167,64 @@ class OracleSolver:
 
     def set_initial(self, phi_re=None, phi_im=None, pi_re=None, pi_im=None):
         arrs = [self._arr(a, self.shape) for a in (phi_re, phi_im, pi_re, pi_im)]
-        lib().orc_set_initial(self._h, *[_p(a) for a in arrs])
+        self._L.orc_set_initial(self._h, *[_p(a) for a in arrs])
 
     def set_source(self, orbit):
         if orbit is None:
-            lib().orc_set_source(self._h, 0, None, None, None, None, 1.0, 1.0, 0)
+            self._L.orc_set_source(self._h, 0, None, None, None, None, 1.0, 1.0, 0)
             return
         ns = int(orbit["n_samples"])
         xs = self._arr(orbit["rs_p"], (ns,))
         th = self._arr(orbit["theta_p"], (ns,))
         ar = self._arr(orbit["amp_re"], (len(self.modes), ns))
         ai = self._arr(orbit["amp_im"], (len(self.modes), ns))
-        lib().orc_set_source(self._h, ns, _p(xs), _p(th), _p(ar), _p(ai), float(orbit["sigma_r"]),
+        self._L.orc_set_source(self._h, ns, _p(xs), _p(th), _p(ar), _p(ai), float(orbit["sigma_r"]),
                              float(orbit["sigma_theta"]), int(orbit["half_window"]))
 
     def set_source_kind(self, kind):
         """0 Gaussian (default), 1 two-point, 2 four-point discrete delta."""
         if kind not in (0, 1, 2):
             raise ValueError("source kind must be 0, 1 or 2")
-        lib().orc_set_source_kind(self._h, int(kind))
+        self._L.orc_set_source_kind(self._h, int(kind))
 
     def add_observer(self, rs_obs, weights=None):
         w = self._arr(weights, (self.shape[2],))
-        k = lib().orc_add_observer(self._h, float(rs_obs), _p(w))
+        k = self._L.orc_add_observer(self._h, float(rs_obs), _p(w))
         if k < 0:
             raise ValueError("observer outside the grid")
         return k
 
     def step(self, n=1):
-        if lib().orc_step(self._h, int(n)) != 0:
+        if self._L.orc_step(self._h, int(n)) != 0:
             raise ValueError("trajectory table too short")
 
     @property
     def step_count(self):
-        return lib().orc_step_count(self._h)
+        return self._L.orc_step_count(self._h)
 
     def get_state(self):
         out = [np.empty(self.shape) for _ in range(4)]
-        lib().orc_get_state(self._h, *[_p(a) for a in out])
+        self._L.orc_get_state(self._h, *[_p(a) for a in out])
         return tuple(out)
 
     def get_half(self):
         shp = (self.shape[0], self.shape[1] - 1, self.shape[2])
         out = [np.empty(shp) for _ in range(4)]
-        lib().orc_get_half(self._h, *[_p(a) for a in out])
+        self._L.orc_get_half(self._h, *[_p(a) for a in out])
         return tuple(out)
 
     def waveform(self, obs=0):
         """(t[n], w[n][n_modes] complex) recorded so far."""
-        n = lib().orc_get_waveform(self._h, obs, None, None, None, 0)
+        n = self._L.orc_get_waveform(self._h, obs, None, None, None, 0)
         t = np.empty(n)
         wr = np.empty((n, self.shape[0]))
         wi = np.empty((n, self.shape[0]))
-        lib().orc_get_waveform(self._h, obs, _p(t), _p(wr), _p(wi), n)
+        self._L.orc_get_waveform(self._h, obs, _p(t), _p(wr), _p(wi), n)
         return t, wr + 1j * wi
 
     def source_field(self, mode_index, sample, half):
         rows = self.shape[1] - 1 if half else self.shape[1]
         re = np.empty((rows, self.shape[2]))
         im = np.empty((rows, self.shape[2]))
-        lib().orc_source_field(self._h, mode_index, sample, 1 if half else 0, _p(re), _p(im))
+        self._L.orc_source_field(self._h, mode_index, sample, 1 if half else 0, _p(re), _p(im))
         return re + 1j * im

@@ -28,6 +28,7 @@ cudaError_t teuk_launch_bump(long long* d_base, long long inc, cudaStream_t st);
 cudaError_t teuk_launch_set_base(long long* d_base, long long v, cudaStream_t st);
 cudaError_t teuk_launch_pack(double* u, double* const src[4], size_t n_rows, int nth, cudaStream_t st);
 cudaError_t teuk_launch_unpack(const double* u, double* const dst[4], size_t n_rows, int nth, cudaStream_t st);
+double teuk_fp64_rate(int kind, cudaError_t* err);
 
 namespace {
 
@@ -333,6 +334,8 @@ int drain_rings(teuk_solver* s) {
   return TEUK_OK;
 }
 
+int tune_if_needed(teuk_solver* s);
+
 int build_tables(teuk_solver* s) {
   CK(teuk_launch_tables(s->d_rtab, s->d_ttab, s->d_m, s->n_modes, s->n_r, s->n_theta, s->rs_min, s->dx,
                         s->dth, s->M, s->a, s->stream),
@@ -389,6 +392,20 @@ int teuk_select_device(int32_t device) {
     cudaGetLastError();
     return fail(nullptr, TEUK_ECUDA, "teuk_select_device: cudaSetDevice failed");
   }
+  return TEUK_OK;
+}
+
+int teuk_measure_fp64(int32_t kind, double* lane_ops_per_s) {
+  if (!lane_ops_per_s || kind < 0 || kind > 3) return fail(nullptr, TEUK_EINVAL, "teuk_measure_fp64: kind must be 0..3, output not NULL");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    return fail(nullptr, TEUK_ECUDA, "teuk_measure_fp64: no CUDA device (this library has no CPU fallback)");
+  }
+  cudaError_t e = cudaSuccess;
+  const double r = teuk_fp64_rate(kind, &e);
+  if (e != cudaSuccess) return cuda_fail(nullptr, e, "teuk_measure_fp64");
+  *lane_ops_per_s = r;
   return TEUK_OK;
 }
 
@@ -453,6 +470,8 @@ int teuk_create(teuk_solver** out, double a, double M, const int32_t* m, int32_t
     if (rc != TEUK_OK) break;
     cudaError_t e = cudaStreamSynchronize(s->stream);
     if (e != cudaSuccess) { rc = cuda_fail(s, e, "teuk_create sync"); break; }
+    rc = tune_if_needed(s);     // launch shape of the marching kernel, measured once on the zeroed state
+    if (rc != TEUK_OK) break;
   } while (0);
   if (rc != TEUK_OK) {
     snprintf(g_create_error, sizeof(g_create_error), "%s", s->err);
@@ -623,6 +642,8 @@ int tune_slab_rows(teuk_solver* s, int tb) {
     StepParams p;
     fill_params(s, &p, s->cur, (int)(s->step - s->base_on_device), 0, tb);
     p.tap_enable2 = 0;
+    p.has_source = 0;      // trial launches read nothing but the state and the tables (no trajectory sample, no observer)
+    p.n_obs = 0;
     auto launch = [&]() { return tb == 2 ? teuk_launch_step_tb2(p, s->stream) : teuk_launch_step(p, s->stream); };
     cudaError_t e = launch();                                      // warm-up
     float ms = 0.f;
@@ -652,6 +673,24 @@ int tune_slab_rows(teuk_solver* s, int tb) {
   if (tb == 2) s->tuned_rows2 = best_slabs; else s->tuned_rows = best_slabs;
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
+  return TEUK_OK;
+}
+
+// Measure the launch shape of the marching kernels the solver would run now, if it has not been measured yet.
+// Called from teuk_create and teuk_set_option (both wait for the stream anyway), never from teuk_step.
+int tune_if_needed(teuk_solver* s) {
+  int rr_ = 0, nc_ = 0;
+  if (!s->autotune || s->slab_rows_opt != 0 || resident_active(s, &rr_, &nc_)) return TEUK_OK;
+  if (s->tuned_rows == 0) {
+    const int rc = tune_slab_rows(s, 1);
+    if (rc != TEUK_OK) return rc;
+    drop_graph(s);
+  }
+  if (tb2_active(s) && s->tuned_rows2 == 0) {
+    const int rc = tune_slab_rows(s, 2);
+    if (rc != TEUK_OK) return rc;
+    drop_graph(s);
+  }
   return TEUK_OK;
 }
 
@@ -775,19 +814,6 @@ int teuk_step(teuk_solver* s, int64_t n) {
   if (n < 0) return fail(s, TEUK_EINVAL, "teuk_step: n < 0");
   if (s->has_source && 2 * (s->step + n) > s->n_samples)
     return fail(s, TEUK_EINVAL, "teuk_step: trajectory table too short for n more iterations");
-  int rr_ = 0, nc_ = 0;
-  if (n > 0 && !resident_active(s, &rr_, &nc_) && s->autotune && s->slab_rows_opt == 0 && (s->base_on_device <= s->step)) {
-    if (s->tuned_rows == 0) {
-      const int rc = tune_slab_rows(s, 1);
-      if (rc != TEUK_OK) return rc;
-      drop_graph(s);
-    }
-    if (tb2_active(s) && s->tuned_rows2 == 0) {
-      const int rc = tune_slab_rows(s, 2);
-      if (rc != TEUK_OK) return rc;
-      drop_graph(s);
-    }
-  }
   long long remaining = n;
   while (remaining > 0) {
     long long room = remaining;
@@ -835,8 +861,10 @@ int teuk_extract(teuk_solver* s, double rs_obs, const double* weights, double* t
     if (weights) memcpy(w.data(), weights, (size_t)s->n_theta * sizeof(double));
     CK(cudaMalloc((void**)&o->d_weights, (size_t)s->n_theta * sizeof(double)), "extract: alloc");
     CK(cudaMalloc((void**)&o->d_ring, (size_t)kRingCap * s->n_modes * 2 * sizeof(double)), "extract: alloc");
-    CK(cudaMemcpy(o->d_weights, w.data(), (size_t)s->n_theta * sizeof(double), cudaMemcpyHostToDevice), "extract: H2D");
-    CK(cudaMemset(o->d_ring, 0, (size_t)kRingCap * s->n_modes * 2 * sizeof(double)), "extract: zero");
+    // on the solver's stream (the legacy default stream is not ordered against it), then wait: `w` is local
+    CK(cudaMemcpyAsync(o->d_weights, w.data(), (size_t)s->n_theta * sizeof(double), cudaMemcpyHostToDevice, s->stream), "extract: H2D");
+    CK(cudaMemsetAsync(o->d_ring, 0, (size_t)kRingCap * s->n_modes * 2 * sizeof(double), s->stream), "extract: zero");
+    CK(cudaStreamSynchronize(s->stream), "extract: sync");
     s->n_obs += 1;
     return TEUK_OK;
   }
@@ -847,7 +875,8 @@ int teuk_extract(teuk_solver* s, double rs_obs, const double* weights, double* t
   CK(cudaStreamSynchronize(s->copy_stream), "extract: sync copies");
   CK(cudaStreamSynchronize(s->stream), "extract: sync");
   int nonfinite = 0;
-  CK(cudaMemcpy(&nonfinite, s->d_nonfinite, sizeof(int), cudaMemcpyDeviceToHost), "extract: flag");
+  CK(cudaMemcpyAsync(&nonfinite, s->d_nonfinite, sizeof(int), cudaMemcpyDeviceToHost, s->stream), "extract: flag");
+  CK(cudaStreamSynchronize(s->stream), "extract: flag sync");
   ObsHost* o = &s->obs[q];
   int64_t written = 0;
   size_t ci = 0;
@@ -957,8 +986,15 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
   } else {
     return fail(s, TEUK_EINVAL, "teuk_set_option: unknown key");
   }
-  if (strcmp(key, "stream") != 0) { s->tuned_rows = 0; s->tuned_rows2 = 0; }   // launch shape may change: measure again
   drop_graph(s);
+  // options that change the launch shape of the marching kernels: measure it again, here, so that teuk_step
+  // never has to wait for the device
+  if (!strcmp(key, "kernel") || !strcmp(key, "coef_mode") || !strcmp(key, "temporal_block") ||
+      !strcmp(key, "slab_rows") || !strcmp(key, "autotune")) {
+    s->tuned_rows = 0;
+    s->tuned_rows2 = 0;
+    return tune_if_needed(s);
+  }
   return TEUK_OK;
 }
 

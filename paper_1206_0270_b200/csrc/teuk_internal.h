@@ -1,5 +1,5 @@
 // teuk_internal.h -- device data layout and kernel parameter blocks of libteuk.so (sm_100a).
-// Product code: shares nothing with oracle/.
+// Product code: shares nothing with the test checker.
 //
 // HBM layout:
 //   state U[2] (ping-pong), each [n_modes][n_r][4][n_theta] FP64, theta fastest; the 4 components

@@ -2,7 +2,7 @@
 // teuk_resident.cu: resident kernel): register rows, the Lax-Wendroff stage (Eq. 3-4) in the
 // scaled variables of DESIGN.md "Stage arithmetic", the source deposit, the waveform tap
 // and the TMA / mbarrier helpers.  Every kernel calls the SAME lw_stage / add_source / tap, which
-// is what makes their fields bit-identical.  Product code: shares nothing with oracle/.
+// is what makes their fields bit-identical.  Product code: shares nothing with the test checker.
 #ifndef TEUK_STAGE_CUH_
 #define TEUK_STAGE_CUH_
 

@@ -1,7 +1,7 @@
 // teuk_tables.cu -- setup kernels (run once per teuk_create, off the hot loop): the separable
 // factors of the coefficient matrices D and S of PAPER.md:102, derived from the Teukolsky
 // equation PAPER.md:68-76 (Eq. 1) with Psi = e^{im phi~} r^3 Phi and s = -2.
-// DESIGN.md section "Coefficients" gives the algebra; the product never calls the CPU oracle.
+// DESIGN.md section "Coefficients" gives the algebra; the product never calls the CPU checker of the tests.
 #include <cuda_runtime.h>
 #include <math.h>
 

@@ -7,7 +7,8 @@ from the sudden switch-on leaves the grid during the overlap, and only the sampl
 kept.  The waveforms of all segments are then patched together.  The other independent units of SURVEY.md 8(e)
 are covered the same way: azimuthal modes (`run_modes`) and the resolutions of a Richardson
 sequence (`run_richardson`).  Nothing here is on the hot path: it plans the replicas, hands
-each one to a solver built by `solver_factory` (the CUDA `Solver` by default) and assembles the series.  With torch.distributed initialised, rank r takes segments r, r + world, ...
+each one to a solver built by `solver_factory` (the CUDA `Solver` by default; anything with its set_initial /
+set_source / set_option / add_observer / step / extract / close methods) and assembles the series.  With torch.distributed initialised, rank r takes segments r, r + world, ...
 and rank 0 gathers the pieces (no collective during the evolution).
 """
 from __future__ import annotations
@@ -50,10 +51,7 @@ def run_segment(cfg: wl.Config, seg: Segment, x_obs: float, weights, solver_fact
         s.set_source(wl.orbit_table(cfg, n_steps=n, t0=seg.t0))
         s.add_observer(x_obs, weights)
         s.step(n)
-        if hasattr(s, "extract"):
-            t, w = s.extract(x_obs)
-        else:                                             # oracle-style interface (tests)
-            t, w = s.waveform(0)
+        t, w = s.extract(x_obs)
     finally:
         s.close()
     keep = slice(seg.lead, n)
@@ -108,13 +106,10 @@ def _evolve(cfg: wl.Config, steps: int, x_obs: float, weights, factory: Callable
         if cfg.source:
             s.set_source(orbit if orbit is not None else wl.orbit_table(cfg, n_steps=steps))
             if source_kind:
-                if hasattr(s, "set_source_kind"):
-                    s.set_source_kind(source_kind)
-                else:
-                    s.set_option("source_kind", source_kind)
+                s.set_option("source_kind", source_kind)
         s.add_observer(x_obs, weights)
         s.step(steps)
-        return s.extract(x_obs) if hasattr(s, "extract") else s.waveform(0)
+        return s.extract(x_obs)
     finally:
         s.close()
 

@@ -1,7 +1,7 @@
 """Thin ctypes binding of libteuk.so (include/teuk.h): argument marshalling only.
 
 Every step of the path runs in the CUDA kernels of csrc/; there is no CPU fallback and this module
-never imports oracle/.  If the shared library is missing or has no CUDA device, calls fail loudly.
+imports nothing but the library.  If the shared library is missing or has no CUDA device, calls fail loudly.
 PyTorch tensors may be passed wherever a device array is expected (their data_ptr() is used) and
 `Solver.use_torch_stream()` makes the solver enqueue on torch's current stream.
 """
@@ -13,10 +13,10 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("TEUK_LIB") or os.path.join(_HERE, "libteuk.so")  # TEUK_LIB: development override
+LIB_PATH = os.path.join(_HERE, "libteuk.so")
 
 TEUK_OK, TEUK_EINVAL, TEUK_ENOMEM, TEUK_ECUDA, TEUK_ENONFINITE = 0, -1, -2, -3, -4
-SYMBOLS = ["teuk_select_device", "teuk_create", "teuk_set_initial", "teuk_set_source", "teuk_step", "teuk_extract",
+SYMBOLS = ["teuk_select_device", "teuk_measure_fp64", "teuk_create", "teuk_set_initial", "teuk_set_source", "teuk_step", "teuk_extract",
            "teuk_get_state", "teuk_set_option", "teuk_get_stat", "teuk_sync", "teuk_destroy",
            "teuk_last_error"]
 
@@ -55,6 +55,7 @@ def load():
     L.teuk_create.argtypes = [C.POINTER(vp), C.c_double, C.c_double, C.POINTER(C.c_int32), C.c_int32,
                               C.POINTER(teuk_grid), C.c_double]
     L.teuk_select_device.argtypes = [C.c_int32]
+    L.teuk_measure_fp64.argtypes = [C.c_int32, _dp]
     L.teuk_set_initial.argtypes = [vp, vp, vp, vp, vp, C.c_int32]
     L.teuk_set_source.argtypes = [vp, C.POINTER(teuk_orbit)]
     L.teuk_step.argtypes = [vp, C.c_int64]
@@ -83,10 +84,22 @@ def _ptr(a):
     return C.c_void_p(a.ctypes.data), False
 
 
+def measure_fp64(kind):
+    """teuk_measure_fp64: lane-operations per second of FP64 instruction kind 0..3 on the current device."""
+    v = C.c_double(0.0)
+    rc = load().teuk_measure_fp64(int(kind), C.byref(v))
+    if rc != TEUK_OK:
+        raise TeukError(rc, load().teuk_last_error(None).decode())
+    return v.value
+
+
 class Solver:
     """One teuk_solver handle.  Field arrays are [n_modes][n_r][n_theta] float64, theta fastest."""
 
     def __init__(self, a, M, modes, rs_min, rs_max, n_r, n_theta, dt, device=None):
+        """`device`: CUDA device index (default: torch's current device if the caller uses torch, else the device
+        current in the thread).  Selecting it calls teuk_select_device, which makes that device current in the
+        calling thread for the library's CUDA runtime and leaves it so (like torch.cuda.set_device)."""
         self._lib = load()
         if device is None:
             import sys
@@ -129,11 +142,16 @@ class Solver:
         except Exception:
             pass
 
-    def _fields(self, arrs):
+    def _fields(self, arrs, output=False):
         ptrs, dev = [], None
         for a in arrs:
             if a is not None and not hasattr(a, "data_ptr"):
-                a = np.ascontiguousarray(a, dtype=np.float64)
+                if output:      # the library writes through the pointer: a hidden copy would be filled instead
+                    if not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags.c_contiguous
+                            and a.flags.writeable):
+                        raise TypeError("output arrays must be writeable C-contiguous float64 numpy arrays")
+                else:
+                    a = np.ascontiguousarray(a, dtype=np.float64)
                 assert a.shape == self.shape, (a.shape, self.shape)
             elif a is not None:
                 assert tuple(a.shape) == self.shape and a.is_contiguous() and a.element_size() == 8
@@ -187,7 +205,7 @@ class Solver:
         """Host copy of (phi_re, phi_im, pi_re, pi_im); or fill 4 given arrays/tensors."""
         if out is None:
             out = [np.empty(self.shape) for _ in range(4)]
-        ptrs, dev = self._fields(list(out))
+        ptrs, dev = self._fields(list(out), output=True)
         self._check(self._lib.teuk_get_state(self._h, *[p for p, _ in ptrs], 1 if dev else 0))
         return tuple(out)
 

@@ -1,7 +1,7 @@
 """Seeded synthetic workloads: the five BASELINE.json configs with every free choice fixed.
 
-This module is the ONLY code shared by the CPU oracle (``oracle/``) and the CUDA path
-(``paper_1206_0270_b200/csrc``).  It generates *inputs* (grids' parameters, initial
+This module is the ONLY code the CUDA path (``paper_1206_0270_b200/csrc``) shares with the CPU checker the
+tests compare it with.  It generates *inputs* (grids' parameters, initial
 data, sampled particle trajectories with their source amplitudes, observer weights).  It
 contains none of the solver's arithmetic: no Lax-Wendroff stage, no Teukolsky coefficient,
 no tortoise-coordinate *inversion*, no Gaussian deposit.

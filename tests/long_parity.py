@@ -1,11 +1,21 @@
 #!/usr/bin/env python
 """Full-length parity runs (not collected by pytest: minutes to hours of host-core time).
 
-  python tests/long_parity.py --config 3 [--steps N] [--out gpurun_out/long_parity.jsonl]
+  python tests/long_parity.py --config 3 [--steps N] [--arm gpu|oracle2] [--checkpoints 8] [--out FILE]
 
-Runs the CUDA path (through the C ABI) and the CPU oracle on the same seeded inputs for the config's
-step count (or --steps), then reports relative L2 errors of Phi, Pi and every observer's waveform
-(protocol of SURVEY.md 8(d) / DESIGN.md section 6) and both throughputs.  Appends one JSON line."""
+Protocol of SURVEY.md 8(d) / DESIGN.md section 6: relative L2 distances of Phi, of Pi and of every observer's
+waveform after the config's step count (or --steps), on the seeded inputs of paper_1206_0270_b200/workloads.py.
+Two arms, each appending ONE JSON line to profiles/r2_long_parity.jsonl (or --out):
+
+  --arm gpu      (needs the GPU) the CUDA path through the C ABI against the CPU oracle ("gpu_vs_oracle"), and the
+                 CUDA path against itself with differently ROUNDED coefficients, coef_mode 1 ("gpu_vs_gpu2");
+  --arm oracle2  (CPU only) the oracle against a second build of the same source with FMA contraction allowed
+                 ("oracle_vs_oracle2": oracle/oracle.py build_fma) -- the distance two correct implementations of
+                 the iteration reach through rounding alone, whatever the hardware.
+
+All solvers advance in lockstep and are compared at --checkpoints evenly spaced iteration counts, so a record
+also shows up to which iteration the 1e-10 bar of BASELINE.json holds ("bar_holds_until").  The waveform distances
+are over the samples recorded up to each checkpoint."""
 import argparse
 import json
 import os
@@ -18,7 +28,9 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 sys.path.insert(0, ROOT)
 
 from oracle import oracle as orc  # noqa: E402
-from paper_1206_0270_b200 import Solver, workloads as wl  # noqa: E402
+from paper_1206_0270_b200 import workloads as wl  # noqa: E402
+
+BAR = 1e-10
 
 
 def rel(got, ref):
@@ -26,75 +38,148 @@ def rel(got, ref):
     return float(np.linalg.norm(got - ref) / den) if den > 0 else float(np.linalg.norm(got))
 
 
+def state_distance(sa, sb):
+    """(rel-L2 Phi, rel-L2 Pi, ||Phi||, ||Pi||) of state sa against the reference sb."""
+    phi_a, phi_b = sa[0] + 1j * sa[1], sb[0] + 1j * sb[1]
+    pi_a, pi_b = sa[2] + 1j * sa[3], sb[2] + 1j * sb[3]
+    return rel(phi_a, phi_b), rel(pi_a, pi_b), float(np.linalg.norm(phi_b)), float(np.linalg.norm(pi_b))
+
+
+def wave_distance(wa, wb):
+    n = float(np.linalg.norm(wb))
+    return "silent" if n < 1e-200 else rel(wa, wb)
+
+
+class Series:
+    """Accumulates the waveform of one observer across extract() calls (the CUDA binding hands out increments)."""
+
+    def __init__(self):
+        self.w = []
+
+    def add(self, w):
+        self.w.append(np.asarray(w))
+
+    def all(self):
+        return np.concatenate(self.w) if self.w else np.empty((0, 1), dtype=complex)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", type=int, required=True)
     ap.add_argument("--steps", type=int, default=0)
-    ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "long_parity.jsonl"))
-    ap.add_argument("--no-oracle", action="store_true", help="GPU only: report the rounding sensitivity")
-    ap.add_argument("--no-sensitivity", action="store_true")
+    ap.add_argument("--arm", default="gpu", choices=["gpu", "oracle2"])
+    ap.add_argument("--checkpoints", type=int, default=8)
+    ap.add_argument("--out", default=os.path.join(ROOT, "profiles", "r2_long_parity.jsonl"))
+    ap.add_argument("--no-oracle", action="store_true", help="--arm gpu without the oracle: gpu_vs_gpu2 only")
+    ap.add_argument("--no-sensitivity", action="store_true", help="--arm gpu without the coef_mode 1 run")
     a = ap.parse_args()
     cfg = wl.CONFIGS[a.config]
     steps = a.steps or cfg.steps
     ini = wl.initial_data(cfg)
     orbit = wl.orbit_table(cfg, n_steps=steps)
     W = wl.observer_weights(cfg)
-    g = Solver.from_config(cfg)
-    g.set_initial(*ini)
-    g.set_source(orbit)
-    for x in cfg.observers:
-        g.add_observer(x, W)
-    g.sync()
-    kernel = g.stat("kernel")     # 2 = resident kernel (state on chip), 0 = marching kernel
-    t0 = time.perf_counter()
-    g.step(steps)
-    g.sync()
-    t_gpu = time.perf_counter() - t0
-    sg = g.get_state()
-    wg = [g.extract(x) for x in cfg.observers]
-    g.close()
-    # rounding sensitivity: the same CUDA path with differently rounded coefficients (streamed planes
-    # instead of per-point rebuilds); any two non-bit-identical implementations differ at least this much
-    sens = None
-    if cfg.n_theta <= 128 and not a.no_sensitivity:
-        g2 = Solver.from_config(cfg)
-        g2.set_option("coef_mode", 1)
-        g2.set_initial(*ini)
-        g2.set_source(orbit)
-        g2.step(steps)
-        s2 = g2.get_state()
-        g2.close()
-        sens = {"rel_l2_phi": rel(s2[0] + 1j * s2[1], sg[0] + 1j * sg[1]),
-                "rel_l2_pi": rel(s2[2] + 1j * s2[3], sg[2] + 1j * sg[3])}
-    if a.no_oracle:
-        print(json.dumps({"config": cfg.cid, "steps": steps, "gpu_gpts": cfg.n_pts * steps / t_gpu / 1e9,
-                          "sensitivity_coef_mode_0_vs_1": sens}))
-        return
-    o = orc.OracleSolver.from_config(cfg)
-    o.set_initial(*ini)
-    o.set_source(orbit)
-    for x in cfg.observers:
-        o.add_observer(x, W)
-    t0 = time.perf_counter()
-    o.step(steps)
-    t_cpu = time.perf_counter() - t0
-    so = o.get_state()
-    wo = [o.waveform(k) for k in range(len(cfg.observers))]
-    o.close()
-    phi_g, phi_o = sg[0] + 1j * sg[1], so[0] + 1j * so[1]
-    pi_g, pi_o = sg[2] + 1j * sg[3], so[2] + 1j * so[3]
-    res = {
-        "config": cfg.cid, "workload": cfg.name, "steps": steps, "full_length": steps == cfg.steps, "kernel": int(kernel),
-        "rel_l2_phi": rel(phi_g, phi_o), "rel_l2_pi": rel(pi_g, pi_o),
-        "norm_phi": float(np.linalg.norm(phi_o)), "norm_pi": float(np.linalg.norm(pi_o)),
-        "waveforms": [{"x_obs": x, "rel_l2": (rel(g_[1], o_[1]) if np.linalg.norm(o_[1]) >= 1e-200 else "silent"),
-                       "norm": float(np.linalg.norm(o_[1])), "samples": int(len(o_[0]))}
-                      for x, g_, o_ in zip(cfg.observers, wg, wo)],
-        "gpu_gpts": cfg.n_pts * steps / t_gpu / 1e9, "oracle_mpts": cfg.n_pts * steps / t_cpu / 1e6,
-        "oracle_threads": int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1)),
-        "oracle_seconds": t_cpu,
-        "sensitivity_coef_mode_0_vs_1": sens,
-    }
+    ncp = max(1, min(a.checkpoints, steps))
+    marks = sorted(set(round(steps * (k + 1) / ncp) for k in range(ncp)))
+
+    def make_oracle(library=None):
+        o = orc.OracleSolver.from_config(cfg, library=library)
+        o.set_initial(*ini)
+        o.set_source(orbit)
+        for x in cfg.observers:
+            o.add_observer(x, W)
+        return o
+
+    res = {"config": cfg.cid, "workload": cfg.name, "steps": steps, "full_length": steps == cfg.steps,
+           "arm": a.arm, "observers": list(cfg.observers), "checkpoints": marks,
+           "threads": int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))}
+    pairs = {}          # name -> list of per-checkpoint dicts
+    t_cpu = t_gpu = 0.0
+    if a.arm == "oracle2":
+        o1, o2 = make_oracle(), make_oracle(orc.lib_fma())
+        done = 0
+        for mk in marks:
+            t0 = time.perf_counter()
+            o1.step(mk - done)
+            t_cpu += time.perf_counter() - t0
+            o2.step(mk - done)
+            done = mk
+            dphi, dpi, nphi, npi = state_distance(o2.get_state(), o1.get_state())
+            waves = [wave_distance(o2.waveform(k)[1], o1.waveform(k)[1]) for k in range(len(cfg.observers))]
+            pairs.setdefault("oracle_vs_oracle2", []).append(
+                {"n": mk, "rel_l2_phi": dphi, "rel_l2_pi": dpi, "norm_phi": nphi, "norm_pi": npi, "waveforms": waves})
+            print("n=%d oracle_vs_oracle2 phi %.2e pi %.2e w %s" % (mk, dphi, dpi, waves), flush=True)
+        res["oracle2_build"] = " ".join(orc.CXXFLAGS_FMA)
+        o1.close()
+        o2.close()
+    else:
+        from paper_1206_0270_b200 import Solver
+
+        def make_gpu(coef_mode):
+            g = Solver.from_config(cfg)
+            if coef_mode:
+                g.set_option("coef_mode", 1)
+            g.set_initial(*ini)
+            g.set_source(orbit)
+            for x in cfg.observers:
+                g.add_observer(x, W)
+            return g
+
+        g = make_gpu(0)
+        res["kernel"] = int(g.stat("kernel"))     # 2 = resident kernel (state on chip), 0 = marching kernel
+        g2 = None if (a.no_sensitivity or cfg.n_theta > 128) else make_gpu(1)
+        o = None if a.no_oracle else make_oracle()
+        sg = [Series() for _ in cfg.observers]
+        sg2 = [Series() for _ in cfg.observers]
+        done = 0
+        for mk in marks:
+            g.sync()
+            t0 = time.perf_counter()
+            g.step(mk - done)
+            g.sync()
+            t_gpu += time.perf_counter() - t0
+            if g2 is not None:
+                g2.step(mk - done)
+            if o is not None:
+                t0 = time.perf_counter()
+                o.step(mk - done)
+                t_cpu += time.perf_counter() - t0
+            done = mk
+            st = g.get_state()
+            for k, x in enumerate(cfg.observers):
+                sg[k].add(g.extract(x)[1])
+                if g2 is not None:
+                    sg2[k].add(g2.extract(x)[1])
+            if o is not None:
+                dphi, dpi, nphi, npi = state_distance(st, o.get_state())
+                waves = [wave_distance(sg[k].all(), o.waveform(k)[1]) for k in range(len(cfg.observers))]
+                pairs.setdefault("gpu_vs_oracle", []).append(
+                    {"n": mk, "rel_l2_phi": dphi, "rel_l2_pi": dpi, "norm_phi": nphi, "norm_pi": npi, "waveforms": waves})
+                print("n=%d gpu_vs_oracle phi %.2e pi %.2e w %s" % (mk, dphi, dpi, waves), flush=True)
+            if g2 is not None:
+                dphi, dpi, nphi, npi = state_distance(g2.get_state(), st)
+                waves = [wave_distance(sg2[k].all(), sg[k].all()) for k in range(len(cfg.observers))]
+                pairs.setdefault("gpu_vs_gpu2", []).append(
+                    {"n": mk, "rel_l2_phi": dphi, "rel_l2_pi": dpi, "norm_phi": nphi, "norm_pi": npi, "waveforms": waves})
+                print("n=%d gpu_vs_gpu2 phi %.2e pi %.2e w %s" % (mk, dphi, dpi, waves), flush=True)
+        res["gpu_gpts"] = cfg.n_pts * steps / t_gpu / 1e9
+        g.close()
+        if g2 is not None:
+            g2.close()
+        if o is not None:
+            o.close()
+    if t_cpu > 0:
+        res["oracle_mpts"] = cfg.n_pts * steps / t_cpu / 1e6
+        res["oracle_seconds"] = t_cpu
+    for name, cps in pairs.items():
+        last = cps[-1]
+        holds = 0
+        for c in cps:      # largest checkpoint up to which Phi, Pi and every audible waveform are within the bar
+            ws = [w for w in c["waveforms"] if w != "silent"]
+            if max([c["rel_l2_phi"], c["rel_l2_pi"]] + ws) <= BAR:
+                holds = c["n"]
+            else:
+                break
+        res[name] = {"final": last, "bar_holds_until": holds, "bar": BAR, "history": cps}
     os.makedirs(os.path.dirname(a.out), exist_ok=True)
     with open(a.out, "a") as f:
         f.write(json.dumps(res) + "\n")

@@ -21,7 +21,7 @@ def lib_path():
 def _declared():
     text = open(os.path.join(ROOT, "include", "teuk.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(teuk_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(teuk_[a-z_0-9]+)\s*\(", text)))
 
 
 def test_header_symbols_are_exported(lib_path):
@@ -70,6 +70,8 @@ def test_product_never_references_the_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle", text, flags=re.M), f
                 assert "liboracle" not in text and "orc_" not in text, f
+                assert "oracle" not in text.lower(), "%s mentions the oracle: the product has no path shaped around it" % f
+                assert "TEUK_LIB" not in text, "%s: no library override in the product" % f
     code = "import sys; import paper_1206_0270_b200; assert not any(m.startswith('oracle') for m in sys.modules)"
     subprocess.check_call([sys.executable, "-c", code], cwd=ROOT)
     oracle_src = open(os.path.join(ROOT, "oracle", "teuk_oracle.cpp")).read()

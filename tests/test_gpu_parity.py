@@ -195,9 +195,12 @@ def test_programmatic_dependent_launch_is_bitwise_identical(orc, teuk):
 def test_ring_buffer_wraps_and_drains(orc, teuk):
     """More iterations than the device ring holds (32768): samples are drained by async copies."""
     cfg = wl.CONFIGS[1].scaled(name="ring", n_r=24, n_theta=8, rs_min=10.0, rs_max=19.2, steps=40000,
-                               dt_over_dx=0.02, observers=(12.3,))
+                               dt_over_dx=0.005, observers=(12.3,))
     res = run_pair(orc, teuk, cfg, 40000, chunks=[5, 32763, 1, 7231])
-    check_pair(res, tol=1e-9)   # 40000 iterations of a 24-point-wide cavity: round-off accumulates
+    # at the bar of BASELINE.json (1e-10): two roundings of the oracle itself (default build vs FMA-contracted
+    # build) end 6e-15 apart on this run (9e-15 in Pi); with dt = 0.02 dx the 24-point cavity amplifies the field
+    # to 1e12 and the same pair ends 6e-14 apart
+    check_pair(res)
     t = res["wg"][0][0]
     assert len(t) == 40000 and abs(t[-1] - 40000 * cfg.dt) < 1e-9
 
@@ -368,9 +371,9 @@ def test_resident_kernel_applicability(teuk):
 def test_resident_kernel_long_run_and_ring_drain(orc, teuk):
     """More iterations than the device ring holds, in the resident kernel: one launch per ring-full of samples."""
     cfg = wl.CONFIGS[1].scaled(name="ring2", n_r=24, n_theta=8, rs_min=10.0, rs_max=19.2, steps=40000,
-                               dt_over_dx=0.02, observers=(12.3,))
+                               dt_over_dx=0.005, observers=(12.3,))
     res = run_pair(orc, teuk, cfg, 40000, chunks=[5, 32763, 1, 7231], options={"kernel": 2})
-    check_pair(res, tol=1e-9)
+    check_pair(res)             # at the bar (see test_ring_buffer_wraps_and_drains)
     assert len(res["wg"][0][0]) == 40000 and res["launches"] < 100
 
 
@@ -400,23 +403,30 @@ def test_streamed_coefficient_planes_theta_sizes(orc, teuk, n_theta):
 
 
 def test_autotune_does_not_change_results(orc, teuk):
-    """The one-time slab-length measurement runs trial launches into scratch memory only."""
+    """The slab-count measurement (inside teuk_create / teuk_set_option, never inside teuk_step) runs trial launches
+    into scratch memory only -- also when it is repeated in the middle of a run, with a source and an observer."""
     cfg = SMALL[3]
     out = []
-    for auto in (1, 0):
+    for auto in (1, 0, 2):
         g = teuk.Solver.from_config(cfg)
         g.set_option("kernel", 0)
-        g.set_option("autotune", auto)
+        g.set_option("autotune", 1 if auto else 0)
         g.set_initial(*wl.random_state(cfg, 17))
         g.set_source(wl.orbit_table(cfg, n_steps=60))
         g.add_observer(30.0, wl.observer_weights(cfg))
-        g.step(60)
+        if auto == 2:
+            g.step(29)
+            g.set_option("autotune", 1)       # measured again on the live state: nothing may change
+            g.step(31)
+        else:
+            g.step(60)
         assert g.stat("steps") == 60 and g.stat("slab_rows") >= 1
         out.append((g.get_state(), g.extract(30.0)))
         g.close()
-    for a, b in zip(out[0][0], out[1][0]):
-        assert np.array_equal(a, b)
-    assert np.array_equal(out[0][1][1], out[1][1][1]) and len(out[0][1][0]) == 60
+    for k in (1, 2):
+        for a, b in zip(out[0][0], out[k][0]):
+            assert np.array_equal(a, b)
+        assert np.array_equal(out[0][1][1], out[k][1][1]) and len(out[k][1][0]) == 60
 
 
 @pytest.mark.parametrize("n_theta", [129, 132, 200, 240, 256, 304, 360, 361, 513, 1000])

@@ -477,3 +477,235 @@ def test_p9_discrete_delta_deposit(orc, kind):
     hs = o2.get_half()
     assert np.allclose(hs[2][0], 0.5 * cfg.dt * Th.real, rtol=1e-14, atol=0)
     assert np.count_nonzero(hs[2][0]) == np.count_nonzero(Th.real) > 0
+
+
+# ------------------------------------------------------------------------------------------ P10
+# The waveform tap ("waveform at a fixed r*"): cell index i0, interpolation
+# fraction f, the (1 - f) / f pairing, the weights' column and the mode index.
+def _tap_case():
+    a, n_r, n_th, rs = 0.6, 41, 12, (-10.0, 30.0)
+    dx = (rs[1] - rs[0]) / (n_r - 1)
+    x_obs = rs[0] + (17 + 0.37) * dx                       # off node: f = 0.37 (up to rounding)
+    rng = np.random.default_rng(1206)
+    W = rng.uniform(0.5, 2.0, n_th) * np.where(np.arange(n_th) % 2, 1.0, -1.0)   # distinct, both signs
+    return a, n_r, n_th, rs, dx, x_obs, W
+
+
+def test_p10_tap_is_the_interpolated_weighted_sum_of_the_state(orc):
+    """Every recorded sample equals sum_j W_j [(1 - f) Phi_{i0,j} + f Phi_{i0+1,j}] evaluated here, with numpy and
+    with i0, f from exact rational arithmetic, on the state the oracle hands out at that iteration."""
+    from fractions import Fraction
+    a, n_r, n_th, rs, dx, x_obs, W = _tap_case()
+    modes = [2, -1, 0]
+    o = orc.OracleSolver(a, 1.0, modes, rs[0], rs[1], n_r, n_th, 0.05 * dx)
+    rng = np.random.default_rng(7)
+    o.set_initial(*[rng.standard_normal((3, n_r, n_th)) for _ in range(4)])
+    o.add_observer(x_obs, W)
+    v = (Fraction(x_obs) - Fraction(rs[0])) / Fraction(dx)          # exact value of (x_obs - x_min)/dx
+    i0 = int(v // 1)
+    f = float(v - i0)
+    assert i0 == 17 and abs(f - 0.37) < 1e-12
+    for n in range(1, 6):
+        o.step(1)
+        pr, pim, _, _ = o.get_state()
+        phi = pr + 1j * pim
+        t, w = o.waveform(0)
+        assert len(t) == n and t[-1] == pytest.approx(n * 0.05 * dx, rel=1e-14)
+        want = ((1.0 - f) * phi[:, i0, :] + f * phi[:, i0 + 1, :]) @ W
+        assert np.all(np.abs(want) > 1e-3)
+        assert np.allclose(w[-1], want, rtol=1e-13, atol=0), (n, w[-1], want)
+        # a plausible mistake must fail: swapped pairing, neighbouring cell, unweighted sum
+        for wrong in ((f * phi[:, i0, :] + (1.0 - f) * phi[:, i0 + 1, :]) @ W,
+                      ((1.0 - f) * phi[:, i0 + 1, :] + f * phi[:, i0 + 2, :]) @ W,
+                      ((1.0 - f) * phi[:, i0, :] + f * phi[:, i0 + 1, :]).sum(axis=1)):
+            assert not np.allclose(w[-1], wrong, rtol=1e-6, atol=0)
+    o.close()
+
+
+@pytest.mark.parametrize("jstar", [0, 5, 11])
+def test_p10_tap_closed_form_on_a_field_linear_in_x(orc, jstar):
+    """Phi(x, theta_j) = (c0 + c1 x) delta_{j,j*}, Pi = 0, frozen by a time step of 1e-13 dx: linear interpolation
+    is exact on it, so the tap is W_{j*} (c0 + c1 x_obs) -- a closed form that knows nothing about i0 or f.
+    A wrong f or a swapped pairing moves x by a fraction of dx, a wrong column picks another weight."""
+    a, n_r, n_th, rs, dx, x_obs, W = _tap_case()
+    x = rs[0] + dx * np.arange(n_r)
+    c0, c1 = 0.3 - 0.2j, 0.05 + 0.11j
+    o = orc.OracleSolver(a, 1.0, [2, 3], rs[0], rs[1], n_r, n_th, 1e-13 * dx)
+    phi = np.zeros((2, n_r, n_th), dtype=complex)
+    phi[0, :, jstar] = c0 + c1 * x
+    phi[1, :, jstar] = 2.0 * (c0 + c1 * x).conjugate()           # second mode: pins the mode index
+    o.set_initial(np.ascontiguousarray(phi.real), np.ascontiguousarray(phi.imag), None, None)
+    o.add_observer(x_obs, W)
+    o.step(1)
+    _, w = o.waveform(0)
+    o.close()
+    want = np.array([W[jstar] * (c0 + c1 * x_obs), W[jstar] * 2.0 * (c0 + c1 * x_obs).conjugate()])
+    assert np.allclose(w[0], want, rtol=1e-10, atol=0), (w[0], want)
+    moved = W[jstar] * (c0 + c1 * (x_obs + 0.26 * dx))             # (1 - f) <-> f swapped
+    assert abs(w[0][0] - moved) > 1e-4 * abs(want[0])
+
+
+def test_p10_tap_default_weights_and_node_observer(orc):
+    """weights = NULL means W_j = 1 (reading B2); an observer on a node has f = 0 and reads that row."""
+    a, n_r, n_th, rs, dx, _, _ = _tap_case()
+    o = orc.OracleSolver(a, 1.0, [2], rs[0], rs[1], n_r, n_th, 0.05 * dx)
+    rng = np.random.default_rng(3)
+    o.set_initial(*[rng.standard_normal((1, n_r, n_th)) for _ in range(4)])
+    o.add_observer(rs[0] + 20 * dx, None)
+    o.step(3)
+    pr, pim, _, _ = o.get_state()
+    _, w = o.waveform(0)
+    o.close()
+    assert np.allclose(w[-1, 0], (pr[0, 20] + 1j * pim[0, 20]).sum(), rtol=1e-12, atol=0)
+
+
+# ------------------------------------------------------------------------------------------ P11
+# The trajectory / amplitude generator (workloads.orbit_table; SURVEY.md 8(c) C.6, A7; PAPER.md:155).  It feeds
+# BOTH sides of every sourced parity test, so a mistake in it is invisible there: it is pinned here against the
+# Boyer-Lindquist metric itself, closed forms, a finer quadrature and hand-worked amplitudes.
+def _bl_metric_equatorial(r, M, a):
+    """Covariant Boyer-Lindquist components at theta = pi/2 [textbook]: g_tt, g_tphi, g_phiphi, g_rr."""
+    return (-(1.0 - 2.0 * M / r), -2.0 * M * a / r, r * r + a * a + 2.0 * M * a * a / r,
+            r * r / (r * r - 2.0 * M * r + a * a))
+
+
+@pytest.mark.parametrize("a", [0.0, 0.7, 0.9, 0.99])
+@pytest.mark.parametrize("r0", [6.5, 10.0, 12.0])
+def test_p11_circular_orbit_satisfies_the_metric(a, r0):
+    """u = u^t (1, 0, 0, Omega): normalisation g(u, u) = -1 and the radial geodesic equation
+    d_r g_tt + 2 Omega d_r g_tphi + Omega^2 d_r g_phiphi = 0 (r-derivatives by central differences)."""
+    M = 1.0
+    Om = float(wl.circular_frequency(r0, M, a))
+    ut = float(wl.circular_ut(r0, M, a))
+    gtt, gtp, gpp, _ = _bl_metric_equatorial(r0, M, a)
+    assert ut * ut * (gtt + 2.0 * gtp * Om + gpp * Om * Om) == pytest.approx(-1.0, rel=1e-13)
+    h = 1e-4
+    lo, hi = _bl_metric_equatorial(r0 - h, M, a), _bl_metric_equatorial(r0 + h, M, a)
+    d = [(p - q) / (2 * h) for p, q in zip(hi, lo)]
+    assert abs(d[0] + 2.0 * Om * d[1] + Om * Om * d[2]) < 1e-9
+    assert Om > 0.0                                                     # prograde
+    if a == 0.0:
+        assert Om == pytest.approx(r0 ** -1.5, rel=1e-15)
+        assert ut == pytest.approx((1.0 - 3.0 * M / r0) ** -0.5, rel=1e-15)
+
+
+@pytest.mark.parametrize("a", [0.0, 0.7])
+def test_p11_eccentric_constants_and_rates(a):
+    """E, L of the p = 8, e = 0.3 orbit: the Schwarzschild closed forms at a = 0; u_r = 0 at both turning points
+    written with the INVERSE metric (g^tt E^2 - 2 g^tphi E L + g^phiphi L^2 = -1), not with the radial potential
+    the generator solves; along the orbit g(u, u) = -1 with u^r = (dr/dchi)(dchi/dtau); prograde; e -> 0 limit."""
+    M, p, e = 1.0, 8.0, 0.3
+    E, L = wl._eccentric_constants(p, e, M, a)
+    if a == 0.0:
+        assert E == pytest.approx(math.sqrt(((p - 2) ** 2 - 4 * e * e) / (p * (p - 3 - e * e))), rel=1e-13)
+        assert L == pytest.approx(p * M / math.sqrt(p - 3 - e * e), rel=1e-13)
+    for r in (p * M / (1 + e), p * M / (1 - e)):
+        gtt, gtp, gpp, _ = _bl_metric_equatorial(r, M, a)
+        det = gtt * gpp - gtp * gtp
+        itt, itp, ipp = gpp / det, -gtp / det, gtt / det              # inverse of the (t, phi) block
+        assert itt * E * E - 2.0 * itp * E * L + ipp * L * L == pytest.approx(-1.0, abs=2e-12)
+    assert 0.0 < E < 1.0 and L > 0.0
+    for chi in (0.3, 1.7, 3.0, 4.4):
+        dchi_dt, dphi_dt, ut, r = wl._eccentric_rates(chi, p, e, M, a, E, L)
+        assert r == pytest.approx(p * M / (1 + e * math.cos(chi)), rel=1e-15)
+        gtt, gtp, gpp, grr = _bl_metric_equatorial(r, M, a)
+        ur = (p * M * e * math.sin(chi) / (1 + e * math.cos(chi)) ** 2) * dchi_dt * ut
+        uphi = dphi_dt * ut
+        norm = gtt * ut * ut + 2.0 * gtp * ut * uphi + gpp * uphi * uphi + grr * ur * ur
+        assert norm == pytest.approx(-1.0, abs=1e-11), (chi, norm)
+        # conserved quantities from the velocities: E = -u_t, L = u_phi
+        assert -(gtt * ut + gtp * uphi) == pytest.approx(E, rel=1e-12)
+        assert gtp * ut + gpp * uphi == pytest.approx(L, rel=1e-12)
+    # e -> 0: the circular orbit of radius p M
+    E0, L0 = wl._eccentric_constants(10.0, 1e-7, M, a)
+    _, dphi_dt, ut, _ = wl._eccentric_rates(0.4, 10.0, 1e-7, M, a, E0, L0)
+    assert dphi_dt == pytest.approx(float(wl.circular_frequency(10.0, M, a)), rel=1e-6)
+    assert ut == pytest.approx(float(wl.circular_ut(10.0, M, a)), rel=1e-6)
+
+
+def test_p11_eccentric_table_integrates_its_own_rates():
+    """The RK4 table of config 4's orbit: phi and r at sample k against an independent high-order quadrature of
+    dphi/dchi = (dphi/dt)/(dchi/dt) and dt/dchi (scipy.integrate.quad) up to the same anomaly."""
+    from scipy import integrate
+    cfg = wl.CONFIGS[4].scaled(n_r=4001, steps=400)                 # dt = 0.05 dx, dx = 0.25: 801 samples, t <= 5
+    tab = wl.orbit_table(cfg)
+    M, a, p, e = cfg.M, cfg.a, 8.0, 0.3
+    E, L = wl._eccentric_constants(p, e, M, a)
+    r_tab = _r_from_tortoise(tab["rs_p"], M, a)
+    # anomaly at the last sample from its radius (chi in (0, pi) on the outgoing branch)
+    chi_end = math.acos((p * M / r_tab[-1] - 1.0) / e)
+    T, _ = integrate.quad(lambda c: 1.0 / wl._eccentric_rates(c, p, e, M, a, E, L)[0], 0.0, chi_end, epsabs=1e-13)
+    PH, _ = integrate.quad(lambda c: wl._eccentric_rates(c, p, e, M, a, E, L)[1] /
+                           wl._eccentric_rates(c, p, e, M, a, E, L)[0], 0.0, chi_end, epsabs=1e-13)
+    assert T == pytest.approx(cfg.steps * cfg.dt, rel=1e-9)
+    phit = PH + float(wl.azimuth_shift(r_tab[-1], M, a))
+    for k, m in enumerate(cfg.modes):
+        amp = tab["amp_re"][k, -1] + 1j * tab["amp_im"][k, -1]
+        assert np.angle(amp * np.exp(1j * m * phit)) == pytest.approx(0.0, abs=1e-8)
+
+
+def _r_from_tortoise(x, M, a):
+    """Invert wl.tortoise_forward by bisection (test helper; the forward map is pinned by P1)."""
+    rp = M + math.sqrt(M * M - a * a)
+    out = []
+    for xv in np.atleast_1d(x):
+        lo, hi = rp * (1 + 1e-15), 1e4
+        for _ in range(200):
+            mid = 0.5 * (lo + hi)
+            if float(wl.tortoise_forward(mid, M, a)) < xv:
+                lo = mid
+            else:
+                hi = mid
+        out.append(0.5 * (lo + hi))
+    return np.array(out)
+
+
+def test_p11_inspiral_phase_against_a_finer_quadrature():
+    """Config 5's phase phi(t) = int Omega(r0(t')) dt' (Simpson per sample interval) against adaptive quadrature
+    of the same integrand, at three sample times and for a table that starts late (t0 > 0)."""
+    from scipy import integrate
+    cfg = wl.CONFIGS[5]
+    n = 3000
+    tab = wl.orbit_table(cfg, n_steps=n)
+    T = cfg.steps * cfg.dt
+    om = lambda t: float(wl.circular_frequency(12.0 - 6.0 * t / T, cfg.M, cfg.a))
+    r_tab = _r_from_tortoise(tab["rs_p"][[0, n, 2 * n]], cfg.M, cfg.a)
+    for q, k in enumerate((0, n, 2 * n)):
+        t = 0.5 * cfg.dt * k
+        assert r_tab[q] == pytest.approx(12.0 - 6.0 * t / T, rel=1e-10)   # r0(t) linear from 12 towards 6
+        phi, _ = integrate.quad(om, 0.0, t, epsabs=1e-14, epsrel=1e-14)
+        phit = phi + float(wl.azimuth_shift(r_tab[q], cfg.M, cfg.a))
+        amp = tab["amp_re"][0, k] + 1j * tab["amp_im"][0, k]
+        assert np.angle(amp * np.exp(2j * phit)) == pytest.approx(0.0, abs=1e-10)
+    t0 = 0.37 * T
+    late = wl.orbit_table(cfg, n_steps=10, t0=t0)
+    phi, _ = integrate.quad(om, 0.0, t0, epsabs=1e-13, epsrel=1e-13, limit=200)
+    r0 = 12.0 - 6.0 * t0 / T
+    amp = late["amp_re"][0, 0] + 1j * late["amp_im"][0, 0]
+    assert np.angle(amp * np.exp(2j * (phi + float(wl.azimuth_shift(r0, cfg.M, cfg.a))))) == pytest.approx(0.0, abs=1e-8)
+
+
+def _golden_amplitudes():
+    rows = []
+    for line in open(os.path.join(GOLDEN, "source_amplitude.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        left, right = line.split("|")
+        rows.append(([float(v) for v in left.split()], [float(v) for v in right.split()]))
+    return rows
+
+
+def test_p11_amplitude_golden_values():
+    """A'_m = (2 mu/u^t) R2 / (Sigma^2 r^3 sin theta) exp(-i m phi~) at the hand-worked points
+    of tests/golden/source_amplitude.txt (derivation in the file), against the generated table of config 3's orbit."""
+    for (a, r0, m, t), (mag, phase) in _golden_amplitudes():
+        cfg = wl.CONFIGS[3].scaled(a=a, modes=(int(m),), n_r=1001, rs_min=-100.0, rs_max=900.0, dt_over_dx=t / 100.0,
+                                   steps=100)                            # sample 200 is at t
+        assert r0 == 10.0
+        tab = wl.orbit_table(cfg)
+        amp = tab["amp_re"][0, 200] + 1j * tab["amp_im"][0, 200]
+        assert abs(amp) == pytest.approx(mag, rel=1e-13)
+        assert np.angle(amp * np.exp(-1j * phase)) == pytest.approx(0.0, abs=1e-11)
+        assert tab["theta_p"][200] == pytest.approx(math.pi / 2, rel=1e-16)
+        assert tab["sigma_r"] == pytest.approx(4 * cfg.dx) and tab["sigma_theta"] == pytest.approx(4 * cfg.dtheta)
+        assert tab["half_window"] == 24 and tab["n_samples"] == 201

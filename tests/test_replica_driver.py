@@ -12,6 +12,7 @@ import torch.multiprocessing as mp
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 sys.path.insert(0, ROOT)
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
 
 from paper_1206_0270_b200 import replicas, workloads as wl  # noqa: E402
 
@@ -26,9 +27,7 @@ RICH_CFG = wl.small_test_configs()[0].scaled(name="richardson_small", n_r=321, r
 RICH_SMALL = RICH_CFG.scaled(name="richardson_tiny", n_r=81, n_theta=8, steps=160)
 
 
-def _oracle_factory(cfg):
-    from oracle import oracle as orc
-    return orc.OracleSolver.from_config(cfg)
+from oracle_adapter import oracle_factory as _oracle_factory  # noqa: E402  (tests/: the oracle behind the Solver method names)
 
 
 def test_plan_segments():
