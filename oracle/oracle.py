@@ -103,6 +103,11 @@ def _declare(L):
         L.orc_set_source_kind.restype = None
         L.orc_delta.argtypes = [C.c_int32, C.c_double, C.c_double]
         L.orc_delta.restype = C.c_double
+        _ip = C.POINTER(C.c_int32)
+        L.orc_set_source_terms.argtypes = [C.c_void_p, C.c_int32, _ip, _ip, _dp, _dp]
+        L.orc_set_source_terms.restype = C.c_int32
+        L.orc_profile_deriv.argtypes = [C.c_int32, C.c_int32, C.c_double, C.c_double]
+        L.orc_profile_deriv.restype = C.c_double
     return L
 
 
@@ -128,6 +133,11 @@ def gauss(y, sigma):
 def delta(kind, y, h):
     """Discrete delta of kind 1 (two-point) or 2 (four-point) at offset y = x_i - x_p, grid spacing h."""
     return lib().orc_delta(int(kind), float(y), float(h))
+
+
+def profile_deriv(kind, order, y, width):
+    """order-th y-derivative of deposit profile `kind` (0 Gaussian of width sigma, 1 / 2 discrete deltas on spacing h)."""
+    return lib().orc_profile_deriv(int(kind), int(order), float(y), float(width))
 
 
 class OracleSolver:
@@ -186,6 +196,18 @@ class OracleSolver:
         if kind not in (0, 1, 2):
             raise ValueError("source kind must be 0, 1 or 2")
         self._L.orc_set_source_kind(self._h, int(kind))
+
+    def set_source_terms(self, terms):
+        """f2: `terms` = list of (order_r, order_theta, amp[n_modes][n_samples] complex) replacing the monopole of
+        the installed trajectory; an empty list restores it."""
+        nt = len(terms)
+        orr = (C.c_int32 * max(nt, 1))(*[int(t[0]) for t in terms])
+        oth = (C.c_int32 * max(nt, 1))(*[int(t[1]) for t in terms])
+        amp = np.ascontiguousarray(np.stack([np.asarray(t[2], dtype=np.complex128) for t in terms])) if nt else \
+            np.zeros((0,), dtype=np.complex128)
+        ar, ai = np.ascontiguousarray(amp.real), np.ascontiguousarray(amp.imag)
+        if self._L.orc_set_source_terms(self._h, nt, orr, oth, _p(ar), _p(ai)) != 0:
+            raise ValueError("bad source terms (orders 0..2, a trajectory must be installed first)")
 
     def add_observer(self, rs_obs, weights=None):
         w = self._arr(weights, (self.shape[2],))

@@ -156,6 +156,65 @@ double delta_cubic(double y, double h) {
   return 0.0;
 }
 
+// ---------------------------------------------------------------------------------------------
+// f2 (SURVEY.md 8(f); PAPER.md:80 "T is ... constructed from the energy-momentum tensor", :145-151): the physical
+// s = -2 source is a sum of terms proportional to the delta function AND ITS FIRST AND SECOND DERIVATIVES in r
+// and theta with long coefficients that are not printed in the paper (its refs [7], [3]) and are NOT in this
+// file.  What is here is the deposit mechanism for such a sum: rank-1 terms
+//     A_t(t) * P^(a_t)(x - x_p; w_r) * P^(b_t)(theta - theta_p; w_theta),   a_t, b_t in {0, 1, 2},
+// where P^(k)(y) is the k-th derivative with respect to y of the deposit profile P (the Gaussian g, or a
+// discrete delta), so that sum_i P^(k)(x_i - x_p) f(x_i) h  ->  (-1)^k f^(k)(x_p): the action of delta^(k).
+// (reading A14.)
+// ---------------------------------------------------------------------------------------------
+
+// k-th y-derivative of g(y; sigma) = exp(-y^2/(2 sigma^2))/(sigma sqrt(2 pi)):
+//   g' = -(y/sigma^2) g,   g'' = (y^2/sigma^4 - 1/sigma^2) g.
+double gauss_deriv(int order, double y, double sigma) {
+  const double g = gauss(y, sigma);
+  if (order == 0) return g;
+  const double s2 = sigma * sigma;
+  if (order == 1) return -(y / s2) * g;
+  return (y * y / (s2 * s2) - 1.0 / s2) * g;
+}
+
+// Derivatives of the discrete deltas.  The weights of delta_linear / delta_cubic are L_i(x_p)/h, L_i the
+// Lagrange basis polynomials of the stencil around x_p = x_k + gamma h, 0 <= gamma < 1 (two points k, k+1; four
+// points k-1 .. k+2).  delta' and delta'' act as -f'(x_p) and +f''(x_p), so their weights are -L_i'(x_p)/h and
+// L_i''(x_p)/h: the y-derivatives of the same piecewise polynomials, piece chosen by the stencil position of the
+// point: y = x_i - x_p lies in (-2h,-h], (-h,0], (0,h], (h,2h] for i = k-1, k, k+1, k+2.  (The pieces join
+// continuously but with kinks, so the half-open ends matter for the derivatives and only for them.)
+// Two points carry no second derivative (L_i'' = 0): order 2 needs the four-point rule.
+double delta_linear_deriv(int order, double y, double h) {
+  if (order == 0) return delta_linear(y, h);
+  if (order == 1) {
+    if (y > -h && y <= 0.0) return 1.0 / (h * h);
+    if (y > 0.0 && y <= h) return -1.0 / (h * h);
+  }
+  return 0.0;
+}
+
+double delta_cubic_deriv(int order, double y, double h) {
+  if (order == 0) return delta_cubic(y, h);
+  const double s = std::fabs(y) / h;
+  const double sg = (y > 0.0) ? 1.0 : -1.0;           // d|y|/dy on the piece the point belongs to
+  const bool inner = (y <= 0.0) ? (s < 1.0) : (s <= 1.0);
+  const bool outer = !inner && ((y <= 0.0) ? (s < 2.0) : (s <= 2.0));
+  if (order == 1) {
+    if (inner) return sg * (-1.0 - 4.0 * s + 3.0 * s * s) / 2.0 / (h * h);     // d/ds (2 - s - 2s^2 + s^3)/2
+    if (outer) return sg * (-11.0 + 12.0 * s - 3.0 * s * s) / 6.0 / (h * h);   // d/ds (6 - 11s + 6s^2 - s^3)/6
+    return 0.0;
+  }
+  if (inner) return (3.0 * s - 2.0) / (h * h * h);
+  if (outer) return (2.0 - s) / (h * h * h);
+  return 0.0;
+}
+
+double profile_deriv(int kind, int order, double y, double width) {
+  if (kind == 1) return delta_linear_deriv(order, y, width);
+  if (kind == 2) return delta_cubic_deriv(order, y, width);
+  return gauss_deriv(order, y, width);
+}
+
 }  // namespace
 
 namespace {
@@ -190,6 +249,10 @@ struct Oracle {
   double sigma_r, sigma_th;
   int W;
   int source_kind;                           // 0 Gaussian (C.6), 1 two-point, 2 four-point discrete delta (f3)
+  // f2: when n_terms > 0 the deposited source is the sum of these rank-1 terms INSTEAD of the monopole `amp`
+  int n_terms;
+  std::vector<int> term_or, term_oth;        // [n_terms] derivative order of the profile in r* and in theta
+  std::vector<cplx> term_amp;                // [term][mode][n_samples]
   std::vector<Observer> obs;
 
   Oracle(double a, double M) : kerr(M, a) {}
@@ -217,6 +280,16 @@ inline cplx source_term(const Oracle& o, int k, int64_t ks, bool half, int i, in
   const int W = (o.source_kind == 0) ? o.W : o.source_kind;
   if (std::abs(i - ip) > W || std::abs(j - jp) > W) return cplx(0.0, 0.0);
   const double xx = half ? o.xh[i] : o.x[i];
+  if (o.n_terms > 0) {                       // f2: sum of rank-1 terms with derivative profiles
+    const double wr = (o.source_kind == 0) ? o.sigma_r : o.dx, wth = (o.source_kind == 0) ? o.sigma_th : o.dth;
+    cplx T(0.0, 0.0);
+    for (int t = 0; t < o.n_terms; ++t) {
+      const cplx At = o.term_amp[((size_t)t * o.n_modes + k) * o.n_samples + ks];
+      T += At * profile_deriv(o.source_kind, o.term_or[t], xx - xp, wr) *
+           profile_deriv(o.source_kind, o.term_oth[t], o.theta[j] - thp, wth);
+    }
+    return T;
+  }
   const cplx A = o.amp[(size_t)k * o.n_samples + ks];
   if (o.source_kind == 1) return A * delta_linear(xx - xp, o.dx) * delta_linear(o.theta[j] - thp, o.dth);
   if (o.source_kind == 2) return A * delta_cubic(xx - xp, o.dx) * delta_cubic(o.theta[j] - thp, o.dth);
@@ -343,6 +416,7 @@ void* orc_create(double a, double M, const int32_t* m, int32_t n_modes, double r
   o->dt = dt;
   o->step = 0;
   o->has_source = false; o->n_samples = 0; o->W = 0; o->sigma_r = o->sigma_th = 1.0; o->source_kind = 0;
+  o->n_terms = 0;
   o->x.resize(n_r); o->xh.resize(n_r - 1); o->theta.resize(n_theta);
   for (int i = 0; i < n_r; ++i) o->x[i] = rs_min + i * o->dx;
   for (int i = 0; i < n_r - 1; ++i) o->xh[i] = o->x[i] + 0.5 * o->dx;
@@ -397,6 +471,7 @@ void orc_set_source(void* h, int64_t n_samples, const double* rs_p, const double
   Oracle* o = (Oracle*)h;
   o->has_source = n_samples > 0;
   o->n_samples = n_samples;
+  o->n_terms = 0;                            // a new trajectory starts with the monopole term only
   if (!o->has_source) return;
   o->xp.assign(rs_p, rs_p + n_samples);
   o->thp.assign(theta_p, theta_p + n_samples);
@@ -407,6 +482,25 @@ void orc_set_source(void* h, int64_t n_samples, const double* rs_p, const double
 
 // 0 = Gaussian of C.6 (default), 1 = two-point, 2 = four-point discrete delta (f3).
 void orc_set_source_kind(void* h, int32_t kind) { ((Oracle*)h)->source_kind = kind; }
+
+// f2: replace the monopole by n_terms rank-1 terms (orders 0..2 per axis; amplitudes [term][mode][n_samples] on the
+// trajectory installed by orc_set_source).  n_terms = 0 goes back to the monopole.  Returns 0, or -1 on a bad order.
+int32_t orc_set_source_terms(void* h, int32_t n_terms, const int32_t* order_r, const int32_t* order_theta,
+                             const double* amp_re, const double* amp_im) {
+  Oracle* o = (Oracle*)h;
+  if (n_terms < 0 || (n_terms > 0 && !o->has_source)) return -1;
+  for (int t = 0; t < n_terms; ++t)
+    if (order_r[t] < 0 || order_r[t] > 2 || order_theta[t] < 0 || order_theta[t] > 2) return -1;
+  o->n_terms = n_terms;
+  o->term_or.assign(order_r, order_r + n_terms);
+  o->term_oth.assign(order_theta, order_theta + n_terms);
+  const size_t n = (size_t)n_terms * o->n_modes * o->n_samples;
+  o->term_amp.resize(n);
+  for (size_t q = 0; q < n; ++q) o->term_amp[q] = cplx(amp_re[q], amp_im[q]);
+  return 0;
+}
+
+double orc_profile_deriv(int32_t kind, int32_t order, double y, double width) { return profile_deriv(kind, order, y, width); }
 
 // Returns the observer index, or -1 if x_obs is outside [x_0, x_{n_r-1}).  weights NULL = all ones.
 int32_t orc_add_observer(void* h, double rs_obs, const double* weights) {

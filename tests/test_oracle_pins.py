@@ -709,3 +709,138 @@ def test_p11_amplitude_golden_values():
         assert tab["theta_p"][200] == pytest.approx(math.pi / 2, rel=1e-16)
         assert tab["sigma_r"] == pytest.approx(4 * cfg.dx) and tab["sigma_theta"] == pytest.approx(4 * cfg.dtheta)
         assert tab["half_window"] == 24 and tab["n_samples"] == 201
+
+
+# ------------------------------------------------------------------------------------------ P12
+# f2: deposit of a SUM of rank-1 terms whose profiles are the delta
+# function's first and second derivatives.  The physical coefficients are not in the paper; what is pinned is the
+# mechanism: each derivative profile acts on grid functions as (-1)^k d^k/dx^k at the particle.
+def _lagrange_weights(nodes, xp, order):
+    """d^order/dx^order at xp of the Lagrange basis polynomials on `nodes`, in exact rational arithmetic."""
+    from fractions import Fraction
+    out = []
+    for i, xi in enumerate(nodes):
+        poly = [Fraction(1)]                                    # coefficients of L_i, lowest power first
+        for q, xq in enumerate(nodes):
+            if q == i:
+                continue
+            den = xi - xq
+            poly = [(poly[k - 1] if k > 0 else 0) - (xq * poly[k] if k < len(poly) else 0) for k in range(len(poly) + 1)]
+            poly = [c / den for c in poly]
+        for _ in range(order):
+            poly = [k * poly[k] for k in range(1, len(poly))] or [Fraction(0)]
+        out.append(sum(c * xp ** k for k, c in enumerate(poly)))
+    return out
+
+
+@pytest.mark.parametrize("kind,order", [(1, 1), (2, 1), (2, 2)])
+def test_p12_discrete_delta_derivatives_are_lagrange_derivatives(orc, kind, order):
+    """delta^(k) weights on the stencil around x_p = x_k + gamma h are (-1)^k L_i^(k)(x_p)/h (exact rationals on
+    dyadic h, gamma: the oracle's floats must agree to the last bits), incl. gamma = 0 (particle on a node) and
+    the points just outside the stencil (weight 0)."""
+    from fractions import Fraction
+    h = Fraction(1, 4)
+    npts = 2 if kind == 1 else 4
+    for gam in (Fraction(0), Fraction(1, 8), Fraction(1, 2), Fraction(13, 16), Fraction(1023, 1024)):
+        k = 7
+        xp = (k + gam) * h
+        first = k if kind == 1 else k - 1
+        nodes = [(first + q) * h for q in range(npts)]
+        want = [(-1) ** order * w / h for w in _lagrange_weights(nodes, xp, order)]
+        for q in range(-2, npts + 2):
+            y = float((first + q) * h - xp)
+            got = orc.profile_deriv(kind, order, y, float(h))
+            exp = float(want[q]) if 0 <= q < npts else 0.0
+            assert got == pytest.approx(exp, rel=4e-15, abs=1e-300), (kind, order, gam, q, got, exp)
+
+
+@pytest.mark.parametrize("kind,order,degree", [(1, 1, 1), (2, 1, 3), (2, 2, 3)])
+def test_p12_discrete_delta_derivative_moments(orc, kind, order, degree):
+    """sum_i P^(k)(x_i - x_p) (x_i - x_p)^q h = (-1)^k k! delta_{qk} for every q up to the degree of the rule."""
+    h = 0.37
+    for gam in (0.0, 0.21, 0.5, 0.93):
+        xp = 5 * h + gam * h
+        xs = h * np.arange(0, 12)
+        w = np.array([orc.profile_deriv(kind, order, x - xp, h) for x in xs])
+        assert np.count_nonzero(w) <= (2 if kind == 1 else 4)
+        for q in range(degree + 1):
+            mom = float((w * (xs - xp) ** q).sum() * h)
+            exp = (-1) ** order * math.factorial(order) if q == order else 0.0
+            assert mom == pytest.approx(exp, abs=2e-12 / h ** max(order - q, 0)), (kind, order, gam, q, mom)
+
+
+def test_p12_gaussian_derivatives(orc):
+    """g' and g'' against mpmath's numerical derivative of the printed Gaussian (C.6), and their
+    discrete moments on a 6-sigma window: sum g' (x - x_p) h = -1, sum g'' (x - x_p)^2 h = 2, lower moments 0."""
+    import mpmath as mp
+    mp.mp.dps = 40
+    sig = 0.8
+    g = lambda y: mp.exp(-y * y / (2 * mp.mpf(sig) ** 2)) / (mp.mpf(sig) * mp.sqrt(2 * mp.pi))
+    for y in (-2.3, -0.4, 0.0, 0.05, 0.8, 3.1):
+        for order in (0, 1, 2):
+            want = float(mp.diff(g, mp.mpf(y), order))
+            assert orc.profile_deriv(0, order, y, sig) == pytest.approx(want, rel=1e-13, abs=1e-15), (y, order)   # abs: g'' vanishes at y = sigma
+    h = sig / 4.0                                                   # the configs' width: sigma = 4 cells
+    xp = 10.3 * h
+    xs = h * np.arange(-20, 45)
+    for order in (1, 2):
+        w = np.array([orc.profile_deriv(0, order, x - xp, sig) for x in xs])
+        for q in range(3):
+            mom = float((w * (xs - xp) ** q).sum() * h)
+            exp = (-1) ** order * math.factorial(order) if q == order else 0.0
+            assert mom == pytest.approx(exp, abs=1e-7), (order, q, mom)
+
+
+@pytest.mark.parametrize("kind", [0, 2])
+def test_p12_multi_term_deposit(orc, kind):
+    """The 2D deposit of a sum of terms: superposition of single-term fields, each term's moments
+    (sum T (x - x_p)^p (theta - theta_p)^q dx dtheta = A (-1)^(a+b) a! b! iff (p, q) = (a, b), else 0 for p <= a,
+    q <= b), the stage grids and time levels of P7, and that an empty term list restores the monopole."""
+    cfg = wl.small_test_configs()[3].scaled(name="terms", n_r=401, rs_min=-10.0, rs_max=30.0, steps=4)
+    orb = wl.orbit_table(cfg)
+    ns, nm = orb["n_samples"], cfg.n_modes
+    rng = np.random.default_rng(5)
+    specs = [(0, 0), (1, 0), (0, 1), (2, 0), (1, 1), (0, 2)]
+    amps = [(rng.standard_normal((nm, ns)) + 1j * rng.standard_normal((nm, ns))) for _ in specs]
+    x = cfg.rs_min + cfg.dx * np.arange(cfg.n_r)
+    xh = x[:-1] + 0.5 * cfg.dx
+    th = (np.arange(cfg.n_theta) + 0.5) * cfg.dtheta
+    o = orc.OracleSolver.from_config(cfg)
+    o.set_source(orb)
+    o.set_source_kind(kind)
+    mono = o.source_field(0, 1, False)
+    tol = 1e-5 if kind == 0 else 1e-10      # Gaussian: the window cuts the tails at 6 sigma (y^2 g'' there is 1e-6 of its peak)
+    singles = []
+    for (a_, b_), A in zip(specs, amps):
+        o.set_source_terms([(a_, b_, A)])
+        for half, ks, xs in ((False, 1, x), (True, 2, xh)):
+            T = o.source_field(0, ks, half)
+            dxp, dthp = xs - orb["rs_p"][ks], th - orb["theta_p"][ks]
+            for p_ in range(a_ + 1):
+                for q_ in range(b_ + 1):
+                    mom = (T * (dxp[:, None] ** p_) * (dthp[None, :] ** q_)).sum() * cfg.dx * cfg.dtheta
+                    exp = A[0, ks] * (-1) ** (a_ + b_) * math.factorial(a_) * math.factorial(b_) if (p_, q_) == (a_, b_) else 0.0
+                    scale = abs(A[0, ks]) / (cfg.dx ** (a_ - p_) * cfg.dtheta ** (b_ - q_))
+                    assert abs(mom - exp) <= tol * scale, (kind, a_, b_, p_, q_, half, mom, exp)
+        singles.append(o.source_field(0, 1, False))
+    o.set_source_terms(list((a_, b_, A) for (a_, b_), A in zip(specs, amps)))
+    both = o.source_field(0, 1, False)
+    assert np.allclose(both, sum(singles), rtol=1e-13, atol=1e-13 * np.abs(both).max())
+    # time levels: from zero data, Pi^1 at the nodes = dt T(sample 1) + what the half step (sample 0) feeds in;
+    # with the amplitudes of sample 0 zeroed only the full step's deposit remains
+    A0 = [A.copy() for A in amps]
+    for A in A0:
+        A[:, 0] = 0.0
+    o.set_source_terms(list((a_, b_, A) for (a_, b_), A in zip(specs, A0)))
+    o.set_initial()
+    o.step(1)
+    _, _, pi_re, pi_im = o.get_state()
+    assert np.allclose((pi_re + 1j * pi_im)[0][1:-1], cfg.dt * both[1:-1], rtol=1e-13, atol=1e-13 * cfg.dt * np.abs(both).max())
+    o.set_source_terms([])
+    assert np.array_equal(o.source_field(0, 1, False), mono)
+    # the (0, 0) term with the trajectory's own amplitude IS the monopole
+    o.set_source_terms([(0, 0, orb["amp_re"] + 1j * orb["amp_im"])])
+    assert np.allclose(o.source_field(0, 1, False), mono, rtol=1e-15, atol=0)
+    with pytest.raises(ValueError):
+        o.set_source_terms([(3, 0, amps[0])])
+    o.close()
