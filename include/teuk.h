@@ -103,6 +103,24 @@ int teuk_set_initial(teuk_solver *s, const double *phi_re, const double *phi_im,
 /* Install (copy to the device) the trajectory table; NULL = source-free.  Host pointers. */
 int teuk_set_source(teuk_solver *s, const teuk_orbit *orbit);
 
+/* Replace the single deposited term of the installed trajectory by a SUM of n_terms (0..12) rank-1 terms
+ *     T(t,x,theta) = sum_t A_t(t) P^(a_t)(x - x_p; w_r) P^(b_t)(theta - theta_p; w_theta),
+ * where P is the deposit profile selected by "source_kind" (the Gaussian g of teuk_orbit, or a discrete delta) and
+ * P^(k), k = order 0, 1 or 2, its k-th derivative with respect to its argument: on the grid, sum_i P^(k)(x_i - x_p)
+ * f(x_i) dx = (-1)^k f^(k)(x_p), the action of the k-th derivative of the delta function.  This is the mechanism
+ * the physical s = -2 source needs -- T is "constructed from the energy-momentum tensor", complex
+ * algebra on "a handful of grid points": a sum of delta, delta' and delta'' terms whose
+ * coefficients the paper does not print and this library does not contain; they are the caller's A_t.
+ * Gaussian: g' = -(y/s^2) g, g'' = (y^2/s^4 - 1/s^2) g, same window W.  Discrete deltas: the weights are
+ * (-1)^k L_i^(k)(x_p)/h, L_i the Lagrange polynomials of the two-point / four-point stencil around the particle
+ * (the two-point rule has no second derivative: its order-2 profile is zero).
+ * order_r, order_theta: [n_terms]; amp_re, amp_im: [n_terms][n_modes][n_samples] on the samples of the installed
+ * table (host pointers, copied before the call returns).  n_terms = 0 restores the single term A'_m of teuk_orbit,
+ * and so does every teuk_set_source call.  TEUK_EINVAL without an installed trajectory, for an order outside 0..2,
+ * or with "kernel" 1, "temporal_block" 2 or "coef_mode" 1 (those variants carry the single-term deposit only). */
+int teuk_set_source_terms(teuk_solver *s, int32_t n_terms, const int32_t *order_r, const int32_t *order_theta,
+                          const double *amp_re, const double *amp_im);
+
 /* Enqueue n >= 0 iterations of the two-step Lax-Wendroff scheme ("Each iteration consists of two
  * steps": the half step Eq. (3), then the full step Eq. (4), with the boundary
  * conditions of PAPER.md:104 and the source of PAPER.md:114).  No host synchronisation, no full-grid host

@@ -91,6 +91,10 @@ struct teuk_solver {
   long long n_samples;
   double *d_xp, *d_thp, *d_amp_re, *d_amp_im;
   double sigma_r, sigma_th;
+  // rank-1 deposit terms installed by teuk_set_source_terms (0 = the single term of the trajectory table)
+  int n_terms;
+  signed char term_or[TEUK_MAX_TERMS], term_oth[TEUK_MAX_TERMS];
+  double *d_term_re, *d_term_im;   // [n_terms][n_modes][n_samples]
   // time
   long long step;        // iterations done since set_initial
   long long recorded;    // samples recorded on the device (== step when observers exist)
@@ -265,6 +269,12 @@ void fill_params(const teuk_solver* s, StepParams* p, int in_buf, int k, int tap
   p->thp = s->d_thp;
   p->amp_re = s->d_amp_re;
   p->amp_im = s->d_amp_im;
+  if (s->n_terms > 0) {
+    p->n_terms = s->n_terms;
+    for (int t = 0; t < s->n_terms; ++t) { p->term_or[t] = s->term_or[t]; p->term_oth[t] = s->term_oth[t]; }
+    p->amp_re = s->d_term_re;
+    p->amp_im = s->d_term_im;
+  }
   p->sigma_r = s->source_kind ? s->dx : s->sigma_r;       // ... and their widths are the grid spacings
   p->sigma_th = s->source_kind ? s->dth : s->sigma_th;
   p->d_base = s->d_base;
@@ -374,6 +384,8 @@ void teuk_destroy(teuk_solver* s) {
   cudaFree(s->d_thp);
   cudaFree(s->d_amp_re);
   cudaFree(s->d_amp_im);
+  cudaFree(s->d_term_re);
+  cudaFree(s->d_term_im);
   if (s->ev_compute) cudaEventDestroy(s->ev_compute);
   if (s->ev_copy) cudaEventDestroy(s->ev_copy);
   if (s->own_stream) cudaStreamDestroy(s->own_stream);
@@ -539,7 +551,9 @@ int teuk_set_source(teuk_solver* s, const teuk_orbit* orbit) {
   CK(cudaStreamSynchronize(s->stream), "set_source: sync");  // old tables may still be in use
   drop_graph(s);
   cudaFree(s->d_xp); cudaFree(s->d_thp); cudaFree(s->d_amp_re); cudaFree(s->d_amp_im);
-  s->d_xp = s->d_thp = s->d_amp_re = s->d_amp_im = nullptr;
+  cudaFree(s->d_term_re); cudaFree(s->d_term_im);
+  s->d_xp = s->d_thp = s->d_amp_re = s->d_amp_im = s->d_term_re = s->d_term_im = nullptr;
+  s->n_terms = 0;                                           // a new trajectory starts with its single term
   s->has_source = 0;
   s->n_samples = 0;
   if (!orbit) return TEUK_OK;
@@ -558,6 +572,41 @@ int teuk_set_source(teuk_solver* s, const teuk_orbit* orbit) {
   s->sigma_r = orbit->sigma_r;
   s->sigma_th = orbit->sigma_theta;
   s->W = orbit->half_window;
+  return TEUK_OK;
+}
+
+int teuk_set_source_terms(teuk_solver* s, int32_t n_terms, const int32_t* order_r, const int32_t* order_theta,
+                          const double* amp_re, const double* amp_im) {
+  if (!s) return TEUK_EINVAL;
+  DeviceGuard guard(s);
+  if (s->sticky) return TEUK_ECUDA;
+  if (n_terms < 0 || n_terms > TEUK_MAX_TERMS) return fail(s, TEUK_EINVAL, "teuk_set_source_terms: n_terms must be 0..12");
+  if (n_terms > 0 && !s->has_source)
+    return fail(s, TEUK_EINVAL, "teuk_set_source_terms: install the trajectory with teuk_set_source first");
+  if (n_terms > 0 && (!order_r || !order_theta || !amp_re || !amp_im))
+    return fail(s, TEUK_EINVAL, "teuk_set_source_terms: NULL array");
+  if (n_terms > 0 && (s->variant == 1 || s->temporal_block == 2 || s->coef_mode != 0))
+    return fail(s, TEUK_EINVAL, "teuk_set_source_terms: needs kernel -1, 0 or 2, temporal_block 1 and coef_mode 0");
+  for (int t = 0; t < n_terms; ++t)
+    if (order_r[t] < 0 || order_r[t] > 2 || order_theta[t] < 0 || order_theta[t] > 2)
+      return fail(s, TEUK_EINVAL, "teuk_set_source_terms: derivative orders must be 0, 1 or 2");
+  CK(cudaStreamSynchronize(s->stream), "set_source_terms: sync");   // the old tables may still be in use
+  drop_graph(s);
+  cudaFree(s->d_term_re); cudaFree(s->d_term_im);
+  s->d_term_re = s->d_term_im = nullptr;
+  s->n_terms = 0;
+  if (n_terms == 0) return TEUK_OK;
+  const size_t n = (size_t)n_terms * s->n_modes * (size_t)s->n_samples;
+  CK(cudaMalloc((void**)&s->d_term_re, n * sizeof(double)), "set_source_terms: alloc");
+  CK(cudaMalloc((void**)&s->d_term_im, n * sizeof(double)), "set_source_terms: alloc");
+  CK(cudaMemcpyAsync(s->d_term_re, amp_re, n * sizeof(double), cudaMemcpyHostToDevice, s->stream), "set_source_terms: H2D");
+  CK(cudaMemcpyAsync(s->d_term_im, amp_im, n * sizeof(double), cudaMemcpyHostToDevice, s->stream), "set_source_terms: H2D");
+  CK(cudaStreamSynchronize(s->stream), "set_source_terms: sync");   // the caller may free its arrays on return
+  for (int t = 0; t < n_terms; ++t) {
+    s->term_or[t] = (signed char)order_r[t];
+    s->term_oth[t] = (signed char)order_theta[t];
+  }
+  s->n_terms = n_terms;
   return TEUK_OK;
 }
 
@@ -723,7 +772,8 @@ int run_chunk(teuk_solver* s, long long c) {
       fill_params(s, &p, s->cur, (int)(s->step - s->base_on_device), 0);   // level s->step was tapped by the last flush
       p.n_iter = (int)m;
       p.res_rows = s->res_rows;
-      p.res_cache = s->res_cache_opt && teuk_resident_smem_bytes(s->n_theta, s->res_rows, 1) <= (size_t)s->smem_optin;
+      p.res_cache = s->res_cache_opt && s->n_terms == 0 &&
+                    teuk_resident_smem_bytes(s->n_theta, s->res_rows, 1) <= (size_t)s->smem_optin;
       p.tag0 = s->ll_tag;
       p.ll = s->d_ll;
       const cudaError_t el = teuk_launch_step_resident(p, s->res_ncta, s->stream);
@@ -942,6 +992,7 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
   } else if (!strcmp(key, "coef_mode")) {
     if (value != 0 && value != 1) return fail(s, TEUK_EINVAL, "coef_mode must be 0 or 1");
     if (value == 1 && s->variant != 0) return fail(s, TEUK_EINVAL, "coef_mode 1 needs kernel 0");
+    if (value == 1 && s->n_terms > 0) return fail(s, TEUK_EINVAL, "coef_mode 1 is not available with teuk_set_source_terms");
     if (value == 1 && n_segments(s) > 1) return fail(s, TEUK_EINVAL, "coef_mode 1 needs n_theta <= 128");
     if (value == 1 && s->temporal_block == 2) return fail(s, TEUK_EINVAL, "coef_mode 1 needs temporal_block 1");
     if (value == 1 && !s->d_coef2d) {
@@ -965,6 +1016,7 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
     s->autotune = value ? 1 : 0;
   } else if (!strcmp(key, "temporal_block")) {
     if (value != 1 && value != 2) return fail(s, TEUK_EINVAL, "temporal_block must be 1 or 2");
+    if (value == 2 && s->n_terms > 0) return fail(s, TEUK_EINVAL, "temporal_block 2 is not available with teuk_set_source_terms");
     s->temporal_block = (int)value;
     if (value == 2 && (!tb2_possible(s) || s->kernel_opt == 2)) {
       s->temporal_block = 1;
@@ -974,6 +1026,7 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
     if (value < -1 || value > 2)
       return fail(s, TEUK_EINVAL, "kernel must be -1 (automatic), 0 (register-resident), 1 (shared-memory-resident) or 2 (resident, whole state on chip)");
     if (value > 0 && s->coef_mode != 0) return fail(s, TEUK_EINVAL, "kernels 1 and 2 need coef_mode 0");
+    if (value == 1 && s->n_terms > 0) return fail(s, TEUK_EINVAL, "kernel 1 is not available with teuk_set_source_terms");
     if (value == 2) {
       if (s->temporal_block == 2) return fail(s, TEUK_EINVAL, "kernel 2 needs temporal_block 1");
       if (!resident_plan(s, &s->res_rows, &s->res_ncta))

@@ -41,6 +41,7 @@ enum {
 };
 
 #define TEUK_MAX_OBS 8
+#define TEUK_MAX_TERMS 12
 #define TEUK_MAX_MODES 64
 
 struct ObsDev {
@@ -68,8 +69,12 @@ struct StepParams {
   int has_source, W;
   int source_kind;        // 0 Gaussian (sigma_r, sigma_th), 1 / 2 two- / four-point discrete delta (widths dx, dth)
   long long n_samples;
-  const double *xp, *thp, *amp_re, *amp_im;
+  const double *xp, *thp, *amp_re, *amp_im;   // amplitudes [n_modes][n_samples] ([n_terms][n_modes][n_samples] if n_terms > 0)
   double sigma_r, sigma_th;
+  // f2, teuk_set_source_terms: n_terms > 0 = sum of rank-1 terms with derivative order 0..2 of the profile in r*
+  // and in theta (kernels instantiated with TERMS = true); 0 = the single term of the trajectory table
+  int n_terms;
+  signed char term_or[TEUK_MAX_TERMS], term_oth[TEUK_MAX_TERMS];
   // iteration index of the INPUT state: n = *d_base + k
   const long long* d_base;
   int k;

@@ -132,7 +132,8 @@ __device__ __forceinline__ uint4* ll_slot(const StepParams& p, int mode, int nct
 // fewer (blockDim.x / 32 = min(NW, rows + 1)).
 // CC: the time-independent coefficients b2d, Q, Re beta^' of every location of the block are kept in shared memory
 // (3 doubles per point and location) when there is room; else they are rebuilt in every stage as in kernel 0.
-template <int V, int NW, bool CC>
+// TERMS: multi-term deposit of teuk_set_source_terms (a separate instantiation: the default kernel is unchanged)
+template <int V, int NW, bool CC, bool TERMS = false>
 __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __grid_constant__ StepParams p) {
   constexpr int NP = 32 * V;        // padded row width in shared memory (columns >= n_theta stay zero)
   constexpr int ROWD = 4 * NP;      // doubles per row
@@ -271,7 +272,7 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
       if (has_source) {
         const double x = p.rs_min + ((double)i + 0.5) * p.dx;
         if (fabs(x - __ldg(p.xp + 2 * n)) <= src_reach) {
-          StageSource<V> s;
+          typename SourceSel<V, TERMS>::type s;
           setup_source<V>(s, p, mode, 2 * n, true, i, i, lane, 0);
           add_source<V>(Hn, s, p, i, true);
         }
@@ -319,7 +320,7 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
       if (has_source) {
         const double x = p.rs_min + (double)i * p.dx;
         if (fabs(x - __ldg(p.xp + 2 * n + 1)) <= src_reach) {
-          StageSource<V> s;
+          typename SourceSel<V, TERMS>::type s;
           setup_source<V>(s, p, mode, 2 * n + 1, false, i, i, lane, 0);
           add_source<V>(out, s, p, i, false);
         }
@@ -380,7 +381,7 @@ size_t teuk_resident_ll_bytes(int n_theta, int n_modes, int ncta) {
   return (size_t)n_modes * ncta * 4 * (4 * 32 * V) * 16;
 }
 
-template <int V, bool CC>
+template <int V, bool CC, bool TERMS = false>
 static cudaError_t launch_resident_v(const StepParams& p, int ncta, cudaStream_t st) {
   constexpr int NW = resident_max_warps<V>();
   const size_t dyn = teuk_resident_smem_bytes(p.n_theta, p.res_rows, CC ? 1 : 0);
@@ -391,7 +392,7 @@ static cudaError_t launch_resident_v(const StepParams& p, int ncta, cudaStream_t
     int optin = 0;
     cudaError_t e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev_);
     if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(teuk_step_resident_kernel<V, NW, CC>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+      e = cudaFuncSetAttribute(teuk_step_resident_kernel<V, NW, CC, TERMS>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
     if (e != cudaSuccess) return e;
     attr_set[dev_ & 63] = true;
   }
@@ -399,12 +400,17 @@ static cudaError_t launch_resident_v(const StepParams& p, int ncta, cudaStream_t
   dim3 grid(ncta, p.n_modes), block(32 * nwarps);
   StepParams pc = p;
   void* args[] = {&pc};
-  return cudaLaunchCooperativeKernel((const void*)teuk_step_resident_kernel<V, NW, CC>, grid, block, args, dyn, st);
+  return cudaLaunchCooperativeKernel((const void*)teuk_step_resident_kernel<V, NW, CC, TERMS>, grid, block, args, dyn, st);
 }
 
 // n_iter iterations in one cooperative launch; the caller sized res_rows / ncta so that the state fits.
 cudaError_t teuk_launch_step_resident(const StepParams& p, int ncta, cudaStream_t st) {
   const int v = (p.n_theta + 31) / 32;
+  if (p.n_terms > 0) {              // multi-term deposit (the host passes res_cache = 0 with it)
+    if (v <= 1) return launch_resident_v<1, false, true>(p, ncta, st);
+    if (v <= 2) return launch_resident_v<2, false, true>(p, ncta, st);
+    return launch_resident_v<4, false, true>(p, ncta, st);
+  }
   if (p.res_cache) {
     if (v <= 1) return launch_resident_v<1, true>(p, ncta, st);
     if (v <= 2) return launch_resident_v<2, true>(p, ncta, st);

@@ -497,6 +497,120 @@ __device__ __forceinline__ void add_source(Row<V>& out, const StageSource<V>& s,
   }
 }
 
+// ---- f2: sums of rank-1 deposit terms with derivative profiles (teuk_set_source_terms) ----------------------
+// The physical s = -2 source (PAPER.md:80 "constructed from the energy-momentum tensor", :145-151) is a sum of
+// terms in the delta function and its first and second derivatives in r and theta; its coefficients are the
+// caller's (they are not printed in the paper and not in this library), the deposit is ours:
+//     dt * sum_t A_t P^(a_t)(x - x_p; w_r) P^(b_t)(theta - theta_p; w_theta),   a_t, b_t in {0, 1, 2},
+// P^(k) = k-th derivative of the deposit profile with respect to its argument.  Gaussian: g' = -(y/s^2) g,
+// g'' = (y^2/s^4 - 1/s^2) g.  Discrete deltas: the weights are L_i(x_p)/h with L_i the Lagrange polynomials of the
+// stencil around x_p = x_k + gamma h (two points k, k+1; four points k-1 .. k+2), so delta^(n) has the weights
+// (-1)^n L_i^(n)(x_p)/h = the y-derivatives of the same piecewise polynomials, the piece chosen by where the point
+// sits in the stencil: y in (-2h,-h], (-h,0], (0,h], (h,2h] for i = k-1 .. k+2 (the pieces join with kinks, so the
+// half-open ends matter here).  Kernels instantiated with TERMS = true use TermSource below; the default kernels
+// (TERMS = false) contain none of this code.
+struct Profile3 {
+  double d[3];
+};
+__device__ __forceinline__ Profile3 deposit_profile3(int kind, double y, double width) {
+  Profile3 r;
+  r.d[0] = deposit_profile(kind, y, width);
+  r.d[1] = 0.0;
+  r.d[2] = 0.0;
+  if (kind == 0) {
+    const double s2 = width * width;
+    r.d[1] = -(y / s2) * r.d[0];
+    r.d[2] = (y * y / (s2 * s2) - 1.0 / s2) * r.d[0];
+    return r;
+  }
+  const double h = width, s = fabs(y) / h;
+  if (kind == 1) {                                  // two points carry no second derivative
+    if (y > -h && y <= 0.0) r.d[1] = 1.0 / (h * h);
+    if (y > 0.0 && y <= h) r.d[1] = -1.0 / (h * h);
+    return r;
+  }
+  const double sg = (y > 0.0) ? 1.0 : -1.0;
+  const bool inner = (y <= 0.0) ? (s < 1.0) : (s <= 1.0);
+  const bool outer = !inner && ((y <= 0.0) ? (s < 2.0) : (s <= 2.0));
+  if (inner) {
+    r.d[1] = sg * (-1.0 - 4.0 * s + 3.0 * s * s) / 2.0 / (h * h);
+    r.d[2] = (3.0 * s - 2.0) / (h * h * h);
+  } else if (outer) {
+    r.d[1] = sg * (-11.0 + 12.0 * s - 3.0 * s * s) / 6.0 / (h * h);
+    r.d[2] = (2.0 - s) / (h * h * h);
+  }
+  return r;
+}
+__device__ __forceinline__ double pick3(const Profile3& r, int order) {
+  return order == 0 ? r.d[0] : (order == 1 ? r.d[1] : r.d[2]);
+}
+
+// Window bookkeeping of one stage for the multi-term deposit: scalars only; the theta profiles are rebuilt on the
+// few rows a window touches, so nothing per column stays live across a marching loop.
+template <int V>
+struct TermSource {
+  bool on;
+  int ip, jp, mode, lane, col0;
+  long long ks;
+  double xp, thp;
+};
+
+template <int V, int MAP = 0>
+__device__ __forceinline__ void setup_source(TermSource<V>& s, const StepParams& p, int mode, long long ks,
+                                             bool half, int row_lo, int row_hi, int lane, int col0 = 0) {
+  s.on = false;
+  if (!p.has_source) return;
+  const double xp = p.xp[ks], thp = p.thp[ks];
+  const double v = __ddiv_rn(__dsub_rn(xp, p.rs_min), p.dx);       // same rounding decisions as the plain deposit
+  const int ip = half ? (int)floor(__dadd_rn(__dsub_rn(v, 0.5), 0.5)) : (int)floor(__dadd_rn(v, 0.5));
+  const int jp = (int)floor(__dadd_rn(__dsub_rn(__ddiv_rn(thp, p.dth), 0.5), 0.5));
+  if (ip + p.W < row_lo || ip - p.W > row_hi) return;
+  s.on = true;
+  s.ip = ip;
+  s.jp = jp;
+  s.mode = mode;
+  s.lane = lane;
+  s.col0 = col0;
+  s.ks = ks;
+  s.xp = xp;
+  s.thp = thp;
+}
+
+template <int V>
+__device__ __forceinline__ void add_source(Row<V>& out, const TermSource<V>& s, const StepParams& p, int i,
+                                           bool half) {
+  if (!s.on || abs(i - s.ip) > p.W) return;
+  double x = __dadd_rn(p.rs_min, __dmul_rn((double)i, p.dx));
+  if (half) x = __dadd_rn(x, __dmul_rn(0.5, p.dx));
+  const Profile3 pr = deposit_profile3(p.source_kind, x - s.xp, p.sigma_r);
+#pragma unroll
+  for (int q = 0; q < V; ++q) {
+    const int j = s.col0 + s.lane * V + q;                           // lane <-> column mapping MAP 0
+    if ((unsigned)j >= (unsigned)p.n_theta || abs(j - s.jp) > p.W) continue;
+    const double th = __dmul_rn((double)j + 0.5, p.dth);
+    const Profile3 pt = deposit_profile3(p.source_kind, th - s.thp, p.sigma_th);
+    double accr = 0.0, acci = 0.0;
+    for (int t = 0; t < p.n_terms; ++t) {
+      const size_t ia = ((size_t)t * p.n_modes + s.mode) * p.n_samples + s.ks;
+      const double gg = (p.dt * pick3(pr, p.term_or[t])) * pick3(pt, p.term_oth[t]);
+      accr = fma(p.amp_re[ia], gg, accr);
+      acci = fma(p.amp_im[ia], gg, acci);
+    }
+    out.c[2][q] += accr;
+    out.c[3][q] += acci;
+  }
+}
+
+// StageSource (one term, the profile itself: the configs' deposit) or TermSource (teuk_set_source_terms)
+template <int V, bool TERMS>
+struct SourceSel {
+  typedef StageSource<V> type;
+};
+template <int V>
+struct SourceSel<V, true> {
+  typedef TermSource<V> type;
+};
+
 // Waveform tap of the INPUT state (sample n): w = sum_j W_j [(1-f) Phi_{i0,j} + f Phi_{i0+1,j}].
 template <int V, int MAP = 0>
 __device__ __forceinline__ void tap(const Row<V>& lo, const Row<V>& hi, const StepParams& p, int i, int mode,

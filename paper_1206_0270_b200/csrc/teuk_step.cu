@@ -65,7 +65,10 @@ __device__ __forceinline__ void stage_rtab_chunk(double* sbuf, const double* __r
 // Measured and rejected for V = 4 (config 5, same box, base 88.6-92.0 GPts/s): 9 warps per SM (96-thread
 // blocks, __maxnreg__(224): 388 B of spill stores) 69.6; bracket B accumulated in two partial sums
 // (shorter dependent chains, more spills) 89.1.
-template <int V, bool VEC, int CM, bool SEG, bool FULLW>
+// TERMS: the deposit is a sum of rank-1 terms with derivative profiles (teuk_set_source_terms)
+// instead of the single term of the trajectory table; a separate instantiation, so that the default kernel's code
+// and register allocation do not change with it.
+template <int V, bool VEC, int CM, bool SEG, bool FULLW, bool TERMS = false>
 __global__ void __launch_bounds__(128, (V == 2 ? TEUK_V2_BLOCKS : TEUK_MIN_BLOCKS)) teuk_step_kernel(const __grid_constant__ StepParams p) {
   const int lane = threadIdx.x & 31;
   // warp index broadcast from lane 0: tells the compiler that everything derived from it (slab bounds, loop
@@ -138,7 +141,7 @@ __global__ void __launch_bounds__(128, (V == 2 ? TEUK_V2_BLOCKS : TEUK_MIN_BLOCK
       th.vals.d0[v] = ok ? tb[TT_D0 * nth + j0 + v] : 0.0;
     }
   }
-  StageSource<V> src_h, src_f;   // half stage: sample 2n at half points; full stage: 2n+1 at nodes
+  typename SourceSel<V, TERMS>::type src_h, src_f;   // half stage: sample 2n at half points; full stage: 2n+1 at nodes
   setup_source<V>(src_h, p, mode, 2 * n, true, r0 - 1, r1 - 1, lane, c_lo);
   setup_source<V>(src_f, p, mode, 2 * n + 1, false, r0, r1 - 1, lane, c_lo);
   bool do_tap = !SEG && p.tap_enable && p.n_obs > 0 && n >= 1;   // segments: separate tap kernel
@@ -851,13 +854,14 @@ static cudaError_t launch_v(const StepParams& p, cudaStream_t st) {
   const bool vec = p.n_theta % V == 0;
   const int dyn_max = (int)((size_t)warps_per_block * TEUK_SLOTS * 4 * 32 * V * sizeof(double));
   const size_t dyn = vec ? (size_t)dyn_max : 0;
-#define TEUK_LAUNCH(VECF, CMF, SEGF, FWF)                                                                        \
+#define TEUK_LAUNCH(VECF, CMF, SEGF, FWF) TEUK_LAUNCH_T(VECF, CMF, SEGF, FWF, false)
+#define TEUK_LAUNCH_T(VECF, CMF, SEGF, FWF, TF)                                                                  \
   do {                                                                                                       \
     static bool attr_set[64] = {false};   /* per device: function attributes belong to a context */         \
     int dev_ = 0;                                                                                            \
     cudaGetDevice(&dev_);                                                                                    \
     if (!attr_set[dev_ & 63]) {                                                                              \
-      cudaError_t e = cudaFuncSetAttribute(teuk_step_kernel<V, VECF, CMF, SEGF, FWF>,                        \
+      cudaError_t e = cudaFuncSetAttribute(teuk_step_kernel<V, VECF, CMF, SEGF, FWF, TF>,                    \
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max);            \
       if (e != cudaSuccess) return e;                                                                        \
       attr_set[dev_ & 63] = true;                                                                            \
@@ -869,13 +873,21 @@ static cudaError_t launch_v(const StepParams& p, cudaStream_t st) {
       cudaLaunchConfig_t lc_ = {};                                                                           \
       lc_.gridDim = grid; lc_.blockDim = block; lc_.dynamicSmemBytes = dyn; lc_.stream = st;                 \
       lc_.attrs = at_; lc_.numAttrs = 1;                                                                     \
-      cudaError_t e = cudaLaunchKernelEx(&lc_, teuk_step_kernel<V, VECF, CMF, SEGF, FWF>, p);                \
+      cudaError_t e = cudaLaunchKernelEx(&lc_, teuk_step_kernel<V, VECF, CMF, SEGF, FWF, TF>, p);            \
       if (e != cudaSuccess) return e;                                                                        \
     } else                                                                                                   \
-    teuk_step_kernel<V, VECF, CMF, SEGF, FWF><<<grid, block, dyn, st>>>(p);                                  \
+    teuk_step_kernel<V, VECF, CMF, SEGF, FWF, TF><<<grid, block, dyn, st>>>(p);                              \
   } while (0)
   const bool fullw = p.n_theta == 32 * V;
-  if (p.n_seg > 1) {
+  if (p.n_terms > 0) {              // multi-term deposit: coef_mode 0 only (checked by teuk_set_source_terms)
+    if (p.n_seg > 1) {
+      if (vec) TEUK_LAUNCH_T(true, 0, true, false, true); else TEUK_LAUNCH_T(false, 0, true, false, true);
+    } else {
+      if (fullw) TEUK_LAUNCH_T(true, 0, false, true, true);
+      else if (vec) TEUK_LAUNCH_T(true, 0, false, false, true);
+      else TEUK_LAUNCH_T(false, 0, false, false, true);
+    }
+  } else if (p.n_seg > 1) {
     if (vec) TEUK_LAUNCH(true, 0, true, false); else TEUK_LAUNCH(false, 0, true, false);
   } else if (p.coef_mode == 1) {
     if (fullw) TEUK_LAUNCH(true, 1, false, true);
@@ -887,6 +899,7 @@ static cudaError_t launch_v(const StepParams& p, cudaStream_t st) {
     else TEUK_LAUNCH(false, 0, false, false);
   }
 #undef TEUK_LAUNCH
+#undef TEUK_LAUNCH_T
   return cudaGetLastError();
 }
 

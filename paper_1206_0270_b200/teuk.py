@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libteuk.so")
 
 TEUK_OK, TEUK_EINVAL, TEUK_ENOMEM, TEUK_ECUDA, TEUK_ENONFINITE = 0, -1, -2, -3, -4
-SYMBOLS = ["teuk_select_device", "teuk_measure_fp64", "teuk_create", "teuk_set_initial", "teuk_set_source", "teuk_step", "teuk_extract",
+SYMBOLS = ["teuk_select_device", "teuk_measure_fp64", "teuk_create", "teuk_set_initial", "teuk_set_source", "teuk_set_source_terms", "teuk_step", "teuk_extract",
            "teuk_get_state", "teuk_set_option", "teuk_get_stat", "teuk_sync", "teuk_destroy",
            "teuk_last_error"]
 
@@ -58,6 +58,8 @@ def load():
     L.teuk_measure_fp64.argtypes = [C.c_int32, _dp]
     L.teuk_set_initial.argtypes = [vp, vp, vp, vp, vp, C.c_int32]
     L.teuk_set_source.argtypes = [vp, C.POINTER(teuk_orbit)]
+    _ip = C.POINTER(C.c_int32)
+    L.teuk_set_source_terms.argtypes = [vp, C.c_int32, _ip, _ip, _dp, _dp]
     L.teuk_step.argtypes = [vp, C.c_int64]
     L.teuk_extract.argtypes = [vp, C.c_double, _dp, _dp, _dp, _dp, C.c_int64, C.POINTER(C.c_int64)]
     L.teuk_get_state.argtypes = [vp, vp, vp, vp, vp, C.c_int32]
@@ -176,6 +178,21 @@ class Solver:
         o = teuk_orbit(ns, *[k.ctypes.data_as(_dp) for k in keep], float(orbit["sigma_r"]),
                        float(orbit["sigma_theta"]), int(orbit["half_window"]))
         self._check(self._lib.teuk_set_source(self._h, C.byref(o)))
+
+    def set_source_terms(self, terms):
+        """teuk_set_source_terms: `terms` = list of (order_r, order_theta, amp[n_modes][n_samples] complex); an empty
+        list restores the single term of the trajectory table."""
+        nt = len(terms)
+        if nt == 0:
+            self._check(self._lib.teuk_set_source_terms(self._h, 0, None, None, None, None))
+            return
+        orr = (C.c_int32 * nt)(*[int(t[0]) for t in terms])
+        oth = (C.c_int32 * nt)(*[int(t[1]) for t in terms])
+        amp = np.stack([np.asarray(t[2], dtype=np.complex128) for t in terms])
+        assert amp.ndim == 3 and amp.shape[1] == self.shape[0], amp.shape
+        ar, ai = np.ascontiguousarray(amp.real), np.ascontiguousarray(amp.imag)
+        self._check(self._lib.teuk_set_source_terms(self._h, nt, orr, oth, ar.ctypes.data_as(_dp),
+                                                    ai.ctypes.data_as(_dp)))
 
     def step(self, n=1):
         self._check(self._lib.teuk_step(self._h, int(n)))

@@ -597,3 +597,119 @@ def test_empty_calls(orc, teuk):
     t, w = g.extract(cfg.observers[0])
     assert len(t) == 33 and np.all(w == 0.0)
     g.close()
+
+
+# ---- f2: sums of rank-1 deposit terms with derivative profiles (teuk_set_source_terms) ----------------------
+TERM_SPECS = [(0, 0), (1, 0), (0, 1), (2, 0), (1, 1), (0, 2)]
+
+
+def _random_terms(cfg, n_samples, seed, specs=TERM_SPECS):
+    rng = np.random.default_rng(seed)
+    return [(a, b, rng.standard_normal((cfg.n_modes, n_samples)) + 1j * rng.standard_normal((cfg.n_modes, n_samples)))
+            for a, b in specs]
+
+
+def _run_terms(orc, teuk, cfg, steps, terms, kind, options=None, chunks=None):
+    orbit = wl.orbit_table(cfg, n_steps=steps)
+    W = wl.observer_weights(cfg)
+    o = orc.OracleSolver.from_config(cfg)
+    g = teuk.Solver.from_config(cfg)
+    for k, v in (options or {}).items():
+        g.set_option(k, v)
+    for s_ in (o, g):
+        s_.set_initial()
+        s_.set_source(orbit)
+        s_.set_source_terms(terms)
+    o.set_source_kind(kind)
+    g.set_option("source_kind", kind)
+    for x in cfg.observers:
+        o.add_observer(x, W)
+        g.add_observer(x, W)
+    o.step(steps)
+    for c in (chunks or [steps]):
+        g.step(c)
+    res = dict(so=o.get_state(), sg=g.get_state(), wo=[o.waveform(k) for k in range(len(cfg.observers))],
+               wg=[g.extract(x) for x in cfg.observers], launches=g.stat("launches"))
+    o.close()
+    g.close()
+    return res
+
+
+@pytest.mark.parametrize("kind", [0, 1, 2])
+@pytest.mark.parametrize("kernel", [0, 2])
+def test_source_terms_parity(orc, teuk, kind, kernel):
+    """Six terms (delta, its first and second derivatives in r* and theta, the mixed one) with independent random
+    amplitudes per mode and sample, from zero data: everything in the fields comes from the deposit."""
+    for cfg in (SMALL[3].scaled(steps=60), SMALL[4].scaled(steps=40), SMALL[5].scaled(steps=30)):
+        terms = _random_terms(cfg, 2 * cfg.steps + 1, 100 + kind)
+        res = _run_terms(orc, teuk, cfg, cfg.steps, terms, kind, options={"kernel": kernel}, chunks=[1, 2, cfg.steps - 3])
+        check_pair(res)
+
+
+def test_source_terms_single_terms_and_launch_shapes(orc, teuk):
+    """Each derivative profile on its own (a wrong sign or a swapped order cannot hide in a sum); kernel 0 with
+    graphs, with plain launches and short slabs, and kernel 2 agree bit for bit."""
+    cfg = SMALL[3].scaled(steps=40, n_r=333)
+    ns = 2 * cfg.steps + 1
+    for spec in TERM_SPECS[1:]:
+        terms = _random_terms(cfg, ns, 7, specs=[spec])
+        base = None
+        for opt in ({"kernel": 0}, {"kernel": 2}, {"kernel": 0, "slab_rows": 3, "graph": 0}):
+            res = _run_terms(orc, teuk, cfg, cfg.steps, terms, 0, options=opt)
+            check_pair(res)
+            if base is None:
+                base = res
+            else:
+                for a, b in zip(base["sg"], res["sg"]):
+                    assert np.array_equal(a, b), (spec, opt)
+
+
+def test_source_terms_theta_segments_and_ragged_width(orc, teuk):
+    """The paper's own grid is 304 columns wide: theta segments; and a width that is not a multiple
+    of the lane width (scalar load path)."""
+    for n_theta in (304, 45):
+        cfg = SMALL[3].scaled(name="terms%d" % n_theta, n_r=151, n_theta=n_theta, dt_over_dx=0.002, steps=12)
+        terms = _random_terms(cfg, 2 * cfg.steps + 1, n_theta)
+        check_pair(_run_terms(orc, teuk, cfg, cfg.steps, terms, 0, chunks=[1, 11]))
+        check_pair(_run_terms(orc, teuk, cfg, cfg.steps, terms, 2))
+
+
+def test_source_terms_reset_and_errors(orc, teuk):
+    cfg = SMALL[3].scaled(steps=16)
+    orbit = wl.orbit_table(cfg, n_steps=16)
+    g = teuk.Solver.from_config(cfg)
+    with pytest.raises(teuk.TeukError):
+        g.set_source_terms(_random_terms(cfg, 33, 1))             # no trajectory installed yet
+    g.set_source(orbit)
+    with pytest.raises(teuk.TeukError):
+        g.set_source_terms([(3, 0, np.zeros((cfg.n_modes, 33)))])
+    with pytest.raises(teuk.TeukError):
+        g.set_source_terms([(0, -1, np.zeros((cfg.n_modes, 33)))])
+    g.set_source_terms(_random_terms(cfg, 33, 1))
+    for key, val in (("kernel", 1), ("temporal_block", 2), ("coef_mode", 1)):    # single-term variants only
+        with pytest.raises(teuk.TeukError):
+            g.set_option(key, val)
+    g.set_source_terms([])
+    # the (0, 0) term with the table's own amplitude is the default deposit; an empty list and a new
+    # teuk_set_source both restore it
+    mono = orbit["amp_re"] + 1j * orbit["amp_im"]
+    out = []
+    for mode in ("default", "explicit", "emptied", "reinstalled"):
+        g.set_initial()
+        if mode == "explicit":
+            g.set_source_terms([(0, 0, mono)])
+        elif mode == "emptied":
+            g.set_source_terms(_random_terms(cfg, 33, 2))
+            g.set_source_terms([])
+        elif mode == "reinstalled":
+            g.set_source_terms(_random_terms(cfg, 33, 3))
+            g.set_source(orbit)
+        g.step(16)
+        out.append(g.get_state())
+    g.close()
+    for a, b in zip(out[0], out[1]):                              # another kernel instantiation: rounding level
+        assert np.allclose(a, b, rtol=1e-12, atol=1e-12 * np.abs(b).max())
+    for k in (2, 3):
+        for a, b in zip(out[0], out[k]):
+            assert np.array_equal(a, b), k
+    assert np.abs(out[0][2]).max() > 0
