@@ -128,6 +128,28 @@ int teuk_set_source_terms(teuk_solver *s, int32_t n_terms, const int32_t *order_
  * every iteration (sample time t = n_done*dt).  TEUK_EINVAL if a source is installed and its table is too short. */
 int teuk_step(teuk_solver *s, int64_t n);
 
+/* Allocation-free variant of teuk_set_initial(device) + teuk_step(n) + teuk_get_state(device) for grids whose state
+ * fits on chip (the resident kernel, "kernel" 2: n_theta <= 128, about n_modes*n_r*n_theta <= 5e5 points), for
+ * callers that cannot call cudaMalloc -- code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it.  The same iteration (Eq. 3-4) by the same kernel: fields are bit-identical to teuk_step's.
+ * The kernel's only scratch memory, the block-to-block exchange buffer that teuk_step cudaMalloc's on first use,
+ * is here a file-scope static device array of 5 MiB (5 242 880 bytes; every GPU that loads the library holds it
+ * until the process exits); a solver that needs more gets TEUK_EINVAL with a message naming both sizes.
+ *   in_dev[4]:  DEVICE arrays Phi_R, Phi_I, Pi_R, Pi_I of time level n0, layout of teuk_set_initial; NULL = zeros.
+ *   n0:         iteration index of that level (a source uses trajectory samples 2*n0, 2*n0 + 1, ...); >= 0.
+ *   n:          iterations to run, 1 <= n <= 2^30.
+ *   out_dev[4]: DEVICE arrays receiving level n0 + n (may alias in_dev); NULL = skip that component.
+ * Everything is enqueued on the solver's stream and nothing is waited for: keep the arrays alive until it has run.
+ * The call makes no cudaMalloc / cudaFree / cudaMallocHost / cudaFreeHost and calls no library that allocates.
+ * Side effects: the solver's own fields become the result and its iteration counter n0 + n, as if teuk_step had
+ * produced them (a later teuk_step / teuk_get_state continues from there).  TEUK_EINVAL with armed observers
+ * (their ring drains allocate pinned memory), with "kernel" 1, "temporal_block" 2 or "coef_mode" 1, if the state
+ * does not fit on chip, or if the trajectory table is too short.
+ * The static array is shared by every solver and every call on a GPU and keeps the last call's contents: each
+ * call clears the part it uses before its kernel starts, so consecutive calls on one stream are safe, but two
+ * calls that OVERLAP on the GPU (different streams or solvers at the same time) race on it. */
+int teuk_step_noalloc(teuk_solver *s, const double *const in_dev[4], int64_t n0, int64_t n, double *const out_dev[4]);
+
 /* Observer at r* = rs_obs (x_0 <= rs_obs < x_{n_r-1}): w(t_n) = sum_j weights[j] *
  * [(1-f) Phi^n_{i0,j} + f Phi^n_{i0+1,j}] (linear interpolation in x).
  * The FIRST call with a new rs_obs arms the observer (weights [n_theta] host array, NULL = all

@@ -23,6 +23,8 @@ cudaError_t teuk_launch_step_tb2(const StepParams& p, cudaStream_t st);
 cudaError_t teuk_launch_step_resident(const StepParams& p, int ncta, cudaStream_t st);
 size_t teuk_resident_smem_bytes(int n_theta, int res_rows, int coef_cache);
 size_t teuk_resident_ll_bytes(int n_theta, int n_modes, int ncta);
+cudaError_t teuk_launch_step_resident_static(const StepParams& p, int ncta, cudaStream_t st);
+size_t teuk_resident_static_capacity();
 cudaError_t teuk_launch_flush_tap(const StepParams& p, cudaStream_t st);
 cudaError_t teuk_launch_bump(long long* d_base, long long inc, cudaStream_t st);
 cudaError_t teuk_launch_set_base(long long* d_base, long long v, cudaStream_t st);
@@ -880,6 +882,56 @@ int teuk_step(teuk_solver* s, int64_t n) {
     if (rc != TEUK_OK) return rc;
     remaining -= c;
   }
+  return TEUK_OK;
+}
+
+// Allocation-free variant of set_initial(device) + step(n) + get_state(device) on the resident kernel, with the
+// exchange scratch in a static device array (teuk_resident.cu).  Calls no cudaMalloc / cudaFree / cudaMallocHost /
+// cudaFreeHost and waits for nothing: three kernels, one memset and at most one counter kernel are enqueued.
+int teuk_step_noalloc(teuk_solver* s, const double* const in_dev[4], int64_t n0, int64_t n, double* const out_dev[4]) {
+  if (!s) return TEUK_EINVAL;
+  DeviceGuard guard(s);
+  if (s->sticky) return TEUK_ECUDA;
+  if (!in_dev || !out_dev) return fail(s, TEUK_EINVAL, "teuk_step_noalloc: in_dev / out_dev is NULL");
+  if (n < 1 || n > (1LL << 30) || n0 < 0) return fail(s, TEUK_EINVAL, "teuk_step_noalloc: need n0 >= 0 and 1 <= n <= 2^30");
+  if (s->n_obs > 0) return fail(s, TEUK_EINVAL, "teuk_step_noalloc: not available with armed observers (their drains allocate)");
+  if (s->variant == 1 || s->temporal_block != 1 || s->coef_mode != 0)
+    return fail(s, TEUK_EINVAL, "teuk_step_noalloc: needs kernel -1, 0 or 2, temporal_block 1, coef_mode 0");
+  int rows = 0, ncta = 0;
+  if (!resident_plan(s, &rows, &ncta))
+    return fail(s, TEUK_EINVAL, "teuk_step_noalloc: the state does not fit on chip (resident kernel: n_theta <= 128 and about n_modes*n_r*n_theta <= 5e5 points)");
+  const size_t need = teuk_resident_ll_bytes(s->n_theta, s->n_modes, ncta);
+  if (need > teuk_resident_static_capacity()) {
+    char buf[200];
+    snprintf(buf, sizeof(buf), "teuk_step_noalloc: exchange scratch of %zu bytes exceeds the static maximum of %zu bytes",
+             need, teuk_resident_static_capacity());
+    return fail(s, TEUK_EINVAL, buf);
+  }
+  if (s->has_source && 2 * (n0 + n) > s->n_samples)
+    return fail(s, TEUK_EINVAL, "teuk_step_noalloc: trajectory table too short for n0 + n iterations");
+  double* planes[4];
+  for (int c = 0; c < 4; ++c) planes[c] = const_cast<double*>(in_dev[c]);
+  CK(teuk_launch_pack(s->d_u[s->cur], planes, (size_t)s->n_modes * s->n_r, s->n_theta, s->stream), "step_noalloc: pack");
+  s->launches += 1;
+  const long long k = n0 - s->base_on_device;
+  if (k < 0 || k > (1LL << 30)) {
+    CK(teuk_launch_set_base(s->d_base, n0, s->stream), "step_noalloc: counter");
+    s->base_on_device = n0;
+    s->launches += 1;
+  }
+  StepParams p;                        // (captured graphs of kernel 0 stay valid: they address the buffers by parity)
+  fill_params(s, &p, s->cur, (int)(n0 - s->base_on_device), 0);
+  p.n_iter = (int)n;
+  p.res_rows = rows;
+  p.res_cache = s->res_cache_opt && s->n_terms == 0 &&
+                teuk_resident_smem_bytes(s->n_theta, rows, 1) <= (size_t)s->smem_optin;
+  CK(teuk_launch_step_resident_static(p, ncta, s->stream), "step_noalloc: resident launch");
+  s->launches += 1;
+  s->cur ^= 1;
+  s->step = n0 + n;
+  for (int c = 0; c < 4; ++c) planes[c] = out_dev[c];
+  CK(teuk_launch_unpack(s->d_u[s->cur], planes, (size_t)s->n_modes * s->n_r, s->n_theta, s->stream), "step_noalloc: unpack");
+  s->launches += 1;
   return TEUK_OK;
 }
 

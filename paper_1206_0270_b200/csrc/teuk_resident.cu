@@ -421,3 +421,39 @@ cudaError_t teuk_launch_step_resident(const StepParams& p, int ncta, cudaStream_
   return launch_resident_v<4, false>(p, ncta, st);
 }
 
+
+// ---- allocation-free variant (teuk_step_noalloc, include/teuk.h) -------------------------------------------
+// Some callers cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+// it).  For them the block-to-block exchange buffer of the resident kernel -- its only scratch memory, normally
+// cudaMalloc'ed by the first teuk_step -- lives in this file-scope device array: TEUK_STATIC_LL_BYTES = 5 MiB, held
+// by every GPU that loads the library until the process exits; enough for 148 blocks of the widest rows (V = 4:
+// 148 x 4 rows x 512 elements x 16 B = 4.6 MiB).  In host code the array's NAME is a host-side stand-in, not a
+// device address: the address is asked for once per device, with that device current, by cudaGetSymbolAddress.
+// Every call shares the array and finds the previous call's rows and tags in it, so each call first clears the
+// part it uses (stream-ordered memset) and starts its tags at 0; calls that overlap on the GPU would race.
+#define TEUK_STATIC_LL_BYTES (5u << 20)
+static __device__ __align__(256) unsigned char g_static_ll[TEUK_STATIC_LL_BYTES];
+
+size_t teuk_resident_static_capacity() { return (size_t)TEUK_STATIC_LL_BYTES; }
+
+// Like teuk_launch_step_resident with p.ll / p.tag0 replaced by the static scratch.  No allocation of any kind.
+cudaError_t teuk_launch_step_resident_static(const StepParams& p, int ncta, cudaStream_t st) {
+  const size_t need = teuk_resident_ll_bytes(p.n_theta, p.n_modes, ncta);
+  if (need > (size_t)TEUK_STATIC_LL_BYTES) return cudaErrorInvalidValue;      // the caller checks first and reports
+  static void* addr[64] = {nullptr};     // per device: a symbol has one address in every context
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (!addr[dev & 63]) {
+    void* ptr = nullptr;
+    e = cudaGetSymbolAddress(&ptr, g_static_ll);
+    if (e != cudaSuccess) return e;
+    addr[dev & 63] = ptr;
+  }
+  e = cudaMemsetAsync(addr[dev & 63], 0, need, st);                           // stale rows and tags of the last call
+  if (e != cudaSuccess) return e;
+  StepParams pc = p;
+  pc.ll = addr[dev & 63];
+  pc.tag0 = 0;
+  return teuk_launch_step_resident(pc, ncta, st);
+}

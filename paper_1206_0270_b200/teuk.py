@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libteuk.so")
 
 TEUK_OK, TEUK_EINVAL, TEUK_ENOMEM, TEUK_ECUDA, TEUK_ENONFINITE = 0, -1, -2, -3, -4
-SYMBOLS = ["teuk_select_device", "teuk_measure_fp64", "teuk_create", "teuk_set_initial", "teuk_set_source", "teuk_set_source_terms", "teuk_step", "teuk_extract",
+SYMBOLS = ["teuk_select_device", "teuk_measure_fp64", "teuk_create", "teuk_set_initial", "teuk_set_source", "teuk_set_source_terms", "teuk_step", "teuk_step_noalloc", "teuk_extract",
            "teuk_get_state", "teuk_set_option", "teuk_get_stat", "teuk_sync", "teuk_destroy",
            "teuk_last_error"]
 
@@ -61,6 +61,7 @@ def load():
     _ip = C.POINTER(C.c_int32)
     L.teuk_set_source_terms.argtypes = [vp, C.c_int32, _ip, _ip, _dp, _dp]
     L.teuk_step.argtypes = [vp, C.c_int64]
+    L.teuk_step_noalloc.argtypes = [vp, C.POINTER(vp), C.c_int64, C.c_int64, C.POINTER(vp)]
     L.teuk_extract.argtypes = [vp, C.c_double, _dp, _dp, _dp, _dp, C.c_int64, C.POINTER(C.c_int64)]
     L.teuk_get_state.argtypes = [vp, vp, vp, vp, vp, C.c_int32]
     L.teuk_set_option.argtypes = [vp, C.c_char_p, C.c_int64]
@@ -196,6 +197,21 @@ class Solver:
 
     def step(self, n=1):
         self._check(self._lib.teuk_step(self._h, int(n)))
+
+    def step_noalloc(self, fields_in, n0, n, fields_out):
+        """teuk_step_noalloc: advance the 4 DEVICE tensors `fields_in` (level n0; None = zeros) by n iterations into
+        the 4 device tensors `fields_out` (None = skip) with the resident kernel, allocating nothing."""
+        def pack(arrs):
+            a4 = (C.c_void_p * 4)()
+            for k, a in enumerate(arrs):
+                if a is None:
+                    a4[k] = None
+                    continue
+                assert hasattr(a, "data_ptr") and a.is_cuda, "teuk_step_noalloc takes device tensors"
+                assert tuple(a.shape) == self.shape and a.is_contiguous() and a.element_size() == 8
+                a4[k] = a.data_ptr()
+            return a4
+        self._check(self._lib.teuk_step_noalloc(self._h, pack(fields_in), int(n0), int(n), pack(fields_out)))
 
     def add_observer(self, rs_obs, weights=None):
         """First teuk_extract call with a new rs_obs: arms the observer."""
