@@ -37,9 +37,6 @@ struct Row {
 #ifndef TEUK_FAST_RSQRT
 #define TEUK_FAST_RSQRT 1   // own MUFU.RSQ64H + one third-order step instead of CUDA's rsqrt(): +6 GPts/s
 #endif
-#ifndef TEUK_UNROLL2
-#define TEUK_UNROLL2 1      // marching loop body instantiated twice with swapped roles (no register rotation): +3
-#endif
 #ifndef TEUK_SLOTS
 #define TEUK_SLOTS 2    // TMA landing slots per warp (register kernel): rows i+2 .. i+TEUK_SLOTS+1 in flight (3, 4: no gain)
 #endif

@@ -22,9 +22,18 @@
 //   B = (2 beta^'/dx) D_Phi + alpha^ E2 + cL^ L'_theta S_Phi + i G1 S_Phi,
 // which uses kappa dPhi + alpha Pi = Q[(beta^ - Q s2 X3) dPhi + alpha^ (Pi - b dPhi)].
 //
+// Loop structure of teuk_step_kernel (round 2): an outer loop over chunks of RT_CH = 16 rows does everything that
+// is rare or per-chunk (r-table chunk hand-over, the radial deposit profile of the chunk's rows -- one exp per lane,
+// kept in a register and fetched by shuffle --, the waveform tap of observers in the chunk), and the inner loop is
+// the marching iteration proper, instantiated twice with the roles of the row / half-row registers swapped (no
+// register rotation): two stages, one TMA issue, one row store.  With the cold code (exp and division slow paths
+// of the deposit, the tap) inlined three times INSIDE the marching loop, as in round 1, the V = 2 kernel spent 16 %
+// of its stall samples waiting for instructions and ran 566 instructions per warp-row for 257 FP64 ones: config 3
+// 64 -> 89 GPts/s, config 4 72 -> 81-87 with this structure, bit-identical results (profiles/r2_bench.md).
+//
 // Kernels in this file: teuk_step_kernel (register-resident marching kernel, the default; template flags
 // VEC = vector/TMA path, CM = coefficients rebuilt / streamed planes, SEG = theta segments, FULLW =
-// n_theta == 32 V compile-time), teuk_step_smem_kernel (same arithmetic, state in shared memory; bitwise
+// n_theta == 32 V compile-time, TERMS = multi-term deposit), teuk_step_smem_kernel (same arithmetic, state in shared memory; bitwise
 // cross-check), teuk_flush_tap_kernel, pack/unpack and counter kernels.  The compile-time knobs below
 // record what was measured on config 5 (profiles/r1_step_kernel_full.md); the defaults are the winners.
 #include <cuda_runtime.h>
@@ -186,6 +195,80 @@ __global__ void __launch_bounds__(128, (V == 2 ? TEUK_V2_BLOCKS : TEUK_MIN_BLOCK
   add_source<V>(hp, src_h, p, r0 - 1, true);
 
   const double* rt_cur = rt_buf;
+  // Work that is rare or happens once per RT_CH rows is kept OUT of the marching iteration, in chunk_begin: the
+  // r-table chunk hand-over, the radial deposit profile of the chunk's rows (one exp per lane: lanes 0-15 hold
+  // dt * P(x_{i+1/2} - x_p) of the half stage for rows cb .. cb+15, lanes 16-31 dt * P(x_i - x_p) of the full stage;
+  // the marching iteration fetches its row's value with one shuffle), and the waveform tap of observers whose cell
+  // starts in the chunk (read from the input level in global memory: same values as the register rows, same
+  // summation order).  The marching iteration is then two stages, one TMA issue, one store and nothing else: a
+  // short hot loop without cold branches in it.
+  double gprof = 0.0;
+  auto chunk_begin = [&](const int cb) {
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncwarp();
+    const int c = (cb - r0) / RT_CH;
+    rt_cur = rt_buf + (c & 1) * RT_CHUNK_DOUBLES;
+    if (cb + RT_CH < r1)
+      stage_rtab_chunk(rt_buf + ((c + 1) & 1) * RT_CHUNK_DOUBLES, rtab, 2 * (cb + RT_CH), 2 * nr - 1, lane);
+    if (!TERMS && any_src) {
+      const bool hf = lane < 16;
+      const int i = cb + (lane & 15);
+      const bool on = hf ? src_h.on : src_f.on;
+      const int ip = hf ? src_h.ip : src_f.ip;
+      double g = 0.0;
+      if (on && i < r1 && abs(i - ip) <= p.W) {
+        double x = __dadd_rn(p.rs_min, __dmul_rn((double)i, p.dx));
+        if (hf) x = __dadd_rn(x, __dmul_rn(0.5, p.dx));
+        g = p.dt * deposit_profile(p.source_kind, x - (hf ? src_h.xp : src_f.xp), p.sigma_r);
+      }
+      gprof = g;
+    }
+    if (do_tap) {
+      for (int q = 0; q < p.n_obs; ++q) {
+        const int i0 = p.obs[q].i0;
+        if (i0 < cb || i0 >= min(cb + RT_CH, r1)) continue;
+        const double* lo = uin + (size_t)i0 * row_stride;
+        const double* hi = lo + row_stride;
+        const double f = p.obs[q].f;
+        double wr = 0.0, wi = 0.0;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+          const int j = lane * V + v;
+          const bool ok = j < p.n_theta;
+          const double wt = ok ? __ldg(p.obs[q].weights + j) : 0.0;
+          const double lr = ok ? lo[j] : 0.0, li = ok ? lo[nth + j] : 0.0;
+          const double hr = ok ? hi[j] : 0.0, hi_i = ok ? hi[nth + j] : 0.0;
+          wr = fma(wt, fma(f, hr, (1.0 - f) * lr), wr);
+          wi = fma(wt, fma(f, hi_i, (1.0 - f) * li), wi);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          wr += __shfl_xor_sync(FULL, wr, o);
+          wi += __shfl_xor_sync(FULL, wi, o);
+        }
+        if (lane == 0) {
+          const long long slot = (n - 1) % p.ring_cap;
+          double* dst = p.obs[q].ring + ((size_t)slot * p.n_modes + mode) * 2;
+          dst[0] = wr;
+          dst[1] = wi;
+          if (!isfinite(wr) || !isfinite(wi)) *p.nonfinite = 1;
+        }
+      }
+    }
+  };
+  // dt * T on this lane's columns of row i: g = the row's radial profile value (0 outside the window)
+  auto deposit = [&](Row<V>& o_, const typename SourceSel<V, TERMS>::type& s_, const double g) {
+    if constexpr (!TERMS) {
+      if (g != 0.0) {
+#pragma unroll
+        for (int q = 0; q < V; ++q) {
+          const double gg = g * s_.gth[q];
+          o_.c[2][q] = fma(s_.are, gg, o_.c[2][q]);
+          o_.c[3][q] = fma(s_.aim, gg, o_.c[3][q]);
+        }
+      }
+    }
+  };
   // One marching iteration at node i.  On entry A = u^n_i, B = u^n_{i+1}, Hp = 2 u^{n+1/2}_{i-1/2};
   // on exit Hn = 2 u^{n+1/2}_{i+1/2} and A = u^n_{i+2}.  The caller alternates the roles of
   // (A, B) and (Hp, Hn), so no register rotation is needed.
@@ -194,15 +277,6 @@ __global__ void __launch_bounds__(128, (V == 2 ? TEUK_V2_BLOCKS : TEUK_MIN_BLOCK
       if (i + 2 <= r1) load_row<V, VEC>(ua, uin + (size_t)(i + 2) * row_stride, nth, j0);
     }
     const int o = (i - r0) & (RT_CH - 1);
-    if (o == 0) {  // chunk boundary (warp-uniform): current chunk has landed, start the next one
-      asm volatile("cp.async.wait_group 0;" ::: "memory");
-      __syncwarp();
-      const int c = (i - r0) / RT_CH;
-      rt_cur = rt_buf + (c & 1) * RT_CHUNK_DOUBLES;
-      if (i + RT_CH < r1)
-        stage_rtab_chunk(rt_buf + ((c + 1) & 1) * RT_CHUNK_DOUBLES, rtab, 2 * (i + RT_CH), 2 * nr - 1, lane);
-    }
-    if (do_tap) tap<V>(A, B, p, i, mode, n, lane);
     if (CM == 1) {
       // pull the next iteration's two coefficient rows (2 x 8 planes) towards L2 while this one computes
       if (i + 1 < r1) {
@@ -214,7 +288,10 @@ __global__ void __launch_bounds__(128, (V == 2 ? TEUK_V2_BLOCKS : TEUK_MIN_BLOCK
     } else {
       lw_stage<V, true>(A, B, A, rt_cur + (2 * o + 1) * RT_N, th, tau_h, tdx, Hn);
     }
-    if (any_src) add_source<V>(Hn, src_h, p, i, true);
+    if (any_src) {
+      if constexpr (TERMS) add_source<V>(Hn, src_h, p, i, true);
+      else deposit(Hn, src_h, __shfl_sync(FULL, gprof, o));
+    }
     if (VEC) {
       // B (row i+1, copied out of slot (i+1) % NS at the end of the last iteration) has been consumed by
       // every lane: its slot may now receive row i+NS+1.
@@ -225,7 +302,10 @@ __global__ void __launch_bounds__(128, (V == 2 ? TEUK_V2_BLOCKS : TEUK_MIN_BLOCK
       lw_stage_planes<V, false, VEC>(Hp, Hn, A, planes + (size_t)(2 * i) * loc_stride, th, tau_f, out, nth, j0);
     else
       lw_stage<V, false>(Hp, Hn, A, rt_cur + (2 * o) * RT_N, th, tau_f, tdx, out);
-    if (any_src) add_source<V>(out, src_f, p, i, false);
+    if (any_src) {
+      if constexpr (TERMS) add_source<V>(out, src_f, p, i, false);
+      else deposit(out, src_f, __shfl_sync(FULL, gprof, 16 + o));
+    }
     store_row<V, VEC>(out, uout + (size_t)i * row_stride, nth, j0, pay_lo, pay_hi);
     if (VEC) {
       if (i + 2 <= r1) {
@@ -236,21 +316,17 @@ __global__ void __launch_bounds__(128, (V == 2 ? TEUK_V2_BLOCKS : TEUK_MIN_BLOCK
       A = ua;
     }
   };
-  {
-    int i = r0;
-#if TEUK_UNROLL2
-    for (; i + 1 < r1; i += 2) {
+  static_assert(RT_CH == 16, "chunk_begin keeps one chunk's deposit profile in the two halves of a warp");
+  for (int cb = r0; cb < r1; cb += RT_CH) {
+    chunk_begin(cb);
+    const int ce = min(cb + RT_CH, r1);
+    int i = cb;
+#pragma unroll 1
+    for (; i + 1 < ce; i += 2) {
       march(i, ub, uc, hp, hn);
       march(i + 1, uc, ub, hn, hp);
     }
-    if (i < r1) march(i, ub, uc, hp, hn);
-#else
-    for (; i < r1; ++i) {
-      march(i, ub, uc, hp, hn);
-      hp = hn;
-      Row<V> t = ub; ub = uc; uc = t;
-    }
-#endif
+    if (i < ce) march(i, ub, uc, hp, hn);     // odd row count: only the last chunk can have one
   }
 
   // radial edges (outer edge: DESIGN.md reading A6)
