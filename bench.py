@@ -254,6 +254,9 @@ def main():
     ap.add_argument("--graph", type=int, default=1)
     ap.add_argument("--coef-mode", type=int, default=0, help="0 rebuild coefficients (default), 1 stream 2D planes")
     ap.add_argument("--source-kind", type=int, default=0, help="0 Gaussian deposit (the configs'), 1 / 2 discrete delta")
+    ap.add_argument("--source-terms", type=int, default=0,
+                    help="0: the config's single-term deposit; N = 1..6: deposit N rank-1 terms with derivative profiles "
+                         "(teuk_set_source_terms, f2) to time the TERMS instantiation of the kernels")
     ap.add_argument("--temporal-block", type=int, default=0, help="0 library default, 1 or 2 iterations per HBM round trip")
     ap.add_argument("--pdl", type=int, default=-1, help="-1 library default, 0/1 programmatic dependent launch inside graph batches")
     ap.add_argument("--kernel", type=int, default=-1, help="-1 library default (automatic), 0 marching kernel, 1 smem-resident marching kernel, 2 resident (state on chip)")
@@ -321,6 +324,11 @@ def main():
                * 1e-3 for _ in range(4)]
         g.set_initial(*dev)
         g.set_source(orbit)
+        if args.source_terms and orbit is not None:
+            # f2: the first N of (delta, d/dx, d/dtheta, d2/dx2, d2/dxdtheta, d2/dtheta2), each with the table's amplitude
+            specs = [(0, 0), (1, 0), (0, 1), (2, 0), (1, 1), (0, 2)][:args.source_terms]
+            amp = orbit["amp_re"] + 1j * orbit["amp_im"]
+            g.set_source_terms([(a_, b_, amp * (cfg.dx ** a_) * (cfg.dtheta ** b_)) for a_, b_ in specs])
         for x in cfg.observers:
             g.add_observer(x, weights)
         # ---- device-resident timing -----------------------------------------------------------
@@ -363,7 +371,7 @@ def main():
             barrier()
             t0 = time.perf_counter()
             g.set_initial(*host_in)                 # H2D: 4 planes
-            g.set_source(orbit_e2e)                 # H2D: trajectory table
+            g.set_source(orbit_e2e)                 # H2D: trajectory table (a --source-terms run times the e2e leg with the single term)
             g.step(K)
             series = [g.extract(x, allow_nonfinite=True) for x in cfg.observers]   # D2H: waveforms
             g.get_state(host_out)                   # D2H: 4 planes
@@ -386,7 +394,7 @@ def main():
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfg.name, "grid": [cfg.n_r, cfg.n_theta], "modes": list(cfg.modes), "a": cfg.a,
-                       "dt": cfg.dt, "source": cfg.source, "source_kind": args.source_kind, "coef_mode": args.coef_mode, "slab_rows": int(slab_rows), "kernel": int(kernel_used), "temporal_block": args.temporal_block or "default", "observers": list(cfg.observers),
+                       "dt": cfg.dt, "source": cfg.source, "source_kind": args.source_kind, "source_terms": args.source_terms, "coef_mode": args.coef_mode, "slab_rows": int(slab_rows), "kernel": int(kernel_used), "temporal_block": args.temporal_block or "default", "observers": list(cfg.observers),
                        "state_mb": 4 * cfg.n_pts * 8 / 1e6, "parallelism": "replicas x%d" % world,
                        "extra_untimed_warmup": XW,
                        "l2": "inputs larger than L2 (two 537 MB state copies stream through a 126 MB L2)"
