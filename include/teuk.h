@@ -200,6 +200,12 @@ int teuk_get_state(teuk_solver *s, double *phi_re, double *phi_im, double *pi_re
  *                   All kernels do the same arithmetic per point: fields are bitwise identical (waveforms too,
  *                   except kernel 1, which sums over theta in another order).  An explicit "slab_rows" makes the
  *                   automatic choice stay with kernel 0.
+ *   "wide"          how kernel 0 maps rows wider than 64 columns onto warps: 0 = one warp per row (V = 4 columns per
+ *                   lane, n_theta <= 128) or per theta segment with recomputed halo columns (n_theta > 128);
+ *                   1 = a GROUP of ceil(n_theta / 64) warps per row, V = 2 columns per lane, the boundary columns of
+ *                   the theta stencil exchanged through shared memory (needs an even n_theta between 66 and 320,
+ *                   coef_mode 0, temporal_block 1, the single-term deposit; otherwise the setting is ignored);
+ *                   -1 (default) = automatic.  Same results bit for bit.
  *   "pdl"           1 (default) = inside a CUDA-graph batch, iteration k + 1 of kernel 0 is launched as a programmatic
  *                   dependent of iteration k (its prologue overlaps k's tail); 0 = fully serialised launches
  *   "resident_cache" 1 (default) = kernel 2 also keeps the time-independent coefficients b, b^2 and Re beta' of its
@@ -209,6 +215,7 @@ int teuk_set_option(teuk_solver *s, const char *key, int64_t value);
 
 /* Read-only counters: "steps" (iterations done), "launches" (kernels launched so far),
  * "n_pts" (n_modes*n_r*n_theta), "state_bytes" (one copy of the fields), "slab_rows" (longest slab in use), "slabs" (slabs per mode),
+ * "wide" (1 if the next teuk_step would run the group-of-warps-per-row kernel),
  * "kernel" (the kernel the next teuk_step would run), "resident_rows" / "resident_blocks" (rows of r* per
  * block and blocks of kernel 2, 0 if it is not in use). */
 int teuk_get_stat(const teuk_solver *s, const char *key, int64_t *value);

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libteuk.so")
-SOURCES = ["teuk_api.cu", "teuk_step.cu", "teuk_resident.cu", "teuk_tables.cu", "teuk_peak.cu"]
+SOURCES = ["teuk_api.cu", "teuk_step.cu", "teuk_resident.cu", "teuk_tables.cu", "teuk_peak.cu", "teuk_wide.cu"]
 HEADERS = [os.path.join(CSRC, "teuk_internal.h"), os.path.join(CSRC, "teuk_stage.cuh"), os.path.join(HERE, "..", "include", "teuk.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]

@@ -20,6 +20,9 @@ cudaError_t teuk_launch_coef2d(double* c2d, const double* rtab, const double* tt
                                int n_theta, double dx, cudaStream_t st);
 cudaError_t teuk_launch_step(const StepParams& p, cudaStream_t st);
 cudaError_t teuk_launch_step_tb2(const StepParams& p, cudaStream_t st);
+cudaError_t teuk_launch_step_wide(const StepParams& p, cudaStream_t st);
+bool teuk_wide_applies(int n_theta);
+int teuk_wide_groups_per_sm(int n_theta);
 cudaError_t teuk_launch_step_resident(const StepParams& p, int ncta, cudaStream_t st);
 size_t teuk_resident_smem_bytes(int n_theta, int res_rows, int coef_cache);
 size_t teuk_resident_ll_bytes(int n_theta, int n_modes, int ncta);
@@ -67,6 +70,7 @@ struct teuk_solver {
   int outer_bc, coef_mode, slab_rows_opt, use_graph, variant, autotune;
   int tuned_rows;        // slabs per mode chosen by the one-time autotune (0 = not tuned yet)
   int temporal_block;    // 1 = one iteration per launch, 2 = two (warp pairs, level n+1 stays on chip)
+  int wide_opt;          // "wide" option: -1 automatic, 0 = one warp per row / theta segment, 1 = a group of warps per row
   int tuned_rows2;       // autotuned slabs per mode of the temporal-blocking kernel
   int force_slabs;       // autotune in progress: slabs per mode of the candidate being timed
   // resident kernel ("kernel" = 2): rows per block, blocks per mode, exchange buffer and its running tag
@@ -174,11 +178,25 @@ int n_segments(const teuk_solver* s) {
   return (s->n_theta + 119) / 120;
 }
 
+// The wide kernel (teuk_wide.cu: a group of ceil(n_theta / 64) warps per row, V = 2 columns per lane) replaces the
+// one-warp-per-row kernel and the theta segments when it applies and is asked for (or chosen by default).
+const int kWideByDefault = 0;
+bool wide_active(const teuk_solver* s) {
+  if (s->wide_opt == 0 || (s->wide_opt < 0 && !kWideByDefault)) return false;
+  return s->variant == 0 && s->coef_mode == 0 && s->temporal_block == 1 && s->n_terms == 0 && teuk_wide_applies(s->n_theta);
+}
+// slabs per row: theta segments of the one-warp-per-row kernel; the wide kernel marches whole rows
+int seg_factor(const teuk_solver* s) { return wide_active(s) ? 1 : n_segments(s); }
+cudaError_t launch_step_any(const teuk_solver* s, const StepParams& p, cudaStream_t st) {
+  return wide_active(s) ? teuk_launch_step_wide(p, st) : teuk_launch_step(p, st);
+}
+
 // Heuristic slab length (rows of r* marched by one warp): two waves of the warps that fit on the chip.
 // It seeds the autotune below and is used as is when autotuning is switched off.
 int resident_warps(const teuk_solver* s) {
   const int sms = s->n_sms > 0 ? s->n_sms : 148;
   const int v = (s->n_theta + 31) / 32;
+  if (wide_active(s)) return sms * teuk_wide_groups_per_sm(s->n_theta);      // slabs in flight = groups of warps
   return sms * (s->variant == 1 ? 12 : (v <= 1 ? 16 : (v == 2 ? 12 : 8)));   // occupancies of the kernels
 }
 
@@ -217,7 +235,7 @@ bool resident_active(const teuk_solver* s, int* res_rows, int* ncta) {
 int rows_for_waves(const teuk_solver* s, double waves, int tb = 1) {
   const long long interior = s->n_r - 2;
   const double target = waves * resident_warps(s) / tb;   // tb = 2: a slab occupies a pair of warps
-  long long rows = (long long)((interior * s->n_modes * n_segments(s) + target - 1) / target);
+  long long rows = (long long)((interior * s->n_modes * seg_factor(s) + target - 1) / target);
   if (rows < 1) rows = 1;
   if (rows > interior) rows = interior;
   return (int)rows;
@@ -451,6 +469,7 @@ int teuk_create(teuk_solver** out, double a, double M, const int32_t* m, int32_t
   for (int q = 0; q < n_modes; ++q) s->m[q] = m[q];
   s->outer_bc = 0; s->coef_mode = 0; s->slab_rows_opt = 0; s->use_graph = 1; s->autotune = 1; s->tuned_rows = 0; s->temporal_block = 1; s->tuned_rows2 = 0;
   s->kernel_opt = -1;
+  s->wide_opt = -1;
   s->res_cache_opt = 1;
   s->use_pdl = 1;
   s->device = dev;
@@ -596,8 +615,12 @@ int teuk_set_source_terms(teuk_solver* s, int32_t n_terms, const int32_t* order_
   drop_graph(s);
   cudaFree(s->d_term_re); cudaFree(s->d_term_im);
   s->d_term_re = s->d_term_im = nullptr;
+  const bool had_terms = s->n_terms > 0;
   s->n_terms = 0;
-  if (n_terms == 0) return TEUK_OK;
+  if (n_terms == 0) {
+    if (had_terms) { s->tuned_rows = 0; return tune_if_needed(s); }
+    return TEUK_OK;
+  }
   const size_t n = (size_t)n_terms * s->n_modes * (size_t)s->n_samples;
   CK(cudaMalloc((void**)&s->d_term_re, n * sizeof(double)), "set_source_terms: alloc");
   CK(cudaMalloc((void**)&s->d_term_im, n * sizeof(double)), "set_source_terms: alloc");
@@ -609,7 +632,8 @@ int teuk_set_source_terms(teuk_solver* s, int32_t n_terms, const int32_t* order_
     s->term_oth[t] = (signed char)order_theta[t];
   }
   s->n_terms = n_terms;
-  return TEUK_OK;
+  s->tuned_rows = 0;               // another kernel instantiation runs from now on: measure its launch shape
+  return tune_if_needed(s);
 }
 
 }  // extern "C"
@@ -622,7 +646,7 @@ int build_graph(teuk_solver* s, int tb) {
   cudaGraph_t graph = nullptr;
   CK(cudaStreamBeginCapture(s->own_stream, cudaStreamCaptureModeThreadLocal), "graph: begin capture");
   cudaError_t e = cudaSuccess;
-  const bool sep_tap = n_segments(s) > 1 && s->n_obs > 0;   // theta segments: the tap is its own small kernel
+  const bool sep_tap = seg_factor(s) > 1 && s->n_obs > 0;   // theta segments: the tap is its own small kernel
   if (tb == 2) {
     for (int j = 0; j < kGraphBatch / 2 && e == cudaSuccess; ++j) {
       StepParams p;
@@ -635,7 +659,7 @@ int build_graph(teuk_solver* s, int tb) {
       fill_params(s, &p, s->cur ^ (k & 1), k, sep_tap ? 0 : 1);
       // iterations 2..32 of the batch follow another step kernel directly: their prologue may overlap its tail
       p.pdl = (s->use_pdl && k > 0 && !sep_tap && s->variant == 0) ? 1 : 0;
-      e = teuk_launch_step(p, s->own_stream);
+      e = launch_step_any(s, p, s->own_stream);
       if (sep_tap && e == cudaSuccess) {
         fill_params(s, &p, s->cur ^ ((k + 1) & 1), k + 1, 1);
         e = teuk_launch_flush_tap(p, s->own_stream);
@@ -681,7 +705,7 @@ int tune_slab_rows(teuk_solver* s, int tb) {
     }
   }
   // whole numbers of waves: k times the warps that are resident at once, shared by the modes and theta segments
-  const long long per_wave = (long long)resident_warps(s) / tb / ((long long)s->n_modes * n_segments(s));
+  const long long per_wave = (long long)resident_warps(s) / tb / ((long long)s->n_modes * seg_factor(s));
   for (int k = 1; k <= 6; ++k) add(k * per_wave);
   cudaEvent_t e0, e1;
   CK(cudaEventCreate(&e0), "autotune: event");
@@ -695,7 +719,7 @@ int tune_slab_rows(teuk_solver* s, int tb) {
     p.tap_enable2 = 0;
     p.has_source = 0;      // trial launches read nothing but the state and the tables (no trajectory sample, no observer)
     p.n_obs = 0;
-    auto launch = [&]() { return tb == 2 ? teuk_launch_step_tb2(p, s->stream) : teuk_launch_step(p, s->stream); };
+    auto launch = [&]() { return tb == 2 ? teuk_launch_step_tb2(p, s->stream) : launch_step_any(s, p, s->stream); };
     cudaError_t e = launch();                                      // warm-up
     float ms = 0.f;
     int reps = 3;
@@ -809,7 +833,7 @@ int run_chunk(teuk_solver* s, long long c) {
       CK(cudaGraphLaunch(*ge, s->stream), "step: graph launch");
       s->base_on_device += kGraphBatch;
       s->step += kGraphBatch;
-      s->launches += (tb2 ? kGraphBatch / 2 : kGraphBatch * (n_segments(s) > 1 && s->n_obs > 0 ? 2 : 1)) + 1;
+      s->launches += (tb2 ? kGraphBatch / 2 : kGraphBatch * (seg_factor(s) > 1 && s->n_obs > 0 ? 2 : 1)) + 1;
       left -= kGraphBatch;
       continue;
     }
@@ -830,10 +854,10 @@ int run_chunk(teuk_solver* s, long long c) {
       first = 0;
       continue;
     }
-    const bool sep_tap = n_segments(s) > 1 && s->n_obs > 0;
+    const bool sep_tap = seg_factor(s) > 1 && s->n_obs > 0;
     StepParams p;
     fill_params(s, &p, s->cur, (int)(s->step - s->base_on_device), (first || sep_tap) ? 0 : 1);
-    CK(teuk_launch_step(p, s->stream), "step: launch");
+    CK(launch_step_any(s, p, s->stream), "step: launch");
     s->launches += 1;
     s->cur ^= 1;
     s->step += 1;
@@ -1060,6 +1084,11 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
     s->slab_rows_opt = (int)value;
   } else if (!strcmp(key, "graph")) {
     s->use_graph = value ? 1 : 0;
+  } else if (!strcmp(key, "wide")) {
+    if (value < -1 || value > 1) return fail(s, TEUK_EINVAL, "wide must be -1 (automatic), 0 or 1");
+    if (value == 1 && !teuk_wide_applies(s->n_theta))
+      return fail(s, TEUK_EINVAL, "wide 1 needs an even n_theta between 66 and 320");
+    s->wide_opt = (int)value;
   } else if (!strcmp(key, "pdl")) {
     s->use_pdl = value ? 1 : 0;
   } else if (!strcmp(key, "resident_cache")) {
@@ -1094,7 +1123,7 @@ int teuk_set_option(teuk_solver* s, const char* key, int64_t value) {
   drop_graph(s);
   // options that change the launch shape of the marching kernels: measure it again, here, so that teuk_step
   // never has to wait for the device
-  if (!strcmp(key, "kernel") || !strcmp(key, "coef_mode") || !strcmp(key, "temporal_block") ||
+  if (!strcmp(key, "kernel") || !strcmp(key, "coef_mode") || !strcmp(key, "temporal_block") || !strcmp(key, "wide") ||
       !strcmp(key, "slab_rows") || !strcmp(key, "autotune")) {
     s->tuned_rows = 0;
     s->tuned_rows2 = 0;
@@ -1115,6 +1144,10 @@ int teuk_get_stat(const teuk_solver* s, const char* key, int64_t* value) {
     if (!strcmp(key, "kernel")) *value = res ? 2 : s->variant;
     else if (!strcmp(key, "resident_rows")) *value = res ? rr : 0;
     else *value = res ? (int64_t)nc * s->n_modes : 0;
+  }
+  else if (!strcmp(key, "wide")) {
+    int rr = 0, nc = 0;
+    *value = (!resident_active(s, &rr, &nc) && wide_active(s)) ? 1 : 0;
   }
   else if (!strcmp(key, "slabs")) *value = slabs_in_use(s, tb2_active(s) ? 2 : 1);
   else if (!strcmp(key, "slab_rows")) {                 // longest slab in use

@@ -206,10 +206,44 @@ __device__ __forceinline__ void theta_neighbours(const double (&f)[V], double (&
 // ---- one Lax-Wendroff stage at one radial location ------------------------------------------
 // HALF: A = u^n_i, B = u^n_{i+1}, out = 2 u^{n+1/2}_{i+1/2}             (Eq. 3, tau = dt/2)
 // else: A = H_{i-1/2}, B = H_{i+1/2} (doubled), out = u^{n+1}_i, base = u^n_i   (Eq. 4, tau = dt/4)
+// The stage comes in two pieces so that a kernel whose rows span several warps can exchange the boundary columns
+// of S_Phi between them (teuk_wide.cu): lw_stage_sums (S_Phi = A_Phi + B_Phi), then the theta-neighbours, then
+// lw_stage_body (everything else).  lw_stage = the three in a row, within one warp.
+template <int V>
+__device__ __forceinline__ void lw_stage_sums(const Row<V>& A, const Row<V>& B, double (&sfr)[V], double (&sfi)[V]) {
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    sfr[v] = A.c[0][v] + B.c[0][v];
+    sfi[v] = A.c[1][v] + B.c[1][v];
+  }
+}
+
+template <int V, bool HALF, class TT>
+__device__ __forceinline__ void lw_stage_body(const Row<V>& A, const Row<V>& B, const Row<V>& base,
+                                              const double* __restrict__ rec, const TT& tht, double tau,
+                                              double two_over_dx, Row<V>& out, const double (&sfr)[V],
+                                              const double (&sfi)[V], const double (&nlr)[V], const double (&nrr)[V],
+                                              const double (&nli)[V], const double (&nri)[V]);
+
 template <int V, bool HALF, int MAP = 0, class TT = ThetaTab<V>>
 __device__ __forceinline__ void lw_stage(const Row<V>& A, const Row<V>& B, const Row<V>& base,
                                          const double* __restrict__ rec, const TT& tht,
                                          double tau, double two_over_dx, Row<V>& out, int lane = 0) {
+  double sfr[V], sfi[V];
+  lw_stage_sums<V>(A, B, sfr, sfi);
+  // theta-neighbours across lanes (pole ghosts are folded into ap/am/d0; see teuk_ttab_kernel)
+  double nlr[V], nrr[V], nli[V], nri[V];
+  theta_neighbours<V, MAP>(sfr, nlr, nrr, lane);
+  theta_neighbours<V, MAP>(sfi, nli, nri, lane);
+  lw_stage_body<V, HALF, TT>(A, B, base, rec, tht, tau, two_over_dx, out, sfr, sfi, nlr, nrr, nli, nri);
+}
+
+template <int V, bool HALF, class TT>
+__device__ __forceinline__ void lw_stage_body(const Row<V>& A, const Row<V>& B, const Row<V>& base,
+                                              const double* __restrict__ rec, const TT& tht, double tau,
+                                              double two_over_dx, Row<V>& out, const double (&sfr)[V],
+                                              const double (&sfi)[V], const double (&nlr)[V], const double (&nrr)[V],
+                                              const double (&nli)[V], const double (&nri)[V]) {
   ThetaVals<V> th;
   tht.get(th);
   const double2 r01 = *reinterpret_cast<const double2*>(rec + 0);
@@ -219,17 +253,6 @@ __device__ __forceinline__ void lw_stage(const Row<V>& A, const Row<V>& B, const
   const double2 r89 = *reinterpret_cast<const double2*>(rec + 8);
   const double eps = r01.x, x32 = r01.y, bre2 = r23.x, bim2 = r23.y;
   const double a0 = r45.x, a1 = r45.y, a2 = r67.x, g1 = r67.y, gr = r89.x, cl = r89.y;
-
-  double sfr[V], sfi[V];
-#pragma unroll
-  for (int v = 0; v < V; ++v) {
-    sfr[v] = A.c[0][v] + B.c[0][v];
-    sfi[v] = A.c[1][v] + B.c[1][v];
-  }
-  // theta-neighbours across lanes (pole ghosts are folded into ap/am/d0; see teuk_ttab_kernel)
-  double nlr[V], nrr[V], nli[V], nri[V];
-  theta_neighbours<V, MAP>(sfr, nlr, nrr, lane);
-  theta_neighbours<V, MAP>(sfi, nli, nri, lane);
   // The V columns are processed in groups of G: inside a group every operation is written for all
   // G columns back to back, so consecutive FP64 instructions are independent (DFMA latency is 8
   // cycles at one issue per 2 cycles: a lone dependent chain leaves the pipe 3/4 idle).
@@ -674,6 +697,25 @@ static __device__ __forceinline__ void mbar_wait_u32(unsigned bar, unsigned pari
 }
 static __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
   mbar_wait_u32(smem_u32(bar), parity);
+}
+
+// r-table staging: the 2*RT_CH records (node + half point) of the next RT_CH marching iterations
+// are copied global -> shared with cp.async while the current chunk is being consumed, so the
+// warp-uniform coefficient loads are short LDS broadcasts instead of exposed L2 round trips.
+constexpr int RT_CH = 16;
+constexpr int RT_CHUNK_DOUBLES = RT_CH * 2 * RT_N;
+
+static __device__ __forceinline__ void stage_rtab_chunk(double* sbuf, const double* __restrict__ rtab, int p_begin,
+                                                 int n_loc, int lane) {
+  const size_t g0 = (size_t)p_begin * RT_N, gend = (size_t)n_loc * RT_N;
+#pragma unroll
+  for (int q = lane; q < RT_CHUNK_DOUBLES / 2; q += 32) {
+    if (g0 + 2 * q < gend) {
+      const unsigned saddr = (unsigned)__cvta_generic_to_shared(sbuf + 2 * q);
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(saddr), "l"(rtab + g0 + 2 * q) : "memory");
+    }
+  }
+  asm volatile("cp.async.commit_group;" ::: "memory");
 }
 
 // shared-memory row (same [comp][n_theta] layout as HBM) -> registers

@@ -44,25 +44,6 @@
 
 #include "teuk_stage.cuh"
 
-// r-table staging: the 2*RT_CH records (node + half point) of the next RT_CH marching iterations
-// are copied global -> shared with cp.async while the current chunk is being consumed, so the
-// warp-uniform coefficient loads are short LDS broadcasts instead of exposed L2 round trips.
-constexpr int RT_CH = 16;
-constexpr int RT_CHUNK_DOUBLES = RT_CH * 2 * RT_N;
-
-__device__ __forceinline__ void stage_rtab_chunk(double* sbuf, const double* __restrict__ rtab, int p_begin,
-                                                 int n_loc, int lane) {
-  const size_t g0 = (size_t)p_begin * RT_N, gend = (size_t)n_loc * RT_N;
-#pragma unroll
-  for (int q = lane; q < RT_CHUNK_DOUBLES / 2; q += 32) {
-    if (g0 + 2 * q < gend) {
-      const unsigned saddr = (unsigned)__cvta_generic_to_shared(sbuf + 2 * q);
-      asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(saddr), "l"(rtab + g0 + 2 * q) : "memory");
-    }
-  }
-  asm volatile("cp.async.commit_group;" ::: "memory");
-}
-
 // SEG: the theta range is split into gridDim.z segments of p.seg_payload columns (n_theta > 32 V, e.g. the
 // paper's 32000 x 304 grid).  A warp then owns a window of 32 V columns: its payload plus a
 // 4-column halo on each side, recomputed redundantly (the stencil reaches 2 columns per iteration), so no

@@ -713,3 +713,74 @@ def test_source_terms_reset_and_errors(orc, teuk):
         for a, b in zip(out[0], out[k]):
             assert np.array_equal(a, b), k
     assert np.abs(out[0][2]).max() > 0
+
+
+# ---- the wide kernel: a group of ceil(n_theta / 64) warps per row ("wide" = 1) -------------------------------
+def _run_gpu(teuk, cfg, steps, options, ini, orbit, observers, chunks=None):
+    g = teuk.Solver.from_config(cfg)
+    for k, v in options.items():
+        g.set_option(k, v)
+    g.set_initial(*ini)
+    g.set_source(orbit)
+    W = wl.observer_weights(cfg)
+    for x in observers:
+        g.add_observer(x, W)
+    for c in (chunks or [steps]):
+        g.step(c)
+    out = (g.get_state(), [g.extract(x) for x in observers], g.stat("wide"), g.stat("launches"))
+    g.close()
+    return out
+
+
+@pytest.mark.parametrize("n_theta", [66, 100, 128, 130, 192, 256, 304, 320])
+def test_wide_kernel_is_bitwise_identical(teuk, n_theta):
+    """Fields AND waveforms of the group-of-warps kernel equal those of the one-warp-per-row / theta-segment kernels
+    bit for bit: 2 .. 5 warps per row, idle lanes in the last warp, source window and observers (one in the first
+    cell, one in the last) crossing slab and chunk boundaries, plain launches, graph batches with and without pdl."""
+    cfg = SMALL[3].scaled(name="wide%d" % n_theta, n_r=211, n_theta=n_theta, dt_over_dx=0.002, steps=70, modes=(2, 1),
+                          rs_min=-30.0, rs_max=45.0)
+    dx = cfg.dx
+    obs = (30.0, cfg.rs_min + 0.3 * dx, cfg.rs_max - 1.2 * dx)
+    ini = wl.random_state(cfg, n_theta)
+    orbit = wl.orbit_table(cfg, n_steps=70)
+    ref = _run_gpu(teuk, cfg, 70, {"kernel": 0, "wide": 0}, ini, orbit, obs)
+    assert ref[2] == 0
+    for opt, chunks in (({"kernel": 0, "wide": 1}, None), ({"kernel": 0, "wide": 1, "pdl": 0}, [1, 2, 67]),
+                        ({"kernel": 0, "wide": 1, "graph": 0, "slab_rows": 5}, [35, 35]),
+                        ({"kernel": 0, "wide": 1, "slab_rows": 40}, None)):
+        got = _run_gpu(teuk, cfg, 70, opt, ini, orbit, obs, chunks)
+        assert got[2] == 1, "the wide kernel did not run"
+        for a, b in zip(ref[0], got[0]):
+            assert np.array_equal(a, b), (n_theta, opt)
+        for (ta, wa), (tb, wb) in zip(ref[1], got[1]):
+            assert len(ta) == 70 and np.array_equal(ta, tb) and np.array_equal(wa, wb), (n_theta, opt)
+
+
+@pytest.mark.parametrize("cfg", [SMALL[5], SMALL[5].scaled(name="wide_dirichlet_304", n_theta=304, n_r=400, outer_bc=1,
+                                                           dt_over_dx=0.01, steps=120)],
+                         ids=["kerr099_small_1500x128", "dirichlet_400x304"])
+def test_wide_kernel_parity(orc, teuk, cfg):
+    res = run_pair(orc, teuk, cfg, min(cfg.steps, 200), options={"kernel": 0, "wide": 1})
+    check_pair(res)
+
+
+def test_wide_option_applicability(teuk):
+    cfg = SMALL[3]                                   # n_theta = 64: one warp per row is all there is
+    g = teuk.Solver.from_config(cfg)
+    with pytest.raises(teuk.TeukError):
+        g.set_option("wide", 1)
+    g.close()
+    cfg = SMALL[5]
+    g = teuk.Solver.from_config(cfg)
+    g.set_option("kernel", 0)
+    g.set_option("wide", 1)
+    assert g.stat("wide") == 1
+    g.set_option("temporal_block", 2)                # variants the wide kernel does not cover: the setting is ignored
+    assert g.stat("wide") == 0
+    g.set_option("temporal_block", 1)
+    g.set_source(wl.orbit_table(cfg, n_steps=4))
+    g.set_source_terms([(1, 0, np.ones((cfg.n_modes, 9), dtype=complex))])
+    assert g.stat("wide") == 0
+    g.set_source_terms([])
+    assert g.stat("wide") == 1
+    g.close()
