@@ -259,6 +259,7 @@ def main():
                          "(teuk_set_source_terms, f2) to time the TERMS instantiation of the kernels")
     ap.add_argument("--temporal-block", type=int, default=0, help="0 library default, 1 or 2 iterations per HBM round trip")
     ap.add_argument("--pdl", type=int, default=-1, help="-1 library default, 0/1 programmatic dependent launch inside graph batches")
+    ap.add_argument("--wide", type=int, default=-1, help="-1 library default, 0 one warp per row / theta segment, 1 a group of warps per row")
     ap.add_argument("--kernel", type=int, default=-1, help="-1 library default (automatic), 0 marching kernel, 1 smem-resident marching kernel, 2 resident (state on chip)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -311,6 +312,8 @@ def main():
             g.set_option("kernel", args.kernel)
         if args.pdl >= 0:
             g.set_option("pdl", args.pdl)
+        if args.wide >= 0:
+            g.set_option("wide", args.wide)
         if args.coef_mode:
             g.set_option("coef_mode", args.coef_mode)
         if args.temporal_block:
@@ -350,6 +353,7 @@ def main():
         launches = g.stat("launches") - l0
         slab_rows = g.stat("slab_rows")
         kernel_used = g.stat("kernel")
+        wide_used = g.stat("wide")
         clocks = sampler.stop() if rank == 0 else None
         ms = max_over_ranks(ms, "cuda", world)
         value = world * cfg.n_pts * K / (ms * 1e-3) / 1e9
@@ -394,7 +398,7 @@ def main():
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfg.name, "grid": [cfg.n_r, cfg.n_theta], "modes": list(cfg.modes), "a": cfg.a,
-                       "dt": cfg.dt, "source": cfg.source, "source_kind": args.source_kind, "source_terms": args.source_terms, "coef_mode": args.coef_mode, "slab_rows": int(slab_rows), "kernel": int(kernel_used), "temporal_block": args.temporal_block or "default", "observers": list(cfg.observers),
+                       "dt": cfg.dt, "source": cfg.source, "source_kind": args.source_kind, "source_terms": args.source_terms, "coef_mode": args.coef_mode, "slab_rows": int(slab_rows), "kernel": int(kernel_used), "wide": int(wide_used), "temporal_block": args.temporal_block or "default", "observers": list(cfg.observers),
                        "state_mb": 4 * cfg.n_pts * 8 / 1e6, "parallelism": "replicas x%d" % world,
                        "extra_untimed_warmup": XW,
                        "l2": "inputs larger than L2 (two 537 MB state copies stream through a 126 MB L2)"
@@ -408,7 +412,8 @@ def main():
             "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
-                         "kernel": "teuk_step_resident_kernel" if kernel_used == 2 else "teuk_step_kernel", "bytes_per_pt_step": BYTES_PER_PT_STEP},
+                         "kernel": "teuk_step_resident_kernel" if kernel_used == 2 else ("teuk_step_wide_kernel" if wide_used else "teuk_step_kernel"),
+                         "bytes_per_pt_step": BYTES_PER_PT_STEP},
         }
         if K < 200:
             line["note"] = "burst (%d steps: the SM clock has not settled under the power cap; sustained figures need >= 1000 steps)" % K
