@@ -63,9 +63,49 @@ class Series:
         return np.concatenate(self.w) if self.w else np.empty((0, 1), dtype=complex)
 
 
+def print_tables(path):
+    """Markdown tables of the last record per (config, arm) in the jsonl file: final distances, the iteration count
+    up to which the 1e-10 bar holds, and the three pairs side by side."""
+    recs = {}
+    for line in open(path):
+        if line.strip():
+            d = json.loads(line)
+            recs[(d["config"], d["arm"], d["steps"])] = d
+
+    def fmt(v):
+        return v if isinstance(v, str) else "%.1e" % v
+
+    def wv(f):
+        ws = [w for w in f["waveforms"] if w != "silent"]
+        return fmt(max(ws)) if ws else "silent"
+
+    print("| config | iterations | pair | Phi | Pi | waveform (audible observers, worst) | 1e-10 holds up to iteration |")
+    print("|---|---|---|---|---|---|---|")
+    for key in sorted(recs):
+        d = recs[key]
+        for pair in ("gpu_vs_oracle", "gpu_vs_gpu2", "oracle_vs_oracle2"):
+            if pair in d:
+                f = d[pair]["final"]
+                full = "full length" if d["full_length"] else "%d of %d" % (d["steps"], wl.CONFIGS[d["config"]].steps)
+                hold = d[pair]["bar_holds_until"]
+                print("| %d | %d (%s) | %s | %s | %s | %s | %s |" % (
+                    d["config"], d["steps"], full, pair.replace("_", " "), fmt(f["rel_l2_phi"]), fmt(f["rel_l2_pi"]), wv(f),
+                    ("the end" if hold == d["steps"] else str(hold))))
+    print()
+    print("History (relative L2 of Pi, the most sensitive field, per checkpoint):")
+    print()
+    for key in sorted(recs):
+        d = recs[key]
+        for pair in ("gpu_vs_oracle", "gpu_vs_gpu2", "oracle_vs_oracle2"):
+            if pair in d:
+                print("- config %d, %s: " % (d["config"], pair.replace("_", " ")) +
+                      ", ".join("%d: %.1e" % (c["n"], c["rel_l2_pi"]) for c in d[pair]["history"]))
+
+
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--config", type=int, required=True)
+    ap.add_argument("--config", type=int, default=0)
+    ap.add_argument("--table", action="store_true", help="print BASELINE.md's parity tables (markdown) from the records in --out and exit")
     ap.add_argument("--steps", type=int, default=0)
     ap.add_argument("--arm", default="gpu", choices=["gpu", "oracle2"])
     ap.add_argument("--checkpoints", type=int, default=8)
@@ -73,6 +113,11 @@ def main():
     ap.add_argument("--no-oracle", action="store_true", help="--arm gpu without the oracle: gpu_vs_gpu2 only")
     ap.add_argument("--no-sensitivity", action="store_true", help="--arm gpu without the coef_mode 1 run")
     a = ap.parse_args()
+    if a.table:
+        print_tables(a.out)
+        return
+    if a.config not in wl.CONFIGS:
+        ap.error("--config 1..6 is required")
     cfg = wl.CONFIGS[a.config]
     steps = a.steps or cfg.steps
     ini = wl.initial_data(cfg)
