@@ -183,7 +183,7 @@ int n_segments(const teuk_solver* s) {
 const int kWideByDefault = 0;
 bool wide_active(const teuk_solver* s) {
   if (s->wide_opt == 0 || (s->wide_opt < 0 && !kWideByDefault)) return false;
-  return s->variant == 0 && s->coef_mode == 0 && s->temporal_block == 1 && s->n_terms == 0 && teuk_wide_applies(s->n_theta);
+  return s->variant == 0 && s->coef_mode == 0 && s->temporal_block == 1 && teuk_wide_applies(s->n_theta);
 }
 // slabs per row: theta segments of the one-warp-per-row kernel; the wide kernel marches whole rows
 int seg_factor(const teuk_solver* s) { return wide_active(s) ? 1 : n_segments(s); }

@@ -38,7 +38,8 @@ __device__ __forceinline__ void group_barrier(int id, int threads) {
 
 }  // namespace
 
-template <int NWR>
+// TERMS: the multi-term deposit of teuk_set_source_terms (a separate instantiation, as in teuk_step_kernel).
+template <int NWR, bool TERMS = false>
 __global__ void __launch_bounds__(32 * WideShape<NWR>::WARPS, WideShape<NWR>::BLOCKS)
 teuk_step_wide_kernel(const __grid_constant__ StepParams p) {
   constexpr int V = 2, GPB = WideShape<NWR>::GPB, WARPS = WideShape<NWR>::WARPS, NS = TEUK_SLOTS;
@@ -92,7 +93,7 @@ teuk_step_wide_kernel(const __grid_constant__ StepParams p) {
       th.vals.d0[v] = lane_ok ? tb[TT_D0 * nth + j0 + v] : 0.0;
     }
   }
-  StageSource<V> src_h, src_f;   // half stage: sample 2n at the half points; full stage: 2n+1 at the nodes
+  typename SourceSel<V, TERMS>::type src_h, src_f;   // half stage: sample 2n at the half points; full stage: 2n+1 at the nodes
   setup_source<V>(src_h, p, mode, 2 * n, true, r0 - 1, r1 - 1, lane, w * 64);
   setup_source<V>(src_f, p, mode, 2 * n + 1, false, r0, r1 - 1, lane, w * 64);
   bool do_tap = w == 0 && p.tap_enable && p.n_obs > 0 && n >= 1;     // warp 0 of the group taps the whole row
@@ -196,7 +197,7 @@ teuk_step_wide_kernel(const __grid_constant__ StepParams p) {
     rt_cur = rt_buf + (c & 1) * RT_CHUNK_DOUBLES;
     if (cb + RT_CH < r1)
       stage_rtab_chunk(rt_buf + ((c + 1) & 1) * RT_CHUNK_DOUBLES, rtab, 2 * (cb + RT_CH), 2 * nr - 1, lane);
-    if (any_src) {
+    if (!TERMS && any_src) {
       const bool hf = lane < 16;
       const int i = cb + (lane & 15);
       const bool on = hf ? src_h.on : src_f.on;
@@ -213,13 +214,15 @@ teuk_step_wide_kernel(const __grid_constant__ StepParams p) {
       for (int q = 0; q < p.n_obs; ++q)
         if (p.obs[q].i0 >= cb && p.obs[q].i0 < min(cb + RT_CH, r1)) tap_row(q);
   };
-  auto deposit = [&](Row<V>& o_, const StageSource<V>& s_, const double g) {
-    if (g != 0.0) {
+  auto deposit = [&](Row<V>& o_, const typename SourceSel<V, TERMS>::type& s_, const double g) {
+    if constexpr (!TERMS) {
+      if (g != 0.0) {
 #pragma unroll
-      for (int q = 0; q < V; ++q) {
-        const double gg = g * s_.gth[q];
-        o_.c[2][q] = fma(s_.are, gg, o_.c[2][q]);
-        o_.c[3][q] = fma(s_.aim, gg, o_.c[3][q]);
+        for (int q = 0; q < V; ++q) {
+          const double gg = g * s_.gth[q];
+          o_.c[2][q] = fma(s_.are, gg, o_.c[2][q]);
+          o_.c[3][q] = fma(s_.aim, gg, o_.c[3][q]);
+        }
       }
     }
   };
@@ -228,11 +231,17 @@ teuk_step_wide_kernel(const __grid_constant__ StepParams p) {
   auto march = [&](const int i, Row<V>& A, Row<V>& B, Row<V>& Hp, Row<V>& Hn) {
     const int o = (i - r0) & (RT_CH - 1);
     stage(std::true_type(), A, B, A, rt_cur + (2 * o + 1) * RT_N, tau_h, Hn);
-    if (any_src) deposit(Hn, src_h, __shfl_sync(FULL, gprof, o));
+    if (any_src) {
+      if constexpr (TERMS) add_source<V>(Hn, src_h, p, i, true);
+      else deposit(Hn, src_h, __shfl_sync(FULL, gprof, o));
+    }
     // every warp of the group is past the barrier of this half stage: slot (i + 1) % NS has been copied out by all
     if (w == 0 && lane == 0 && i + NS + 1 <= r1) issue_row(i + NS + 1);
     stage(std::false_type(), Hp, Hn, A, rt_cur + (2 * o) * RT_N, tau_f, out);
-    if (any_src) deposit(out, src_f, __shfl_sync(FULL, gprof, 16 + o));
+    if (any_src) {
+      if constexpr (TERMS) add_source<V>(out, src_f, p, i, false);
+      else deposit(out, src_f, __shfl_sync(FULL, gprof, 16 + o));
+    }
     store_row<V, true>(out, uout + (size_t)i * row_stride, nth, j0, 0, nth);
     if (i + 2 <= r1) {
       mbar_wait_u32(bars_u32 + 8u * (unsigned)((i + 2) % NS), (unsigned)((i - r0) / NS) & 1u);
@@ -284,7 +293,7 @@ teuk_step_wide_kernel(const __grid_constant__ StepParams p) {
 }
 
 // ---- host-side launcher (called from teuk_api.cu) ------------------------------------------------------------
-template <int NWR>
+template <int NWR, bool TERMS>
 static cudaError_t launch_wide(const StepParams& p, cudaStream_t st) {
   constexpr int GPB = WideShape<NWR>::GPB, WARPS = WideShape<NWR>::WARPS;
   dim3 grid((p.n_slabs + GPB - 1) / GPB, p.n_modes), block(32 * WARPS);
@@ -294,7 +303,7 @@ static cudaError_t launch_wide(const StepParams& p, cudaStream_t st) {
   int dev_ = 0;
   cudaGetDevice(&dev_);
   if (!attr_set[dev_ & 63]) {
-    cudaError_t e = cudaFuncSetAttribute(teuk_step_wide_kernel<NWR>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max);
+    cudaError_t e = cudaFuncSetAttribute(teuk_step_wide_kernel<NWR, TERMS>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_max);
     if (e != cudaSuccess) return e;
     attr_set[dev_ & 63] = true;
   }
@@ -305,15 +314,15 @@ static cudaError_t launch_wide(const StepParams& p, cudaStream_t st) {
     cudaLaunchConfig_t lc_ = {};
     lc_.gridDim = grid; lc_.blockDim = block; lc_.dynamicSmemBytes = dyn; lc_.stream = st;
     lc_.attrs = at_; lc_.numAttrs = 1;
-    cudaError_t e = cudaLaunchKernelEx(&lc_, teuk_step_wide_kernel<NWR>, p);
+    cudaError_t e = cudaLaunchKernelEx(&lc_, teuk_step_wide_kernel<NWR, TERMS>, p);
     if (e != cudaSuccess) return e;
   } else {
-    teuk_step_wide_kernel<NWR><<<grid, block, dyn, st>>>(p);
+    teuk_step_wide_kernel<NWR, TERMS><<<grid, block, dyn, st>>>(p);
   }
   return cudaGetLastError();
 }
 
-// n_theta even, 66 .. 320; coef_mode 0, single-term deposit (the caller checks: teuk_wide_applies).
+// n_theta even, 66 .. 320; coef_mode 0 (the caller checks: teuk_wide_applies).
 bool teuk_wide_applies(int n_theta) { return n_theta % 2 == 0 && n_theta > 64 && n_theta <= 320; }
 
 // slabs that are in flight at once on one SM (for the launch-shape measurement)
@@ -323,11 +332,12 @@ int teuk_wide_groups_per_sm(int n_theta) {
 }
 
 cudaError_t teuk_launch_step_wide(const StepParams& p, cudaStream_t st) {
+  const bool terms = p.n_terms > 0;
   switch ((p.n_theta + 63) / 64) {
-    case 2: return launch_wide<2>(p, st);
-    case 3: return launch_wide<3>(p, st);
-    case 4: return launch_wide<4>(p, st);
-    case 5: return launch_wide<5>(p, st);
+    case 2: return terms ? launch_wide<2, true>(p, st) : launch_wide<2, false>(p, st);
+    case 3: return terms ? launch_wide<3, true>(p, st) : launch_wide<3, false>(p, st);
+    case 4: return terms ? launch_wide<4, true>(p, st) : launch_wide<4, false>(p, st);
+    case 5: return terms ? launch_wide<5, true>(p, st) : launch_wide<5, false>(p, st);
     default: return cudaErrorInvalidValue;
   }
 }

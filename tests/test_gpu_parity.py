@@ -780,7 +780,17 @@ def test_wide_option_applicability(teuk):
     g.set_option("temporal_block", 1)
     g.set_source(wl.orbit_table(cfg, n_steps=4))
     g.set_source_terms([(1, 0, np.ones((cfg.n_modes, 9), dtype=complex))])
-    assert g.stat("wide") == 0
-    g.set_source_terms([])
-    assert g.stat("wide") == 1
+    assert g.stat("wide") == 1                       # the multi-term deposit has its own wide instantiation
     g.close()
+
+
+def test_wide_kernel_source_terms(orc, teuk):
+    """f2 on the paper's 304-column grid and on 128 columns through the group-of-warps kernel."""
+    for n_theta in (304, 128):
+        cfg = SMALL[3].scaled(name="wterms%d" % n_theta, n_r=151, n_theta=n_theta, dt_over_dx=0.002, steps=12)
+        terms = _random_terms(cfg, 2 * cfg.steps + 1, n_theta)
+        res = _run_terms(orc, teuk, cfg, cfg.steps, terms, 0, options={"kernel": 0, "wide": 1}, chunks=[1, 11])
+        check_pair(res)
+        base = _run_terms(orc, teuk, cfg, cfg.steps, terms, 0, options={"kernel": 0, "wide": 0})
+        for a, b in zip(base["sg"], res["sg"]):
+            assert np.array_equal(a, b), n_theta
