@@ -794,3 +794,13 @@ def test_wide_kernel_source_terms(orc, teuk):
         base = _run_terms(orc, teuk, cfg, cfg.steps, terms, 0, options={"kernel": 0, "wide": 0})
         for a, b in zip(base["sg"], res["sg"]):
             assert np.array_equal(a, b), n_theta
+
+
+def test_fp64_microbenchmark_is_plausible(teuk):
+    """teuk_measure_fp64 (the "alu" ceiling of bench.py): every instruction kind within a factor of the nominal
+    148 SMs x 64 lanes x 1.965 GHz = 1.86e13 lane-operations per second; bad arguments are refused."""
+    rates = [teuk.measure_fp64(k) for k in range(4)]
+    for r in rates:
+        assert 4e12 < r < 2.5e13, rates
+    with pytest.raises(teuk.TeukError):
+        teuk.measure_fp64(4)
