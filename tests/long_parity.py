@@ -110,6 +110,12 @@ def main():
     ap.add_argument("--arm", default="gpu", choices=["gpu", "oracle2"])
     ap.add_argument("--checkpoints", type=int, default=8)
     ap.add_argument("--out", default=os.path.join(ROOT, "profiles", "r2_long_parity.jsonl"))
+    ap.add_argument("--resume-dir", default=None, help="directory for the states between segments (see --segment)")
+    ap.add_argument("--segment", type=int, default=0)
+    ap.add_argument("--segments", type=int, default=1,
+                    help="--arm gpu only: run iterations [k S, (k+1) S), S = steps / segments, of the run in this call: every "
+                         "solver restarts from the state ITS OWN previous segment saved in --resume-dir, with a trajectory table "
+                         "that starts at t0 = k S dt (one call on the GPU box is limited to an hour; config 5 needs three)")
     ap.add_argument("--no-oracle", action="store_true", help="--arm gpu without the oracle: gpu_vs_gpu2 only")
     ap.add_argument("--no-sensitivity", action="store_true", help="--arm gpu without the coef_mode 1 run")
     a = ap.parse_args()
@@ -121,8 +127,17 @@ def main():
     cfg = wl.CONFIGS[a.config]
     steps = a.steps or cfg.steps
     ini = wl.initial_data(cfg)
-    orbit = wl.orbit_table(cfg, n_steps=steps)
     W = wl.observer_weights(cfg)
+    seg = None
+    if a.segments > 1:
+        assert a.arm == "gpu" and a.resume_dir and steps % a.segments == 0 and 0 <= a.segment < a.segments
+        S = steps // a.segments
+        seg = {"k": a.segment, "S": S, "dir": a.resume_dir, "first": a.segment * S}
+        os.makedirs(a.resume_dir, exist_ok=True)
+        orbit = wl.orbit_table(cfg, n_steps=S, t0=seg["first"] * cfg.dt)     # both sides get the same table
+        total_steps, steps = steps, S
+    else:
+        orbit = wl.orbit_table(cfg, n_steps=steps)
     ncp = max(1, min(a.checkpoints, steps))
     marks = sorted(set(round(steps * (k + 1) / ncp) for k in range(ncp)))
 
@@ -159,11 +174,18 @@ def main():
     else:
         from paper_1206_0270_b200 import Solver
 
+        def saved(name):
+            """state a solver saved at the end of the previous segment (its own: errors accumulate as in one run)"""
+            if seg is None or seg["k"] == 0:
+                return ini
+            z = np.load(os.path.join(seg["dir"], "%s_seg%d.npy" % (name, seg["k"] - 1)))
+            return [np.ascontiguousarray(z[c]) for c in range(4)]
+
         def make_gpu(coef_mode):
             g = Solver.from_config(cfg)
             if coef_mode:
                 g.set_option("coef_mode", 1)
-            g.set_initial(*ini)
+            g.set_initial(*saved("gpu2" if coef_mode else "gpu"))
             g.set_source(orbit)
             for x in cfg.observers:
                 g.add_observer(x, W)
@@ -173,8 +195,17 @@ def main():
         res["kernel"] = int(g.stat("kernel"))     # 2 = resident kernel (state on chip), 0 = marching kernel
         g2 = None if (a.no_sensitivity or cfg.n_theta > 128) else make_gpu(1)
         o = None if a.no_oracle else make_oracle()
+        if o is not None and seg is not None and seg["k"] > 0:
+            o.set_initial(*saved("oracle"))
         sg = [Series() for _ in cfg.observers]
         sg2 = [Series() for _ in cfg.observers]
+        so_prev = [np.empty((0, cfg.n_modes), dtype=complex) for _ in cfg.observers]   # oracle samples of earlier segments
+        hist_prev = {}
+        if seg is not None and seg["k"] > 0:
+            z = np.load(os.path.join(seg["dir"], "waves_seg%d.npz" % (seg["k"] - 1)))
+            for k in range(len(cfg.observers)):
+                sg[k].add(z["g%d" % k]); sg2[k].add(z["h%d" % k]); so_prev[k] = z["o%d" % k]
+            hist_prev = json.load(open(os.path.join(seg["dir"], "history_seg%d.json" % (seg["k"] - 1))))
         done = 0
         for mk in marks:
             g.sync()
@@ -194,19 +225,42 @@ def main():
                 sg[k].add(g.extract(x)[1])
                 if g2 is not None:
                     sg2[k].add(g2.extract(x)[1])
+            off = seg["first"] if seg is not None else 0
             if o is not None:
                 dphi, dpi, nphi, npi = state_distance(st, o.get_state())
-                waves = [wave_distance(sg[k].all(), o.waveform(k)[1]) for k in range(len(cfg.observers))]
+                waves = [wave_distance(sg[k].all(), np.concatenate([so_prev[k], o.waveform(k)[1]])) for k in range(len(cfg.observers))]
                 pairs.setdefault("gpu_vs_oracle", []).append(
-                    {"n": mk, "rel_l2_phi": dphi, "rel_l2_pi": dpi, "norm_phi": nphi, "norm_pi": npi, "waveforms": waves})
+                    {"n": mk + off, "rel_l2_phi": dphi, "rel_l2_pi": dpi, "norm_phi": nphi, "norm_pi": npi, "waveforms": waves})
                 print("n=%d gpu_vs_oracle phi %.2e pi %.2e w %s" % (mk, dphi, dpi, waves), flush=True)
             if g2 is not None:
                 dphi, dpi, nphi, npi = state_distance(g2.get_state(), st)
                 waves = [wave_distance(sg2[k].all(), sg[k].all()) for k in range(len(cfg.observers))]
                 pairs.setdefault("gpu_vs_gpu2", []).append(
-                    {"n": mk, "rel_l2_phi": dphi, "rel_l2_pi": dpi, "norm_phi": nphi, "norm_pi": npi, "waveforms": waves})
+                    {"n": mk + off, "rel_l2_phi": dphi, "rel_l2_pi": dpi, "norm_phi": nphi, "norm_pi": npi, "waveforms": waves})
                 print("n=%d gpu_vs_gpu2 phi %.2e pi %.2e w %s" % (mk, dphi, dpi, waves), flush=True)
         res["gpu_gpts"] = cfg.n_pts * steps / t_gpu / 1e9
+        if seg is not None:      # hand the states, series and histories to the next segment
+            for name, sol in (("gpu", g), ("gpu2", g2), ("oracle", o)):
+                if sol is not None:
+                    np.save(os.path.join(seg["dir"], "%s_seg%d.npy" % (name, seg["k"])), np.stack(sol.get_state()))
+            wz = {}
+            for k in range(len(cfg.observers)):
+                wz["g%d" % k] = sg[k].all(); wz["h%d" % k] = sg2[k].all() if g2 is not None else np.empty((0, cfg.n_modes), dtype=complex)
+                wz["o%d" % k] = np.concatenate([so_prev[k], o.waveform(k)[1]]) if o is not None else so_prev[k]
+            np.savez(os.path.join(seg["dir"], "waves_seg%d.npz" % seg["k"]), **wz)
+            for name in pairs:
+                pairs[name] = hist_prev.get(name, []) + pairs[name]
+            json.dump(pairs, open(os.path.join(seg["dir"], "history_seg%d.json" % seg["k"]), "w"))
+            for name in ("gpu", "gpu2", "oracle"):       # the previous segment's states are no longer needed
+                old = os.path.join(seg["dir"], "%s_seg%d.npy" % (name, seg["k"] - 1))
+                if os.path.exists(old):
+                    os.remove(old)
+            res["segments"] = {"count": a.segments, "done": seg["k"] + 1, "iterations_each": seg["S"],
+                               "note": "one call on the GPU box is limited to an hour: the run is cut into segments; every solver "
+                                       "restarts from the state its own previous segment saved, with a trajectory table starting at t0"}
+            res["steps"] = seg["first"] + seg["S"]
+            res["full_length"] = res["steps"] == total_steps
+            res["checkpoints"] = [c["n"] for c in pairs.get("gpu_vs_oracle", pairs.get("gpu_vs_gpu2", []))]
         g.close()
         if g2 is not None:
             g2.close()
