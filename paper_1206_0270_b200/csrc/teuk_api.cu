@@ -180,9 +180,11 @@ int n_segments(const teuk_solver* s) {
 
 // The wide kernel (teuk_wide.cu: a group of ceil(n_theta / 64) warps per row, V = 2 columns per lane) replaces the
 // one-warp-per-row kernel and the theta segments when it applies and is asked for (or chosen by default).
-const int kWideByDefault = 0;
+// Automatic choice (measured, profiles/r2_bench.md): for n_theta <= 128 one warp per row with V = 4 is faster (config 5:
+// 86.5 vs 81.0 GPts/s: the group kernel issues 833 instead of 535 instructions per row and pays two barriers);
+// for wider rows the group kernel beats the theta segments with their recomputed halo columns (32000 x 304: 68.0 vs 65.1).
 bool wide_active(const teuk_solver* s) {
-  if (s->wide_opt == 0 || (s->wide_opt < 0 && !kWideByDefault)) return false;
+  if (s->wide_opt == 0 || (s->wide_opt < 0 && s->n_theta <= 128)) return false;
   return s->variant == 0 && s->coef_mode == 0 && s->temporal_block == 1 && teuk_wide_applies(s->n_theta);
 }
 // slabs per row: theta segments of the one-warp-per-row kernel; the wide kernel marches whole rows
@@ -719,11 +721,14 @@ int tune_slab_rows(teuk_solver* s, int tb) {
     p.tap_enable2 = 0;
     p.has_source = 0;      // trial launches read nothing but the state and the tables (no trajectory sample, no observer)
     p.n_obs = 0;
+    // launched like iterations 2..32 of a graph batch (programmatic dependent launch), so that what is timed is
+    // the back-to-back rate of production and not the gap between two plain launches
+    p.pdl = (tb == 1 && s->use_pdl && s->variant == 0 && seg_factor(s) == 1) ? 1 : 0;
     auto launch = [&]() { return tb == 2 ? teuk_launch_step_tb2(p, s->stream) : launch_step_any(s, p, s->stream); };
     cudaError_t e = launch();                                      // warm-up
     float ms = 0.f;
     int reps = 3;
-    for (int pass = 0; pass < 3 && e == cudaSuccess; ++pass) {   // short kernels: time at least ~0.3 ms of launches
+    for (int pass = 0; pass < 3 && e == cudaSuccess; ++pass) {   // short kernels: time at least ~1 ms of launches
       e = cudaEventRecord(e0, s->stream);
       for (int r = 0; r < reps && e == cudaSuccess; ++r) e = launch();
       if (e == cudaSuccess) e = cudaEventRecord(e1, s->stream);
@@ -732,8 +737,18 @@ int tune_slab_rows(teuk_solver* s, int tb) {
       s->launches += reps;
       const float total = ms;
       ms /= reps;
-      if (total > 0.3f) break;
+      if (total > 1.0f || pass == 2) break;
       reps *= 8;
+    }
+    if (e == cudaSuccess) {   // once more at the final repetition count: the smaller of the two (clock ramps, stragglers)
+      float ms2 = 0.f;
+      e = cudaEventRecord(e0, s->stream);
+      for (int r = 0; r < reps && e == cudaSuccess; ++r) e = launch();
+      if (e == cudaSuccess) e = cudaEventRecord(e1, s->stream);
+      if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+      if (e == cudaSuccess) e = cudaEventElapsedTime(&ms2, e0, e1);
+      s->launches += reps;
+      if (e == cudaSuccess && ms2 / reps < ms) ms = ms2 / reps;
     }
     s->launches += 1;
     if (e != cudaSuccess) {

@@ -132,8 +132,10 @@ __device__ __forceinline__ uint4* ll_slot(const StepParams& p, int mode, int nct
 // fewer (blockDim.x / 32 = min(NW, rows + 1)).
 // CC: the time-independent coefficients b2d, Q, Re beta^' of every location of the block are kept in shared memory
 // (3 doubles per point and location) when there is room; else they are rebuilt in every stage as in kernel 0.
-// TERMS: multi-term deposit of teuk_set_source_terms (a separate instantiation: the default kernel is unchanged)
-template <int V, int NW, bool CC, bool TERMS = false>
+// SRC: 0 = source-free (no deposit code in the task loop at all: the loop is 47 KB of instructions with it, and on
+// the source-free configs 1 and 2 its mere presence cost 8 % and 2 %), 1 = the single-term deposit, 2 = the
+// multi-term deposit of teuk_set_source_terms.  Separate instantiations chosen by the launcher.
+template <int V, int NW, bool CC, int SRC = 1>
 __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __grid_constant__ StepParams p) {
   constexpr int NP = 32 * V;        // padded row width in shared memory (columns >= n_theta stay zero)
   constexpr int ROWD = 4 * NP;      // doubles per row
@@ -248,7 +250,8 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
   // Measured on config 2 (28 rows per block, 16 warps): two __syncthreads per iteration 4.08 us per iteration,
   // this task list 3.63 us; a fixed chunk of rows per warp (no rotation, two hand-overs per warp) 4.6 us: what
   // counts is the length of the serial chain of tasks per warp, see DESIGN.md 5.1d.
-  const bool has_source = p.has_source != 0;
+  constexpr bool TERMS = SRC == 2;
+  const bool has_source = SRC != 0 && p.has_source != 0;
   const double src_reach = ((double)p.W + 2.0) * p.dx;   // conservative pre-test of the source window in x
   const int T = 2 * rows + 1;
   int it = 0, t = w;
@@ -267,12 +270,32 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
       else lds_row_s<V>(A, uU + (unsigned)h * ROWB);
       if (h == rows && !last && it > 0) ll_receive<V>(ll_slot<V>(p, mode, ncta, cta + 1, 0, tag_in), B, tag_in, lane);
       else lds_row_s<V>(B, uU + (unsigned)(h + 1) * ROWB);
-      if (cta_taps && n >= 1 && (it > 0 || p.tap_enable)) tap<V>(A, B, p, i, mode, n, lane);
+      // Tap of the cell that starts at row i: this lane's part now (it needs A and B), the warp reduction and the
+      // ring store AFTER the row has been handed over, off the critical path of the tasks that wait for it (the
+      // block that holds an observer sets the pace of all the others through the neighbour exchange).  Further
+      // observers in the same cell (rare) are finished on the spot.
+      int tap_q = -1;
+      double tap_wr = 0.0, tap_wi = 0.0;
+      if (cta_taps && n >= 1 && (it > 0 || p.tap_enable)) {
+        for (int q = 0; q < p.n_obs; ++q) {
+          if (p.obs[q].i0 != i) continue;
+          double wr, wi;
+          tap_partial<V>(A, B, p, q, lane, wr, wi);
+          if (tap_q < 0) {
+            tap_q = q;
+            tap_wr = wr;
+            tap_wi = wi;
+          } else {
+            tap_finish(p, q, mode, n, lane, wr, wi);
+          }
+        }
+      }
       stage(std::true_type(), A, B, A, 2 * h, tau_h, Hn);
       if (has_source) {
         const double x = p.rs_min + ((double)i + 0.5) * p.dx;
         if (fabs(x - __ldg(p.xp + 2 * n)) <= src_reach) {
           typename SourceSel<V, TERMS>::type s;
+          if constexpr (TERMS) s.tab = nullptr;   // one task = one row: profiles built on the spot
           setup_source<V>(s, p, mode, 2 * n, true, i, i, lane, 0);
           add_source<V>(Hn, s, p, i, true);
         }
@@ -301,6 +324,7 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
       }
       __syncwarp();
       if (lane == 0) flag_set(verH + 4u * (unsigned)h, it + 1);
+      if (tap_q >= 0) tap_finish(p, tap_q, mode, n, lane, tap_wr, tap_wi);
     } else {
       // ---- full-step row in place (Eq. 4) ----
       const int tt = t - (rows + 1);
@@ -321,6 +345,7 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
         const double x = p.rs_min + (double)i * p.dx;
         if (fabs(x - __ldg(p.xp + 2 * n + 1)) <= src_reach) {
           typename SourceSel<V, TERMS>::type s;
+          if constexpr (TERMS) s.tab = nullptr;   // one task = one row: profiles built on the spot
           setup_source<V>(s, p, mode, 2 * n + 1, false, i, i, lane, 0);
           add_source<V>(out, s, p, i, false);
         }
@@ -381,7 +406,7 @@ size_t teuk_resident_ll_bytes(int n_theta, int n_modes, int ncta) {
   return (size_t)n_modes * ncta * 4 * (4 * 32 * V) * 16;
 }
 
-template <int V, bool CC, bool TERMS = false>
+template <int V, bool CC, int SRC>
 static cudaError_t launch_resident_v(const StepParams& p, int ncta, cudaStream_t st) {
   constexpr int NW = resident_max_warps<V>();
   const size_t dyn = teuk_resident_smem_bytes(p.n_theta, p.res_rows, CC ? 1 : 0);
@@ -392,7 +417,7 @@ static cudaError_t launch_resident_v(const StepParams& p, int ncta, cudaStream_t
     int optin = 0;
     cudaError_t e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev_);
     if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(teuk_step_resident_kernel<V, NW, CC, TERMS>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+      e = cudaFuncSetAttribute(teuk_step_resident_kernel<V, NW, CC, SRC>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
     if (e != cudaSuccess) return e;
     attr_set[dev_ & 63] = true;
   }
@@ -400,25 +425,31 @@ static cudaError_t launch_resident_v(const StepParams& p, int ncta, cudaStream_t
   dim3 grid(ncta, p.n_modes), block(32 * nwarps);
   StepParams pc = p;
   void* args[] = {&pc};
-  return cudaLaunchCooperativeKernel((const void*)teuk_step_resident_kernel<V, NW, CC, TERMS>, grid, block, args, dyn, st);
+  return cudaLaunchCooperativeKernel((const void*)teuk_step_resident_kernel<V, NW, CC, SRC>, grid, block, args, dyn, st);
 }
 
 // n_iter iterations in one cooperative launch; the caller sized res_rows / ncta so that the state fits.
 cudaError_t teuk_launch_step_resident(const StepParams& p, int ncta, cudaStream_t st) {
   const int v = (p.n_theta + 31) / 32;
-  if (p.n_terms > 0) {              // multi-term deposit (the host passes res_cache = 0 with it)
-    if (v <= 1) return launch_resident_v<1, false, true>(p, ncta, st);
-    if (v <= 2) return launch_resident_v<2, false, true>(p, ncta, st);
-    return launch_resident_v<4, false, true>(p, ncta, st);
+  if (p.has_source && p.n_terms > 0) {   // multi-term deposit (the host passes res_cache = 0 with it)
+    if (v <= 1) return launch_resident_v<1, false, 2>(p, ncta, st);
+    if (v <= 2) return launch_resident_v<2, false, 2>(p, ncta, st);
+    return launch_resident_v<4, false, 2>(p, ncta, st);
   }
-  if (p.res_cache) {
-    if (v <= 1) return launch_resident_v<1, true>(p, ncta, st);
-    if (v <= 2) return launch_resident_v<2, true>(p, ncta, st);
-    return launch_resident_v<4, true>(p, ncta, st);
-  }
-  if (v <= 1) return launch_resident_v<1, false>(p, ncta, st);
-  if (v <= 2) return launch_resident_v<2, false>(p, ncta, st);
-  return launch_resident_v<4, false>(p, ncta, st);
+#define TEUK_RES_DISPATCH(SRCV)                                             \
+  do {                                                                      \
+    if (p.res_cache) {                                                      \
+      if (v <= 1) return launch_resident_v<1, true, SRCV>(p, ncta, st);     \
+      if (v <= 2) return launch_resident_v<2, true, SRCV>(p, ncta, st);     \
+      return launch_resident_v<4, true, SRCV>(p, ncta, st);                 \
+    }                                                                       \
+    if (v <= 1) return launch_resident_v<1, false, SRCV>(p, ncta, st);      \
+    if (v <= 2) return launch_resident_v<2, false, SRCV>(p, ncta, st);      \
+    return launch_resident_v<4, false, SRCV>(p, ncta, st);                  \
+  } while (0)
+  if (p.has_source) TEUK_RES_DISPATCH(1);
+  TEUK_RES_DISPATCH(0);
+#undef TEUK_RES_DISPATCH
 }
 
 

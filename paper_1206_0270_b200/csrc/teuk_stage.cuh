@@ -565,14 +565,19 @@ __device__ __forceinline__ double pick3(const Profile3& r, int order) {
   return order == 0 ? r.d[0] : (order == 1 ? r.d[1] : r.d[2]);
 }
 
-// Window bookkeeping of one stage for the multi-term deposit: scalars only; the theta profiles are rebuilt on the
-// few rows a window touches, so nothing per column stays live across a marching loop.
+// Window bookkeeping of one stage for the multi-term deposit.  The theta profiles (three derivative orders per
+// column) do not depend on the row: a marching kernel gives every warp a table in shared memory (`tab`,
+// [3][V][32] doubles, this lane's entries at [(k V + q) 32 + lane]) that setup_source fills once per stage, so a row
+// of the window costs one radial profile and a short loop over the terms (round 2, first version: the profiles were
+// rebuilt per row and column, exp and divisions included, and the one warp whose slab meets the window made the
+// whole launch 3.5 times longer).  tab = nullptr (the resident kernel: one task = one row): built on the spot.
 template <int V>
 struct TermSource {
   bool on;
   int ip, jp, mode, lane, col0;
   long long ks;
   double xp, thp;
+  double* tab;
 };
 
 template <int V, int MAP = 0>
@@ -594,6 +599,17 @@ __device__ __forceinline__ void setup_source(TermSource<V>& s, const StepParams&
   s.ks = ks;
   s.xp = xp;
   s.thp = thp;
+  if (s.tab) {
+    for (int q = 0; q < V; ++q) {
+      const int j = col0 + lane * V + q;                             // lane <-> column mapping MAP 0
+      Profile3 pt;
+      pt.d[0] = pt.d[1] = pt.d[2] = 0.0;
+      if ((unsigned)j < (unsigned)p.n_theta && abs(j - jp) <= p.W)
+        pt = deposit_profile3(p.source_kind, __dmul_rn((double)j + 0.5, p.dth) - thp, p.sigma_th);
+#pragma unroll
+      for (int k = 0; k < 3; ++k) s.tab[(k * V + q) * 32 + lane] = pt.d[k];
+    }
+  }
 }
 
 template <int V>
@@ -603,23 +619,35 @@ __device__ __forceinline__ void add_source(Row<V>& out, const TermSource<V>& s, 
   double x = __dadd_rn(p.rs_min, __dmul_rn((double)i, p.dx));
   if (half) x = __dadd_rn(x, __dmul_rn(0.5, p.dx));
   const Profile3 pr = deposit_profile3(p.source_kind, x - s.xp, p.sigma_r);
+  Profile3 pt[V];
+  if (!s.tab) {
 #pragma unroll
-  for (int q = 0; q < V; ++q) {
-    const int j = s.col0 + s.lane * V + q;                           // lane <-> column mapping MAP 0
-    if ((unsigned)j >= (unsigned)p.n_theta || abs(j - s.jp) > p.W) continue;
-    const double th = __dmul_rn((double)j + 0.5, p.dth);
-    const Profile3 pt = deposit_profile3(p.source_kind, th - s.thp, p.sigma_th);
-    double accr = 0.0, acci = 0.0;
-    for (int t = 0; t < p.n_terms; ++t) {
-      const size_t ia = ((size_t)t * p.n_modes + s.mode) * p.n_samples + s.ks;
-      const double gg = (p.dt * pick3(pr, p.term_or[t])) * pick3(pt, p.term_oth[t]);
-      accr = fma(p.amp_re[ia], gg, accr);
-      acci = fma(p.amp_im[ia], gg, acci);
+    for (int q = 0; q < V; ++q) {
+      const int j = s.col0 + s.lane * V + q;
+      pt[q].d[0] = pt[q].d[1] = pt[q].d[2] = 0.0;
+      if ((unsigned)j < (unsigned)p.n_theta && abs(j - s.jp) <= p.W)
+        pt[q] = deposit_profile3(p.source_kind, __dmul_rn((double)j + 0.5, p.dth) - s.thp, p.sigma_th);
     }
-    out.c[2][q] += accr;
-    out.c[3][q] += acci;
+  }
+  for (int t = 0; t < p.n_terms; ++t) {
+    const size_t ia = ((size_t)t * p.n_modes + s.mode) * p.n_samples + s.ks;
+    const double are = p.amp_re[ia], aim = p.amp_im[ia];
+    const double gr = p.dt * pick3(pr, p.term_or[t]);
+    const int kth = p.term_oth[t];
+#pragma unroll
+    for (int q = 0; q < V; ++q) {
+      const double gg = gr * (s.tab ? s.tab[(kth * V + q) * 32 + s.lane] : pick3(pt[q], kth));
+      out.c[2][q] = fma(are, gg, out.c[2][q]);
+      out.c[3][q] = fma(aim, gg, out.c[3][q]);
+    }
   }
 }
+
+// Shared-memory doubles of one warp's theta-profile tables (two stages) in a TERMS instantiation of a marching kernel
+template <int V>
+struct TermTab {
+  static constexpr int PER_STAGE = 3 * V * 32;
+};
 
 // StageSource (one term, the profile itself: the configs' deposit) or TermSource (teuk_set_source_terms)
 template <int V, bool TERMS>
@@ -631,33 +659,47 @@ struct SourceSel<V, true> {
   typedef TermSource<V> type;
 };
 
-// Waveform tap of the INPUT state (sample n): w = sum_j W_j [(1-f) Phi_{i0,j} + f Phi_{i0+1,j}].
+// Waveform tap of the INPUT state (sample n): w = sum_j W_j [(1-f) Phi_{i0,j} + f Phi_{i0+1,j}], in two pieces:
+// tap_partial = this lane's columns (cheap, needs the rows), tap_finish = the warp reduction and the ring store
+// (latency: ten shuffles and a global store; needs two doubles).  A kernel whose tasks sit on a critical path
+// (teuk_resident.cu) runs tap_finish after it has handed its row over.  tap = both, for every observer of cell i.
+template <int V, int MAP = 0>
+__device__ __forceinline__ void tap_partial(const Row<V>& lo, const Row<V>& hi, const StepParams& p, int q, int lane,
+                                            double& wr, double& wi) {
+  const double f = p.obs[q].f;
+  wr = 0.0;
+  wi = 0.0;
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    const int j = col_of<V, MAP>(lane, v);
+    const double wt = (j < p.n_theta) ? __ldg(p.obs[q].weights + j) : 0.0;
+    wr = fma(wt, fma(f, hi.c[0][v], (1.0 - f) * lo.c[0][v]), wr);
+    wi = fma(wt, fma(f, hi.c[1][v], (1.0 - f) * lo.c[1][v]), wi);
+  }
+}
+__device__ __forceinline__ void tap_finish(const StepParams& p, int q, int mode, long long n, int lane, double wr,
+                                           double wi) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    wr += __shfl_xor_sync(FULL, wr, o);
+    wi += __shfl_xor_sync(FULL, wi, o);
+  }
+  if (lane == 0) {
+    const long long slot = (n - 1) % p.ring_cap;
+    double* dst = p.obs[q].ring + ((size_t)slot * p.n_modes + mode) * 2;
+    dst[0] = wr;
+    dst[1] = wi;
+    if (!isfinite(wr) || !isfinite(wi)) *p.nonfinite = 1;
+  }
+}
 template <int V, int MAP = 0>
 __device__ __forceinline__ void tap(const Row<V>& lo, const Row<V>& hi, const StepParams& p, int i, int mode,
                                     long long n, int lane) {
   for (int q = 0; q < p.n_obs; ++q) {
     if (p.obs[q].i0 != i) continue;
-    const double f = p.obs[q].f;
-    double wr = 0.0, wi = 0.0;
-#pragma unroll
-    for (int v = 0; v < V; ++v) {
-      const int j = col_of<V, MAP>(lane, v);
-      const double wt = (j < p.n_theta) ? __ldg(p.obs[q].weights + j) : 0.0;
-      wr = fma(wt, fma(f, hi.c[0][v], (1.0 - f) * lo.c[0][v]), wr);
-      wi = fma(wt, fma(f, hi.c[1][v], (1.0 - f) * lo.c[1][v]), wi);
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      wr += __shfl_xor_sync(FULL, wr, o);
-      wi += __shfl_xor_sync(FULL, wi, o);
-    }
-    if (lane == 0) {
-      const long long slot = (n - 1) % p.ring_cap;
-      double* dst = p.obs[q].ring + ((size_t)slot * p.n_modes + mode) * 2;
-      dst[0] = wr;
-      dst[1] = wi;
-      if (!isfinite(wr) || !isfinite(wi)) *p.nonfinite = 1;
-    }
+    double wr, wi;
+    tap_partial<V, MAP>(lo, hi, p, q, lane, wr, wi);
+    tap_finish(p, q, mode, n, lane, wr, wi);
   }
 }
 

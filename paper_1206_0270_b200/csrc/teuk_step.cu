@@ -132,6 +132,11 @@ __global__ void __launch_bounds__(128, (V == 2 ? TEUK_V2_BLOCKS : TEUK_MIN_BLOCK
     }
   }
   typename SourceSel<V, TERMS>::type src_h, src_f;   // half stage: sample 2n at half points; full stage: 2n+1 at nodes
+  __shared__ double s_tp[TERMS ? 4 * 2 * TermTab<V>::PER_STAGE : 1];   // theta-profile tables of the multi-term deposit
+  if constexpr (TERMS) {
+    src_h.tab = &s_tp[(wib_u * 2 + 0) * TermTab<V>::PER_STAGE];
+    src_f.tab = &s_tp[(wib_u * 2 + 1) * TermTab<V>::PER_STAGE];
+  }
   setup_source<V>(src_h, p, mode, 2 * n, true, r0 - 1, r1 - 1, lane, c_lo);
   setup_source<V>(src_f, p, mode, 2 * n + 1, false, r0, r1 - 1, lane, c_lo);
   bool do_tap = !SEG && p.tap_enable && p.n_obs > 0 && n >= 1;   // segments: separate tap kernel

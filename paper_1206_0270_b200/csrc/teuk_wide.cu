@@ -94,6 +94,11 @@ teuk_step_wide_kernel(const __grid_constant__ StepParams p) {
     }
   }
   typename SourceSel<V, TERMS>::type src_h, src_f;   // half stage: sample 2n at the half points; full stage: 2n+1 at the nodes
+  __shared__ double s_tp[TERMS ? WARPS * 2 * TermTab<V>::PER_STAGE : 1];   // theta-profile tables of the multi-term deposit
+  if constexpr (TERMS) {
+    src_h.tab = &s_tp[(wib * 2 + 0) * TermTab<V>::PER_STAGE];
+    src_f.tab = &s_tp[(wib * 2 + 1) * TermTab<V>::PER_STAGE];
+  }
   setup_source<V>(src_h, p, mode, 2 * n, true, r0 - 1, r1 - 1, lane, w * 64);
   setup_source<V>(src_f, p, mode, 2 * n + 1, false, r0, r1 - 1, lane, w * 64);
   bool do_tap = w == 0 && p.tap_enable && p.n_obs > 0 && n >= 1;     // warp 0 of the group taps the whole row
