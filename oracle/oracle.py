@@ -11,6 +11,10 @@ import subprocess
 
 import numpy as np
 
+# idle OpenMP threads sleep instead of spinning: on an oversubscribed host (another job on the cores) spinning
+# barriers make the row loops of the oracle many times slower
+os.environ.setdefault("OMP_WAIT_POLICY", "passive")
+
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "teuk_oracle.cpp")
 _LIB = os.path.join(_HERE, "liboracle.so")
