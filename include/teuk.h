@@ -205,7 +205,9 @@ int teuk_get_state(teuk_solver *s, double *phi_re, double *phi_im, double *pi_re
  *                   1 = a GROUP of ceil(n_theta / 64) warps per row, V = 2 columns per lane, the boundary columns of
  *                   the theta stencil exchanged through shared memory (needs an even n_theta between 66 and 320,
  *                   coef_mode 0, temporal_block 1; otherwise the setting is ignored);
- *                   -1 (default) = automatic.  Same results bit for bit.
+ *                   -1 (default) = automatic: 1 for rows wider than 128 columns when it applies (measured faster than
+ *                   theta segments), 0 otherwise (for n_theta <= 128 one warp per row is faster).  Same results
+ *                   bit for bit.
  *   "pdl"           1 (default) = inside a CUDA-graph batch, iteration k + 1 of kernel 0 is launched as a programmatic
  *                   dependent of iteration k (its prologue overlaps k's tail); 0 = fully serialised launches
  *   "resident_cache" 1 (default) = kernel 2 also keeps the time-independent coefficients b, b^2 and Re beta' of its
