@@ -21,10 +21,14 @@
 // tests/test_oracle_pins.py against a computer-algebra substitution into Eq. (1) (pin P1),
 // by second-order self-convergence (P2), by the Schwarzschild and Kerr l=m=2 quasinormal
 // frequencies (P3, P3b), by the (m, theta) reflection invariant (P4), a = 0 realness (P5),
-// linearity (P6), the unit norm of the deposit (P7), the edge rows' closed forms (P8) and, for the
-// discrete-delta deposits, the paper's step-function construction in exact rationals and the moment /
-// interpolation conditions (P9).  The paper prints no field values:
-// beyond those pins the numbers this file produces are "parity unpinned" by the paper.
+// linearity (P6), the unit norm of the deposit (P7), the edge rows' closed forms (P8), for the
+// discrete-delta deposits the paper's step-function construction in exact rationals and the moment /
+// interpolation conditions (P9), the waveform tap with an off-node observer against the interpolated weighted sum of
+// the state and a closed form on a field linear in x (P10), and the derivative profiles of the multi-term deposit
+// against exact-rational Lagrange derivatives, moment conditions and mpmath derivatives of the printed Gaussian
+// (P12).  (P11 pins the shared input generator, paper_1206_0270_b200/workloads.py.)  The paper prints no field
+// values: beyond those pins the numbers this file produces are "parity unpinned" by the paper; no function of this
+// file is without a pin of its own.
 //
 // Readings of silent/ambiguous passages are the A1-A12 of SURVEY.md 8(c), restated in DESIGN.md.
 
