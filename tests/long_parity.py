@@ -113,7 +113,7 @@ def main():
     ap.add_argument("--resume-dir", default=None, help="directory for the states between segments (see --segment)")
     ap.add_argument("--segment", type=int, default=0)
     ap.add_argument("--segments", type=int, default=1,
-                    help="--arm gpu only: run iterations [k S, (k+1) S), S = steps / segments, of the run in this call: every "
+                    help="run iterations [k S, (k+1) S), S = steps / segments, of the run in this call: every "
                          "solver restarts from the state ITS OWN previous segment saved in --resume-dir, with a trajectory table "
                          "that starts at t0 = k S dt (one call on the GPU box is limited to an hour; config 5 needs three)")
     ap.add_argument("--no-oracle", action="store_true", help="--arm gpu without the oracle: gpu_vs_gpu2 only")
@@ -130,7 +130,7 @@ def main():
     W = wl.observer_weights(cfg)
     seg = None
     if a.segments > 1:
-        assert a.arm == "gpu" and a.resume_dir and steps % a.segments == 0 and 0 <= a.segment < a.segments
+        assert a.resume_dir and steps % a.segments == 0 and 0 <= a.segment < a.segments
         S = steps // a.segments
         seg = {"k": a.segment, "S": S, "dir": a.resume_dir, "first": a.segment * S}
         os.makedirs(a.resume_dir, exist_ok=True)
@@ -156,6 +156,16 @@ def main():
     t_cpu = t_gpu = 0.0
     if a.arm == "oracle2":
         o1, o2 = make_oracle(), make_oracle(orc.lib_fma())
+        w_prev = [[np.empty((0, cfg.n_modes), dtype=complex)] * 2 for _ in cfg.observers]
+        hist_prev = {}
+        if seg is not None and seg["k"] > 0:
+            for name, oo in (("o1", o1), ("o2", o2)):
+                z = np.load(os.path.join(seg["dir"], "%s_seg%d.npy" % (name, seg["k"] - 1)))
+                oo.set_initial(*[np.ascontiguousarray(z[c]) for c in range(4)])
+            z = np.load(os.path.join(seg["dir"], "owaves_seg%d.npz" % (seg["k"] - 1)))
+            w_prev = [[z["a%d" % k], z["b%d" % k]] for k in range(len(cfg.observers))]
+            hist_prev = json.load(open(os.path.join(seg["dir"], "ohistory_seg%d.json" % (seg["k"] - 1))))
+        off = seg["first"] if seg is not None else 0
         done = 0
         for mk in marks:
             t0 = time.perf_counter()
@@ -164,11 +174,30 @@ def main():
             o2.step(mk - done)
             done = mk
             dphi, dpi, nphi, npi = state_distance(o2.get_state(), o1.get_state())
-            waves = [wave_distance(o2.waveform(k)[1], o1.waveform(k)[1]) for k in range(len(cfg.observers))]
+            waves = [wave_distance(np.concatenate([w_prev[k][1], o2.waveform(k)[1]]),
+                                   np.concatenate([w_prev[k][0], o1.waveform(k)[1]])) for k in range(len(cfg.observers))]
             pairs.setdefault("oracle_vs_oracle2", []).append(
-                {"n": mk, "rel_l2_phi": dphi, "rel_l2_pi": dpi, "norm_phi": nphi, "norm_pi": npi, "waveforms": waves})
+                {"n": mk + off, "rel_l2_phi": dphi, "rel_l2_pi": dpi, "norm_phi": nphi, "norm_pi": npi, "waveforms": waves})
             print("n=%d oracle_vs_oracle2 phi %.2e pi %.2e w %s" % (mk, dphi, dpi, waves), flush=True)
         res["oracle2_build"] = " ".join(orc.CXXFLAGS_FMA)
+        if seg is not None:
+            for name, oo in (("o1", o1), ("o2", o2)):
+                np.save(os.path.join(seg["dir"], "%s_seg%d.npy" % (name, seg["k"])), np.stack(oo.get_state()))
+                old = os.path.join(seg["dir"], "%s_seg%d.npy" % (name, seg["k"] - 1))
+                if os.path.exists(old):
+                    os.remove(old)
+            wz = {}
+            for k in range(len(cfg.observers)):
+                wz["a%d" % k] = np.concatenate([w_prev[k][0], o1.waveform(k)[1]])
+                wz["b%d" % k] = np.concatenate([w_prev[k][1], o2.waveform(k)[1]])
+            np.savez(os.path.join(seg["dir"], "owaves_seg%d.npz" % seg["k"]), **wz)
+            pairs["oracle_vs_oracle2"] = hist_prev.get("oracle_vs_oracle2", []) + pairs["oracle_vs_oracle2"]
+            json.dump(pairs, open(os.path.join(seg["dir"], "ohistory_seg%d.json" % seg["k"]), "w"))
+            res["segments"] = {"count": a.segments, "done": seg["k"] + 1, "iterations_each": seg["S"],
+                               "note": "run cut into segments; each oracle build restarts from the state its own previous segment saved"}
+            res["steps"] = seg["first"] + seg["S"]
+            res["full_length"] = res["steps"] == total_steps
+            res["checkpoints"] = [c["n"] for c in pairs["oracle_vs_oracle2"]]
         o1.close()
         o2.close()
     else:
