@@ -270,26 +270,10 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
       else lds_row_s<V>(A, uU + (unsigned)h * ROWB);
       if (h == rows && !last && it > 0) ll_receive<V>(ll_slot<V>(p, mode, ncta, cta + 1, 0, tag_in), B, tag_in, lane);
       else lds_row_s<V>(B, uU + (unsigned)(h + 1) * ROWB);
-      // Tap of the cell that starts at row i: this lane's part now (it needs A and B), the warp reduction and the
-      // ring store AFTER the row has been handed over, off the critical path of the tasks that wait for it (the
-      // block that holds an observer sets the pace of all the others through the neighbour exchange).  Further
-      // observers in the same cell (rare) are finished on the spot.
-      int tap_q = -1;
-      double tap_wr = 0.0, tap_wi = 0.0;
-      if (cta_taps && n >= 1 && (it > 0 || p.tap_enable)) {
-        for (int q = 0; q < p.n_obs; ++q) {
-          if (p.obs[q].i0 != i) continue;
-          double wr, wi;
-          tap_partial<V>(A, B, p, q, lane, wr, wi);
-          if (tap_q < 0) {
-            tap_q = q;
-            tap_wr = wr;
-            tap_wi = wi;
-          } else {
-            tap_finish(p, q, mode, n, lane, wr, wi);
-          }
-        }
-      }
+      // (Tried in round 2: the tap's warp reduction and ring store deferred until after the row has been handed over.
+      // The two doubles it keeps across the stage push the V = 2 kernel to its 128-register cap: config 2 79 -> 69
+      // GPts/s, config 1 12.5 -> 13.0.  Not kept.)
+      if (cta_taps && n >= 1 && (it > 0 || p.tap_enable)) tap<V>(A, B, p, i, mode, n, lane);
       stage(std::true_type(), A, B, A, 2 * h, tau_h, Hn);
       if (has_source) {
         const double x = p.rs_min + ((double)i + 0.5) * p.dx;
@@ -324,7 +308,6 @@ __global__ void __launch_bounds__(32 * NW, 1) teuk_step_resident_kernel(const __
       }
       __syncwarp();
       if (lane == 0) flag_set(verH + 4u * (unsigned)h, it + 1);
-      if (tap_q >= 0) tap_finish(p, tap_q, mode, n, lane, tap_wr, tap_wi);
     } else {
       // ---- full-step row in place (Eq. 4) ----
       const int tt = t - (rows + 1);

@@ -643,6 +643,27 @@ __device__ __forceinline__ void add_source(Row<V>& out, const TermSource<V>& s, 
   }
 }
 
+// The same with the radial profile values given (marching kernels: built once per 16-row chunk, one row per lane,
+// and fetched by shuffle) and the theta profiles in the table: all that is left per row is the loop over the terms.
+template <int V>
+__device__ __forceinline__ void add_source_row(Row<V>& out, const TermSource<V>& s, const StepParams& p,
+                                               const Profile3& pr) {
+  for (int t = 0; t < p.n_terms; ++t) {
+    const size_t ia = ((size_t)t * p.n_modes + s.mode) * p.n_samples + s.ks;
+    const double are = p.amp_re[ia], aim = p.amp_im[ia];
+    const double gr = p.dt * pick3(pr, p.term_or[t]);
+    const int kth = p.term_oth[t];
+#pragma unroll
+    for (int q = 0; q < V; ++q) {
+      const double gg = gr * s.tab[(kth * V + q) * 32 + s.lane];
+      out.c[2][q] = fma(are, gg, out.c[2][q]);
+      out.c[3][q] = fma(aim, gg, out.c[3][q]);
+    }
+  }
+}
+template <int V>
+__device__ __forceinline__ void add_source_row(Row<V>&, const StageSource<V>&, const StepParams&, const Profile3&) {}
+
 // Shared-memory doubles of one warp's theta-profile tables (two stages) in a TERMS instantiation of a marching kernel
 template <int V>
 struct TermTab {

@@ -188,7 +188,7 @@ __global__ void __launch_bounds__(128, (V == 2 ? TEUK_V2_BLOCKS : TEUK_MIN_BLOCK
   // starts in the chunk (read from the input level in global memory: same values as the register rows, same
   // summation order).  The marching iteration is then two stages, one TMA issue, one store and nothing else: a
   // short hot loop without cold branches in it.
-  double gprof = 0.0;
+  double gprof = 0.0, gprof1 = 0.0, gprof2 = 0.0;
   auto chunk_begin = [&](const int cb) {
     asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncwarp();
@@ -208,6 +208,22 @@ __global__ void __launch_bounds__(128, (V == 2 ? TEUK_V2_BLOCKS : TEUK_MIN_BLOCK
         g = p.dt * deposit_profile(p.source_kind, x - (hf ? src_h.xp : src_f.xp), p.sigma_r);
       }
       gprof = g;
+    }
+    if (TERMS && any_src) {    // multi-term deposit: the three radial profile values of this lane's row (0 outside the window)
+      const bool hf = lane < 16;
+      const int i = cb + (lane & 15);
+      const bool on = hf ? src_h.on : src_f.on;
+      const int ip = hf ? src_h.ip : src_f.ip;
+      Profile3 g3;
+      g3.d[0] = g3.d[1] = g3.d[2] = 0.0;
+      if (on && i < r1 && abs(i - ip) <= p.W) {
+        double x = __dadd_rn(p.rs_min, __dmul_rn((double)i, p.dx));
+        if (hf) x = __dadd_rn(x, __dmul_rn(0.5, p.dx));
+        g3 = deposit_profile3(p.source_kind, x - (hf ? src_h.xp : src_f.xp), p.sigma_r);
+      }
+      gprof = g3.d[0];
+      gprof1 = g3.d[1];
+      gprof2 = g3.d[2];
     }
     if (do_tap) {
       for (int q = 0; q < p.n_obs; ++q) {
@@ -275,7 +291,13 @@ __global__ void __launch_bounds__(128, (V == 2 ? TEUK_V2_BLOCKS : TEUK_MIN_BLOCK
       lw_stage<V, true>(A, B, A, rt_cur + (2 * o + 1) * RT_N, th, tau_h, tdx, Hn);
     }
     if (any_src) {
-      if constexpr (TERMS) add_source<V>(Hn, src_h, p, i, true);
+      if constexpr (TERMS) {
+        Profile3 pr;
+        pr.d[0] = __shfl_sync(FULL, gprof, o);
+        pr.d[1] = __shfl_sync(FULL, gprof1, o);
+        pr.d[2] = __shfl_sync(FULL, gprof2, o);
+        if (pr.d[0] != 0.0 || pr.d[1] != 0.0 || pr.d[2] != 0.0) add_source_row<V>(Hn, src_h, p, pr);
+      }
       else deposit(Hn, src_h, __shfl_sync(FULL, gprof, o));
     }
     if (VEC) {
@@ -289,7 +311,13 @@ __global__ void __launch_bounds__(128, (V == 2 ? TEUK_V2_BLOCKS : TEUK_MIN_BLOCK
     else
       lw_stage<V, false>(Hp, Hn, A, rt_cur + (2 * o) * RT_N, th, tau_f, tdx, out);
     if (any_src) {
-      if constexpr (TERMS) add_source<V>(out, src_f, p, i, false);
+      if constexpr (TERMS) {
+        Profile3 pr;
+        pr.d[0] = __shfl_sync(FULL, gprof, 16 + o);
+        pr.d[1] = __shfl_sync(FULL, gprof1, 16 + o);
+        pr.d[2] = __shfl_sync(FULL, gprof2, 16 + o);
+        if (pr.d[0] != 0.0 || pr.d[1] != 0.0 || pr.d[2] != 0.0) add_source_row<V>(out, src_f, p, pr);
+      }
       else deposit(out, src_f, __shfl_sync(FULL, gprof, 16 + o));
     }
     store_row<V, VEC>(out, uout + (size_t)i * row_stride, nth, j0, pay_lo, pay_hi);

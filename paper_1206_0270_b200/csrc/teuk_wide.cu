@@ -7,12 +7,8 @@
 // the largest bucket (profiles/r2_step_kernel_before_chunk.md).  With V = 2 the same code needs 162 registers and
 // runs 12 warps per SM.  Here every lane owns V = 2 columns and warp w of a group owns columns 64 w .. 64 w + 63;
 // the only data the warps of a group exchange are the two boundary columns of S_Phi per stage (the theta stencil
-// of PAPER.md:102 reaches one column), through shared memory.  A warp needs only its two NEIGHBOURS' columns, so
-// there is no group-wide barrier: every warp publishes a stage counter (st.release) after writing its columns, and
-// lane 0 / lane 31 -- the only lanes that read a neighbour's value -- poll the left / right neighbour's counter
-// (first version: one named barrier per stage for the whole group: 21 % of the stall samples with five warps per
-// row).  Everything else is private to a warp: its 64 columns of a row arrive by its own four TMA bulk copies (one
-// per component) in its own landing slots, its r-table chunks, its deposit profile.
+// of PAPER.md:102 reaches one column), through shared memory behind one named barrier per stage.  The same barrier
+// orders the hand-over of the TMA landing slots, which are per GROUP: one bulk copy per row, whatever the width.
 // Rows wider than 128 columns -- the paper's own grid has 304 -- no longer need theta segments with
 // recomputed halos (79 % useful lanes): 5 warps cover 320 columns (95 %).
 //
@@ -36,16 +32,8 @@ struct WideShape {
   static constexpr int BLOCKS = NWR == 2 ? 3 : (NWR == 3 ? 4 : (NWR == 4 ? 3 : 2));   // resident blocks per SM (<= 168 / 204 registers)
 };
 
-__device__ __forceinline__ void seq_publish(unsigned addr, unsigned v) {
-  asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
-}
-// bounded spin (see mbar_wait_u32): a lost neighbour becomes a reported CUDA error, not a hung GPU
-__device__ __forceinline__ void seq_wait(unsigned addr, unsigned v) {
-  unsigned got, tries = 0;
-  do {
-    asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(got) : "r"(addr) : "memory");
-    if ((int)(got - v) < 0 && ++tries > (1u << 26)) asm volatile("trap;");
-  } while ((int)(got - v) < 0);
+__device__ __forceinline__ void group_barrier(int id, int threads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
 
 }  // namespace
@@ -62,19 +50,18 @@ teuk_step_wide_kernel(const __grid_constant__ StepParams p) {
   const int mode = blockIdx.y;
   const int nth = p.n_theta, nr = p.n_r;
   __shared__ __align__(16) double s_rt[WARPS][2][RT_CHUNK_DOUBLES];
-  __shared__ __align__(8) unsigned long long s_bar[WARPS][NS];
+  __shared__ __align__(8) unsigned long long s_bar[GPB][NS];
   __shared__ __align__(16) double s_x[GPB][2][NWR][2][2];           // [parity][warp][left / right column][re, im]
-  __shared__ unsigned s_seq[GPB][NWR];                               // stages whose boundary columns warp w has published
-  extern __shared__ __align__(128) unsigned char s_dyn[];           // [WARPS][NS][4][64] doubles: TMA landing slots
-  if (lane == 0) {
+  extern __shared__ __align__(128) unsigned char s_dyn[];           // [GPB][NS][4 n_theta] doubles: TMA landing slots
+  if (w == 0 && lane == 0) {
 #pragma unroll
-    for (int q = 0; q < NS; ++q) mbar_init(&s_bar[wib][q], 1);
-    s_seq[grp][w] = 0u;
+    for (int q = 0; q < NS; ++q) mbar_init(&s_bar[grp][q], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
-  __syncthreads();                                                   // counters zeroed before any neighbour polls them
+  __syncthreads();                                                   // barriers initialised for every warp of the group
   if (slab >= p.n_slabs) return;                                     // the whole group leaves together
+  const int bar_id = 1 + grp;                                        // named barrier of this group (0 = __syncthreads)
   const int r0 = slab_first_row(p, slab);
   const int r1 = slab_first_row(p, slab + 1);
   const int j0 = w * 64 + lane * V;                                  // this lane's two columns (n_theta is even)
@@ -85,19 +72,12 @@ teuk_step_wide_kernel(const __grid_constant__ StepParams p) {
   const double* __restrict__ rtab = p.rtab + (size_t)mode * (2 * nr - 1) * RT_N;
   double* const rt_buf = &s_rt[wib][0][0];
   stage_rtab_chunk(rt_buf, rtab, 2 * r0, 2 * nr - 1, lane);
-  constexpr int SLOT_D = 4 * 64;                                     // doubles per landing slot: 4 components x 64 columns
-  double* const slot0 = reinterpret_cast<double*>(s_dyn) + (size_t)wib * NS * SLOT_D;
-  const unsigned slot0_u32 = smem_u32(slot0), bars_u32 = smem_u32(&s_bar[wib][0]);
-  const unsigned seg_bytes = (unsigned)(min(64, nth - w * 64) * (int)sizeof(double));   // this warp's columns of one component
-  auto issue_row = [&](int q) {                                      // this warp's part of row q lands in its slot q % NS
-    const unsigned bar = bars_u32 + 8u * (unsigned)(q % NS);
-    const unsigned dst = slot0_u32 + (unsigned)((q % NS) * SLOT_D * sizeof(double));
-    const double* src = uin + (size_t)q * row_stride + w * 64;
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(4u * seg_bytes) : "memory");
-#pragma unroll
-    for (int c = 0; c < 4; ++c)
-      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                   ::"r"(dst + (unsigned)(c * 64 * sizeof(double))), "l"(src + (size_t)c * nth), "r"(seg_bytes), "r"(bar) : "memory");
+  const unsigned row_bytes = (unsigned)(row_stride * sizeof(double));
+  double* const slot0 = reinterpret_cast<double*>(s_dyn) + (size_t)grp * NS * row_stride;
+  const unsigned slot0_u32 = smem_u32(slot0), bars_u32 = smem_u32(&s_bar[grp][0]);
+  auto issue_row = [&](int q) {                                      // row q lands in slot q % NS of the group
+    tma_load_row_u32(slot0_u32 + (unsigned)((q % NS) * row_stride * sizeof(double)), uin + (size_t)q * row_stride,
+                     row_bytes, bars_u32 + 8u * (unsigned)(q % NS));
   };
   const long long n = *p.d_base + p.k;                               // index of the input time level
 
@@ -165,45 +145,39 @@ teuk_step_wide_kernel(const __grid_constant__ StepParams p) {
   // Programmatic dependent launch: everything above reads nothing a step kernel writes (see teuk_step_kernel).
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  if (lane == 0) {
+  if (w == 0 && lane == 0) {
 #pragma unroll
     for (int q = 2; q <= NS; ++q)
       if (r0 + q <= r1) issue_row(r0 + q);
   }
-  __syncwarp();
 
-  // One stage across the group: S_Phi, exchange of its boundary columns with the two neighbour warps, then the rest
-  // of the stage.  Two buffers suffice: a warp writes the columns of stage k + 2 after its wait of stage k + 1, i.e.
-  // after both neighbours have published stage k + 1, which they do after their reads of stage k.
-  unsigned stage_no = 0;
-  const unsigned seq_u32 = smem_u32(&s_seq[grp][0]);
+  // One stage across the group: S_Phi, exchange of its boundary columns, then the rest of the stage.  The barrier is
+  // also what orders the landing slots: when a warp has passed the barrier of the half stage of iteration i, every
+  // warp of the group has finished iteration i - 1, including its copy of row i + 1 out of slot (i + 1) % NS.
+  int xpar = 0;
   auto stage = [&](auto half_tag, const Row<V>& A, const Row<V>& B, const Row<V>& base, const double* rec, double tau,
                    Row<V>& o_) {
     constexpr bool HALF = decltype(half_tag)::value;
     double sfr[V], sfi[V];
     lw_stage_sums<V>(A, B, sfr, sfi);
-    double* xs = &s_x[grp][stage_no & 1u][0][0][0];
+    double* xs = &s_x[grp][xpar][0][0][0];
     if (lane == 0) *reinterpret_cast<double2*>(xs + (w * 2 + 0) * 2) = make_double2(sfr[0], sfi[0]);
     if (lane == 31) *reinterpret_cast<double2*>(xs + (w * 2 + 1) * 2) = make_double2(sfr[V - 1], sfi[V - 1]);
-    __syncwarp();
-    stage_no += 1;
-    if (lane == 0) seq_publish(seq_u32 + 4u * (unsigned)w, stage_no);
+    group_barrier(bar_id, 32 * NWR);
     double nlr[V], nrr[V], nli[V], nri[V];
-    theta_neighbours<V, 0>(sfr, nlr, nrr, lane);     // the in-warp neighbours while the other warps catch up
+    theta_neighbours<V, 0>(sfr, nlr, nrr, lane);
     theta_neighbours<V, 0>(sfi, nli, nri, lane);
     if (lane == 0 && w > 0) {                        // left neighbour of this warp's first column
-      seq_wait(seq_u32 + 4u * (unsigned)(w - 1), stage_no);
       const double2 t = *reinterpret_cast<const double2*>(xs + ((w - 1) * 2 + 1) * 2);
       nlr[0] = t.x;
       nli[0] = t.y;
     }
     if (lane == 31 && w < NWR - 1) {                 // right neighbour of its last column
-      seq_wait(seq_u32 + 4u * (unsigned)(w + 1), stage_no);
       const double2 t = *reinterpret_cast<const double2*>(xs + ((w + 1) * 2 + 0) * 2);
       nrr[V - 1] = t.x;
       nri[V - 1] = t.y;
     }
-    __syncwarp();
+    xpar ^= 1;   // two buffers suffice: the next-but-one stage's writes come after the next stage's barrier
     lw_stage_body<V, HALF, ThetaTab<V>>(A, B, base, rec, th, tau, tdx, o_, sfr, sfi, nlr, nrr, nli, nri);
   };
 
@@ -218,7 +192,7 @@ teuk_step_wide_kernel(const __grid_constant__ StepParams p) {
   add_source<V>(hp, src_h, p, r0 - 1, true);
 
   const double* rt_cur = rt_buf;
-  double gprof = 0.0;
+  double gprof = 0.0, gprof1 = 0.0, gprof2 = 0.0;
   // Per-chunk work, outside the marching iteration (see teuk_step_kernel): r-table hand-over, the radial deposit
   // profile of the chunk's rows (lanes 0-15: half stage, lanes 16-31: full stage), taps of observers in the chunk.
   auto chunk_begin = [&](const int cb) {
@@ -240,6 +214,22 @@ teuk_step_wide_kernel(const __grid_constant__ StepParams p) {
         g = p.dt * deposit_profile(p.source_kind, x - (hf ? src_h.xp : src_f.xp), p.sigma_r);
       }
       gprof = g;
+    }
+    if (TERMS && any_src) {    // multi-term deposit: the three radial profile values of this lane's row (0 outside the window)
+      const bool hf = lane < 16;
+      const int i = cb + (lane & 15);
+      const bool on = hf ? src_h.on : src_f.on;
+      const int ip = hf ? src_h.ip : src_f.ip;
+      Profile3 g3;
+      g3.d[0] = g3.d[1] = g3.d[2] = 0.0;
+      if (on && i < r1 && abs(i - ip) <= p.W) {
+        double x = __dadd_rn(p.rs_min, __dmul_rn((double)i, p.dx));
+        if (hf) x = __dadd_rn(x, __dmul_rn(0.5, p.dx));
+        g3 = deposit_profile3(p.source_kind, x - (hf ? src_h.xp : src_f.xp), p.sigma_r);
+      }
+      gprof = g3.d[0];
+      gprof1 = g3.d[1];
+      gprof2 = g3.d[2];
     }
     if (do_tap)
       for (int q = 0; q < p.n_obs; ++q)
@@ -263,22 +253,32 @@ teuk_step_wide_kernel(const __grid_constant__ StepParams p) {
     const int o = (i - r0) & (RT_CH - 1);
     stage(std::true_type(), A, B, A, rt_cur + (2 * o + 1) * RT_N, tau_h, Hn);
     if (any_src) {
-      if constexpr (TERMS) add_source<V>(Hn, src_h, p, i, true);
+      if constexpr (TERMS) {
+        Profile3 pr;
+        pr.d[0] = __shfl_sync(FULL, gprof, o);
+        pr.d[1] = __shfl_sync(FULL, gprof1, o);
+        pr.d[2] = __shfl_sync(FULL, gprof2, o);
+        if (pr.d[0] != 0.0 || pr.d[1] != 0.0 || pr.d[2] != 0.0) add_source_row<V>(Hn, src_h, p, pr);
+      }
       else deposit(Hn, src_h, __shfl_sync(FULL, gprof, o));
     }
-    // B (row i + 1, copied out of slot (i + 1) % NS at the end of the last iteration) has been consumed by every
-    // lane of this warp: its slot may now receive row i + NS + 1
-    __syncwarp();
-    if (lane == 0 && i + NS + 1 <= r1) issue_row(i + NS + 1);
+    // every warp of the group is past the barrier of this half stage: slot (i + 1) % NS has been copied out by all
+    if (w == 0 && lane == 0 && i + NS + 1 <= r1) issue_row(i + NS + 1);
     stage(std::false_type(), Hp, Hn, A, rt_cur + (2 * o) * RT_N, tau_f, out);
     if (any_src) {
-      if constexpr (TERMS) add_source<V>(out, src_f, p, i, false);
+      if constexpr (TERMS) {
+        Profile3 pr;
+        pr.d[0] = __shfl_sync(FULL, gprof, 16 + o);
+        pr.d[1] = __shfl_sync(FULL, gprof1, 16 + o);
+        pr.d[2] = __shfl_sync(FULL, gprof2, 16 + o);
+        if (pr.d[0] != 0.0 || pr.d[1] != 0.0 || pr.d[2] != 0.0) add_source_row<V>(out, src_f, p, pr);
+      }
       else deposit(out, src_f, __shfl_sync(FULL, gprof, 16 + o));
     }
     store_row<V, true>(out, uout + (size_t)i * row_stride, nth, j0, 0, nth);
     if (i + 2 <= r1) {
       mbar_wait_u32(bars_u32 + 8u * (unsigned)((i + 2) % NS), (unsigned)((i - r0) / NS) & 1u);
-      lds_row<V>(A, slot0 + (size_t)((i + 2) % NS) * SLOT_D, 64, lane * V, lane_ok);
+      lds_row<V>(A, slot0 + (size_t)((i + 2) % NS) * row_stride, nth, j0, lane_ok);
     }
   };
   static_assert(RT_CH == 16, "chunk_begin keeps one chunk's deposit profile in the two halves of a warp");
@@ -330,8 +330,8 @@ template <int NWR, bool TERMS>
 static cudaError_t launch_wide(const StepParams& p, cudaStream_t st) {
   constexpr int GPB = WideShape<NWR>::GPB, WARPS = WideShape<NWR>::WARPS;
   dim3 grid((p.n_slabs + GPB - 1) / GPB, p.n_modes), block(32 * WARPS);
-  const size_t dyn = (size_t)WARPS * TEUK_SLOTS * 4 * 64 * sizeof(double);
-  const int dyn_max = (int)dyn;
+  const size_t dyn = (size_t)GPB * TEUK_SLOTS * 4 * p.n_theta * sizeof(double);
+  const int dyn_max = (int)((size_t)GPB * TEUK_SLOTS * 4 * 64 * NWR * sizeof(double));
   static bool attr_set[64] = {false};   // per device
   int dev_ = 0;
   cudaGetDevice(&dev_);
