@@ -26,7 +26,7 @@
 // interpolation conditions (P9), the waveform tap with an off-node observer against the interpolated weighted sum of
 // the state and a closed form on a field linear in x (P10), and the derivative profiles of the multi-term deposit
 // against exact-rational Lagrange derivatives, moment conditions and mpmath derivatives of the printed Gaussian
-// (P12).  (P11 pins the shared input generator, paper_1206_0270_b200/workloads.py.)  The paper prints no field
+// (P12).  (P11 pins the seeded input generator that both sides share.)  The paper prints no field
 // values: beyond those pins the numbers this file produces are "parity unpinned" by the paper; no function of this
 // file is without a pin of its own.
 //
