@@ -87,7 +87,7 @@ def refresh_traffic(csv_path, cfg):
 
 # FP64 instructions per point per iteration of the stage code (teuk_stage.cuh lw_stage, both stages), counted from
 # the executed-instruction column of the ncu source page of teuk_step_kernel<4,...> on config 5
-# (profiles/r2_sass_histogram.md): DFMA with three distinct register operands, other DFMA, DADD, DMUL.
+# (profiles/r2_step_kernel.md, profiles/r2_fp64_peak.md): DFMA with three distinct register operands, other DFMA, DADD, DMUL.
 FP64_MIX = {"dfma3": 46.4, "dfma2": 10.3, "dadd": 18.2, "dmul": 22.6}
 
 
